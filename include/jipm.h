@@ -1,0 +1,133 @@
+/* jipm.h -- C ABI of the B200-native batched interior-point NLP solver.
+ *
+ * What it computes: the interior-point iteration of arxiv 2606.26341 section IV applied to a
+ * batch of independent parametric NLPs
+ *        min f(x,theta)  s.t.  c(x,theta) = 0,  x_L < x < x_U          (eqs 1a-1c)
+ * that share f, c and the bounds and differ only in theta and the initial guess (eq 2).
+ * General inequalities enter through slack variables.  Each problem runs the barrier
+ * iteration (eqs 3-7) with the fallbacks of Table I that this
+ * build covers (backtracking, second-order correction, inertia correction, monotone barrier update,
+ * feasibility restoration) and a problem slot is refilled from the queue as soon as its problem ends
+ * (iteration-level batching).
+ *
+ * Decision vector ("stage order", n entries) and equality vector (m entries) of every family:
+ *        x = [ x_0 | u_0 x_1 s_1 | u_1 x_2 s_2 | ... | u_{N-1} x_N s_N ]
+ *        c = [ x_0 - xhat0 | dyn_1 g_1 | ... | dyn_N g_N ],  dyn_k = x_k - F(x_{k-1},u_{k-1}),  g_k = h(x_k) - s_k
+ * n = (N+1) nx + N nu + N ng,  m = (N+1) nx + N ng;  slacks s >= 0 carry the inequalities h(x_k) >= 0.
+ *
+ * Conventions: every pointer argument says HOST or DEVICE.  The caller owns all buffers; the library keeps
+ * no caller pointer after a call returns.  All work is enqueued on the stream given at create time and
+ * jipm_solve_batch returns after that work has completed.  Return value = call-level error code (0 = ok);
+ * per-problem outcomes are only in status_out.  There is no CPU fallback: without a CUDA device every
+ * compute entry returns JIPM_ERR_CUDA.
+ */
+#ifndef JIPM_H
+#define JIPM_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct jipm_solver jipm_solver; /* opaque, owned by the library */
+
+enum { JIPM_OK = 0, JIPM_ERR_ARG = 1, JIPM_ERR_DIM = 2, JIPM_ERR_BOUNDS = 3, JIPM_ERR_CUDA = 4, JIPM_ERR_NOMEM = 5 };
+enum { JIPM_FAM_POINTMASS2D = 0, JIPM_FAM_QUAD_TRACK = 1, JIPM_FAM_MULTIQUAD = 2, JIPM_FAM_QUAD_CLUTTER = 3 };
+enum { JIPM_ST_NOT_RUN = -1, JIPM_ST_SOLVED = 0, JIPM_ST_MAXITER = 1, JIPM_ST_LOCALLY_INFEASIBLE = 2,
+       JIPM_ST_RESTORATION_FAILED = 3, JIPM_ST_RESTO_AT_FEASIBLE_POINT = 4, JIPM_ST_NONFINITE = 5 };
+
+/* Problem family dimensions (BASELINE.json configs). */
+typedef struct {
+    int32_t horizon_N;   /* control intervals; N+1 state knots */
+    int32_t n_agents;    /* 1 except JIPM_FAM_MULTIQUAD */
+    int32_t n_obstacles; /* obstacles per knot (ignored by JIPM_FAM_MULTIQUAD: pair constraints) */
+    double dt;
+} jipm_family_dims;
+
+/* Algorithmic constants.  The paper gives none (it defers to its ref. [7]); the
+ * defaults are the readings listed in DESIGN.md "Readings". */
+typedef struct {
+    double tol, mu_init, kappa_eps, kappa_mu, theta_mu, tau_min, s_max, kappa_sigma;
+    double kappa_1, kappa_2, bound_relax_factor, bound_mult_init, lam_init_max, kappa_d;
+    double gamma_theta, gamma_phi, eta_phi, delta, s_theta, s_phi, gamma_alpha;
+    double theta_max_fact, theta_min_fact, alpha_red, kappa_soc;
+    double delta_w_min, delta_w_0, delta_w_max, kappa_w_minus, kappa_w_plus, kappa_w_plus_first;
+    double delta_c_bar, kappa_c, residual_ratio_max, rho_resto, kappa_resto, z_reset_threshold;
+    int32_t max_iter, max_backtrack, max_soc, refine_min, refine_max, max_mu_updates;
+    int32_t init_slacks, enable_restoration;
+} jipm_options;
+
+/* Fill *o with the defaults.  o: HOST.  Returns JIPM_ERR_ARG if o is NULL. */
+int jipm_default_options(jipm_options* o);
+
+/* Internal sizes (slacks included) of a family.  n, m, n_theta: HOST out.  JIPM_ERR_DIM on a bad family/dims. */
+int jipm_family_sizes(int family, const jipm_family_dims* d, int64_t* n, int64_t* m, int64_t* n_theta);
+
+/* Create a solver for one family.
+ *   n, m            must equal jipm_family_sizes (else JIPM_ERR_DIM)
+ *   x_L, x_U        HOST [n], +-INFINITY = no bound, shared by all problems; x_L >= x_U on a
+ *                   component -> JIPM_ERR_BOUNDS (PAPER.md:63 needs a strict interior).  Copied.
+ *   opts            HOST or NULL (defaults).  Copied.
+ *   resident_slots  R = problem slots in flight (one warp per slot); 0 -> library picks (fills the GPU).
+ *   cuda_stream     cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = default stream. */
+int jipm_create(jipm_solver** out, int family, const jipm_family_dims* d, int64_t n, int64_t m,
+                const double* x_L, const double* x_U, const jipm_options* opts, int64_t resident_slots,
+                void* cuda_stream);
+
+/* Solve P problems.  Outputs are indexed by problem id (row of the inputs), never by slot;
+ * the result of a row does not depend on P, R or row order.
+ *   x0       DEVICE [P x n]  initial guess (slack entries are overwritten when opts.init_slacks)
+ *   params   DEVICE [P x n_theta]
+ *   x_out    DEVICE [P x n];  lam_out DEVICE [P x m] (y_c, sign of eq 4)
+ *   zL_out, zU_out  DEVICE [P x n] (0 where no bound) or NULL
+ *   status_out, iters_out  DEVICE [P] int32 */
+int jipm_solve_batch(jipm_solver* s, int64_t P, const double* x0, const double* params, double* x_out,
+                     double* lam_out, double* zL_out, double* zU_out, int32_t* status_out, int32_t* iters_out);
+
+/* Same call with HOST buffers: copies in, solves, copies out (all on the solver's stream). */
+int jipm_solve_batch_host(jipm_solver* s, int64_t P, const double* x0, const double* params, double* x_out,
+                          double* lam_out, double* zL_out, double* zU_out, int32_t* status_out,
+                          int32_t* iters_out);
+
+/* Free everything.  NULL is a no-op. */
+int jipm_destroy(jipm_solver* s);
+
+/* Last error text of the calling thread (static storage, never NULL). */
+const char* jipm_last_error(void);
+
+/* ---- statistics of the last jipm_solve_batch (HOST out) ------------------------------------------------
+ * stats[0] total IPM iterations, [1] factorisations, [2] KKT solves, [3] derivative evaluations,
+ * [4] f/c-only evaluations, [5] slots launched, [6] kernel launches, [7] restoration iterations. */
+int jipm_last_stats(jipm_solver* s, int64_t* stats, int64_t n_stats);
+
+/* ---- debug / parity-test entries (load a state, step once, compare) ------------------
+ * Decision trace: per problem, per iteration JIPM_TRACE_W doubles:
+ *   [0] mode (0 regular, 1 restoration) [1] #factorisations [2] delta_w [3] delta_c [4] #refinements
+ *   [5] kind (0 newton, 1 soc, 2 ls_fail->resto, 3 ic_fail->resto, 4 terminal) [6] #backtracks [7] #soc
+ *   [8] alpha [9] alpha_z [10] f-type? [11] #mu updates [12] E0 at iteration start [13] mu used
+ *   [14] theta_k [15] phi_k */
+#define JIPM_TRACE_W 16
+/* Enable tracing for the next solves: trace DEVICE [P x max_records x JIPM_TRACE_W] (or NULL to disable). */
+int jipm_debug_set_trace(jipm_solver* s, double* trace, int64_t max_records);
+
+/* Layout of the debug state vector used by jipm_debug_step: HOST out, offsets in doubles:
+ * lay[0]=len, [1]=x, [2]=y, [3]=zL, [4]=zU, [5]=scalars(mu,tau,delta_w_last,theta_min,theta_max,k,status,nfilt),
+ * [6]=filter (32 pairs theta,phi), [7]=dx, [8]=dy, [9]=dzL, [10]=dzU (step of the last iteration),
+ * [11]=grad f, [12]=c, [13]=J blocks [N][nx][nx+nu], [14]=W blocks [N][nz][nz] then [nx][nx] */
+int jipm_debug_state_layout(jipm_solver* s, int64_t* lay, int64_t n_lay);
+
+/* Load P states (DEVICE [P x len], regular mode), run n_steps iterations each (stops early on a final
+ * status), write the states back in place (step and derivative fields filled from the last iteration). */
+int jipm_debug_step(jipm_solver* s, int64_t P, const double* params, double* state, int64_t n_steps);
+
+/* Step I only: initialise P problems from (x0, params) and write their states (DEVICE [P x len]). */
+int jipm_debug_init(jipm_solver* s, int64_t P, const double* x0, const double* params, double* state);
+
+/* FP64 FMA microbenchmark (roofline denominator): runs dependent-free DFMA chains on all SMs and returns
+ * the achieved TFLOP/s in *tflops (HOST out). */
+int jipm_bench_fp64_peak(void* cuda_stream, double* tflops);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* JIPM_H */

@@ -1,0 +1,235 @@
+// iter.cuh -- the fused interior-point iteration (Table I) for one problem slot
+// owned by one warp, plus Step I (initialisation) and the slot refill loop.
+// Step names (I-*, A-*, IC-*) follow SURVEY.md section 8(c) / DESIGN.md.
+#pragma once
+#include "core.cuh"
+#include "derivs.cuh"
+#include "kkt.cuh"
+
+namespace jipm {
+
+enum { KIND_NEWTON = 0, KIND_SOC = 1, KIND_LS_FAIL = 2, KIND_IC_FAIL = 3, KIND_TERMINAL = 4 };
+
+template <class C>
+struct Solver {
+    using X = Ctx<C>;
+    using K = Kkt<C>;
+    static constexpr int NX = C::NX, NU = C::NU, NZ = C::NZ, PD = C::PD, AX = C::AX, NA = C::NA;
+    X& c;
+    const Args& A;
+    const Pb& pb;
+    const Lay& L;
+    const jipm_options& o;
+    int lane;
+    // warp-uniform scalar state of the problem in this slot
+    double mu, tau, dw_last, theta_min, theta_max, f, theta, cmax;
+    int k, status, nfilt, nrec;
+    long long pid;
+    unsigned n_fact, n_solve, n_deriv, n_fc, n_iter;
+
+    __device__ Solver(X& c_, const Args& A_) : c(c_), A(A_), pb(A_.pb), L(A_.L), o(A_.o), lane(c_.lane) {
+        n_fact = n_solve = n_deriv = n_fc = n_iter = 0;
+    }
+    __device__ __forceinline__ double* V(int off) const { return c.ws + off; }
+    __device__ __forceinline__ bool hasL(int i) const { return pb.xL[i] > -INFINITY; }
+    __device__ __forceinline__ bool hasU(int i) const { return pb.xU[i] < INFINITY; }
+
+    // barrier objective (3) with the one-sided damping term; NaN outside the interior
+    __device__ double phi(const double* x, double fv, double mu_) const {
+        double s = 0.0;
+        int badpt = 0;
+        for (int i = lane; i < pb.n; i += 32) {
+            const double l = pb.xL[i], u = pb.xU[i], xi = x[i];
+            const bool hl = l > -INFINITY, hu = u < INFINITY;
+            if (hl) {
+                const double sl = xi - l;
+                if (!(sl > 0.0)) badpt = 1;
+                s -= mu_ * log(sl);
+                if (!hu) s += o.kappa_d * mu_ * sl;
+            }
+            if (hu) {
+                const double su = u - xi;
+                if (!(su > 0.0)) badpt = 1;
+                s -= mu_ * log(su);
+                if (!hl) s += o.kappa_d * mu_ * su;
+            }
+        }
+        s = wsum(s);
+        if (wor(badpt)) return NAN;
+        return fv + s;
+    }
+
+    // fraction to the boundary (PAPER.md:148 fn 2) on the primal step
+    __device__ double ftb_primal(const double* x, const double* dx, double tau_) const {
+        double a = 1.0;
+        for (int i = lane; i < pb.n; i += 32) {
+            const double l = pb.xL[i], u = pb.xU[i], d = dx[i];
+            if (l > -INFINITY && d < 0.0) a = fmin(a, -tau_ * (x[i] - l) / d);
+            if (u < INFINITY && d > 0.0) a = fmin(a, tau_ * (u - x[i]) / d);
+        }
+        return wmin(a);
+    }
+    __device__ double ftb_dual(const double* zL, const double* zU, const double* dzL, const double* dzU,
+                               double tau_) const {
+        double a = 1.0;
+        for (int i = lane; i < pb.n; i += 32) {
+            if (hasL(i) && dzL[i] < 0.0) a = fmin(a, -tau_ * zL[i] / dzL[i]);
+            if (hasU(i) && dzU[i] < 0.0) a = fmin(a, -tau_ * zU[i] / dzU[i]);
+        }
+        return wmin(a);
+    }
+
+    // optimality error E_mu from the dual residual base in b1 (= grad f + A^T y - zL + zU)
+    __device__ double opt_error(double mu_, double sd, double sc) const {
+        const double* x = V(L.x); const double* zL = V(L.zL); const double* zU = V(L.zU); const double* rdb = V(L.b1);
+        double ed = 0.0, es = 0.0;
+        for (int i = lane; i < pb.n; i += 32) {
+            const double l = pb.xL[i], u = pb.xU[i];
+            const bool hl = l > -INFINITY, hu = u < INFINITY;
+            double dmp = 0.0;
+            if (hl && !hu) dmp = o.kappa_d * mu_;
+            if (hu && !hl) dmp = -o.kappa_d * mu_;
+            ed = fmax(ed, fabs(rdb[i] + dmp));
+            if (hl) es = fmax(es, fabs((x[i] - l) * zL[i] - mu_));
+            if (hu) es = fmax(es, fabs((u - x[i]) * zU[i] - mu_));
+        }
+        ed = wmax(ed); es = wmax(es);
+        return fmax(fmax(ed / sd, cmax), es / sc);
+    }
+
+    // filter ([7] sec 2.3): entries (theta_j, phi_j) in the workspace
+    __device__ bool in_filter(double th_t, double ph_t) const {
+        if (th_t >= theta_max) return true;
+        const double* F = V(L.filt);
+        int hit = 0;
+        for (int j = lane; j < nfilt; j += 32) hit |= (th_t >= F[2 * j] && ph_t >= F[2 * j + 1]);
+        return wor(hit);
+    }
+    __device__ void filter_add(double th_e, double ph_e) {
+        double* F = V(L.filt);
+        const int slot = (nfilt < MAX_FILTER) ? nfilt : (nfilt % MAX_FILTER);  // overflow: overwrite the oldest
+        if (lane == 0) { F[2 * slot] = th_e; F[2 * slot + 1] = ph_e; }
+        if (nfilt < MAX_FILTER) nfilt++;
+        __syncwarp();
+    }
+    __device__ bool switching(double alpha, double g, double theta_k) const {
+        return g < 0.0 && alpha * pow(-g, o.s_phi) > o.delta * pow(theta_k, o.s_theta);
+    }
+    __device__ bool armijo(double phi_t, double phi_k, double alpha, double g) const {
+        return phi_t - phi_k - 10.0 * EPS_MACH * fabs(phi_k) <= o.eta_phi * alpha * g;
+    }
+    __device__ bool acceptable(double th_t, double ph_t, double th_k, double ph_k, double alpha, double g) const {
+        if (!(isfinite(th_t) && isfinite(ph_t))) return false;
+        if (in_filter(th_t, ph_t)) return false;
+        if (th_k <= theta_min && switching(alpha, g, th_k)) return armijo(ph_t, ph_k, alpha, g);
+        return th_t <= (1.0 - o.gamma_theta) * th_k ||
+               ph_t - ph_k - 10.0 * EPS_MACH * fabs(ph_k) <= -o.gamma_phi * th_k;
+    }
+
+    // ---- linear algebra of one iteration ---------------------------------------------------------------
+    // Sig = zL/sL + zU/sU + Hd
+    __device__ void set_sigma(double dw, double dc) const {
+        const double* x = V(L.x); const double* zL = V(L.zL); const double* zU = V(L.zU);
+        double* Sig = V(L.Sig); double* Hd = V(L.Hd); double* Dc = V(L.Dc);
+        for (int i = lane; i < pb.n; i += 32) {
+            const double l = pb.xL[i], u = pb.xU[i];
+            double s = dw;
+            if (l > -INFINITY) s += zL[i] / (x[i] - l);
+            if (u < INFINITY) s += zU[i] / (u - x[i]);
+            Sig[i] = s; Hd[i] = dw;
+        }
+        for (int i = lane; i < pb.m; i += 32) Dc[i] = dc;
+        __syncwarp();
+    }
+
+    // solve (6) through (7) + the Delta z recovery of PAPER.md:110 for rhs (b1,b2,b3,b4) -> (d1..d4)
+    __device__ void reduced_solve(const double* b1, const double* b2, const double* b3, const double* b4,
+                                  double* d1, double* d2, double* d3, double* d4) {
+        const double* x = V(L.x); const double* zL = V(L.zL); const double* zU = V(L.zU);
+        double* rr = V(L.rr);
+        for (int i = lane; i < pb.n; i += 32) {
+            const double l = pb.xL[i], u = pb.xU[i];
+            double r = b1[i];
+            if (l > -INFINITY) r += b3[i] / (x[i] - l);
+            if (u < INFINITY) r -= b4[i] / (u - x[i]);
+            rr[i] = r;
+        }
+        __syncwarp();
+        K::solve(c, rr, b2, d1, d2);
+        n_solve++;
+        for (int i = lane; i < pb.n; i += 32) {
+            const double l = pb.xL[i], u = pb.xU[i];
+            d3[i] = (l > -INFINITY) ? (b3[i] - zL[i] * d1[i]) / (x[i] - l) : 0.0;
+            d4[i] = (u < INFINITY) ? (b4[i] + zU[i] * d1[i]) / (u - x[i]) : 0.0;
+        }
+        __syncwarp();
+    }
+
+    // residual of the unreduced system (6): r = b - M d; returns ||r||_inf; dnorm = ||d||_inf
+    __device__ double full_residual(const double* b1, const double* b2, const double* b3, const double* b4,
+                                    const double* d1, const double* d2, const double* d3, const double* d4,
+                                    double& dnorm) const {
+        const double* x = V(L.x); const double* zL = V(L.zL); const double* zU = V(L.zU);
+        const double* Hd = V(L.Hd); const double* Dc = V(L.Dc);
+        double* r1 = V(L.r1); double* r2 = V(L.r2); double* r3 = V(L.r3); double* r4 = V(L.r4);
+        double rn = 0.0, dn = 0.0;
+        for (int i = lane; i < pb.n; i += 32) {
+            const double l = pb.xL[i], u = pb.xU[i];
+            const double lhs1 = c.W_entry(d1, i) + Hd[i] * d1[i] + c.AT_entry(d2, i) - d3[i] + d4[i];
+            const double v1 = b1[i] - lhs1;
+            r1[i] = v1; rn = fmax(rn, fabs(v1));
+            double v3 = 0.0, v4 = 0.0;
+            if (l > -INFINITY) v3 = b3[i] - (zL[i] * d1[i] + (x[i] - l) * d3[i]);
+            if (u < INFINITY) v4 = b4[i] - (-zU[i] * d1[i] + (u - x[i]) * d4[i]);
+            r3[i] = v3; r4[i] = v4;
+            rn = fmax(rn, fmax(fabs(v3), fabs(v4)));
+            dn = fmax(dn, fmax(fabs(d1[i]), fmax(fabs(d3[i]), fabs(d4[i]))));
+        }
+        c.A_mul(d1, r2);
+        for (int i = lane; i < pb.m; i += 32) {
+            const double v2 = b2[i] - (r2[i] - Dc[i] * d2[i]);
+            r2[i] = v2; rn = fmax(rn, fabs(v2)); dn = fmax(dn, fabs(d2[i]));
+        }
+        __syncwarp();
+        dnorm = wmax(dn);
+        return wmax(rn);
+    }
+
+    // solve (6) with iterative refinement on the unreduced system (reading S-7); returns #refinements
+    __device__ int solve_full(const double* b1, const double* b2, const double* b3, const double* b4,
+                              double* d1, double* d2, double* d3, double* d4) {
+        reduced_solve(b1, b2, b3, b4, d1, d2, d3, d4);
+        double bn = 0.0;
+        for (int i = lane; i < pb.n; i += 32) bn = fmax(bn, fmax(fabs(b1[i]), fmax(fabs(b3[i]), fabs(b4[i]))));
+        for (int i = lane; i < pb.m; i += 32) bn = fmax(bn, fabs(b2[i]));
+        bn = wmax(bn);
+        int nref = 0;
+        double* e1 = V(L.e1); double* e2 = V(L.e2); double* e3 = V(L.e3); double* e4 = V(L.e4);
+        while (nref < o.refine_max) {
+            double dn;
+            const double rn = full_residual(b1, b2, b3, b4, d1, d2, d3, d4, dn);
+            if (nref >= o.refine_min && rn <= o.residual_ratio_max * (bn + dn)) break;
+            reduced_solve(V(L.r1), V(L.r2), V(L.r3), V(L.r4), e1, e2, e3, e4);
+            for (int i = lane; i < pb.n; i += 32) { d1[i] += e1[i]; d3[i] += e3[i]; d4[i] += e4[i]; }
+            for (int i = lane; i < pb.m; i += 32) d2[i] += e2[i];
+            __syncwarp();
+            nref++;
+        }
+        return nref;
+    }
+
+    __device__ void trace_put(const double* rec) {
+        if (A.trace != nullptr && nrec < A.trace_cap && lane < JIPM_TRACE_W)
+            A.trace[(pid * A.trace_cap + nrec) * JIPM_TRACE_W + lane] = rec[lane];
+        nrec++;
+    }
+
+    __device__ void init_problem(long long id);
+    __device__ void iterate();
+    __device__ void enter_restoration(double* rec, int kind);
+    __device__ void write_outputs();
+    __device__ void dbg_load(const double* st);
+    __device__ void dbg_store(double* st);
+};
+
+}  // namespace jipm

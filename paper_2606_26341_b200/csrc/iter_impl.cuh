@@ -1,0 +1,305 @@
+// iter_impl.cuh -- Step I (initialise), Step A (one iteration) and the persistent slot kernel.
+#pragma once
+#include "iter.cuh"
+
+namespace jipm {
+
+// ---- Step I: slack init, interior push, z0 = 1, least-squares y0, mu0, filter bounds ------
+template <class C>
+__device__ void Solver<C>::init_problem(long long id) {
+    pid = id;
+    c.th = A.th + id * pb.nth;
+    const double* th = c.th;
+    const int N = pb.N;
+    double* x = V(L.x); double* y = V(L.y); double* zL = V(L.zL); double* zU = V(L.zU);
+    const double* x0 = A.x0 + id * pb.n;
+    for (int i = lane; i < pb.n; i += 32) x[i] = x0[i];
+    // cost targets per knot / agent
+    double* tgt = V(L.tgt);
+    for (int it = lane; it < (N + 1) * NA; it += 32) {
+        const int kk = it / NA, a = it % NA;
+        if (pb.family == JIPM_FAM_QUAD_TRACK) {
+            const double rho = th[12], phase = th[13];
+            const double ang = phase + 1.5 * (kk * pb.dt) / rho;
+            tgt[it * PD + 0] = rho * cos(ang); tgt[it * PD + 1] = rho * sin(ang);
+            if (PD > 2) tgt[it * PD + 2] = 0.0;
+        } else {
+            const double* gl = th + pb.th_goal + PD * a;
+#pragma unroll
+            for (int i = 0; i < PD; ++i) tgt[it * PD + i] = gl[i];
+        }
+    }
+    if (NA > 1) {
+        for (int it = lane; it < N * NX * NZ; it += 32) V(L.J)[it] = 0.0;
+    }
+    __syncwarp();
+    if (o.init_slacks) {  // I-2
+        for (int it = lane; it < N * pb.ng; it += 32) {
+            const int kk = it / pb.ng + 1, j = it % pb.ng;
+            x[c.is(kk) + j] = c.ineq_val(x, kk, j);
+        }
+        __syncwarp();
+    }
+    for (int i = lane; i < pb.n; i += 32) {  // I-3 push into the interior, I-4 z0
+        const double l = pb.xL[i], u = pb.xU[i];
+        const bool hl = l > -INFINITY, hu = u < INFINITY;
+        double xi = x[i];
+        if (hl && hu) {
+            const double pl = fmin(o.kappa_1 * fmax(1.0, fabs(l)), o.kappa_2 * (u - l));
+            const double pu = fmin(o.kappa_1 * fmax(1.0, fabs(u)), o.kappa_2 * (u - l));
+            xi = fmin(fmax(xi, l + pl), u - pu);
+        } else if (hl) xi = fmax(xi, l + o.kappa_1 * fmax(1.0, fabs(l)));
+        else if (hu) xi = fmin(xi, u - o.kappa_1 * fmax(1.0, fabs(u)));
+        x[i] = xi;
+        zL[i] = hl ? o.bound_mult_init : 0.0;
+        zU[i] = hu ? o.bound_mult_init : 0.0;
+    }
+    for (int i = lane; i < pb.m; i += 32) y[i] = 0.0;
+    __syncwarp();
+    // I-5 least-squares multipliers: [[I, A^T],[A, 0]] [w; y] = -[grad f - zL + zU; 0]
+    c.eval_derivs(x, y, 1.0);
+    n_deriv++;
+    {
+        double* Sig = V(L.Sig); double* Hd = V(L.Hd); double* Dc = V(L.Dc);
+        double* rr = V(L.rr); double* b2 = V(L.b2); const double* g = V(L.g);
+        for (int i = lane; i < pb.n; i += 32) { Sig[i] = 1.0; Hd[i] = 0.0; rr[i] = -(g[i] - zL[i] + zU[i]); }
+        for (int i = lane; i < pb.m; i += 32) { Dc[i] = 0.0; b2[i] = 0.0; }
+        __syncwarp();
+        int nz;
+        const int bad = K::factor(c, nz, false);
+        n_fact++;
+        K::solve(c, rr, b2, V(L.dx), V(L.dy));
+        n_solve++;
+        const double* dy = V(L.dy);
+        double ym = 0.0, ys = 0.0;
+        for (int i = lane; i < pb.m; i += 32) { ym = fmax(ym, fabs(dy[i])); ys += dy[i]; }
+        ym = wmax(ym); ys = wsum(ys);
+        const bool okls = bad == 0 && isfinite(ys) && ym <= o.lam_init_max;
+        for (int i = lane; i < pb.m; i += 32) y[i] = okls ? dy[i] : 0.0;
+        __syncwarp();
+    }
+    mu = o.mu_init;  // I-6
+    tau = fmax(o.tau_min, 1.0 - mu);
+    dw_last = 0.0;
+    bool fin;
+    f = c.eval_fc(x, V(L.c), theta, cmax, fin);  // I-7
+    n_fc++;
+    theta_max = o.theta_max_fact * fmax(1.0, theta);
+    theta_min = o.theta_min_fact * fmax(1.0, theta);
+    nfilt = 0; k = 0; nrec = 0;
+    status = fin ? JIPM_ST_NOT_RUN : JIPM_ST_NONFINITE;
+}
+
+// Restoration entry (Table I row 6).  [round-1 state: the fused restoration mode is not
+// built yet -- the problem ends with RESTORATION_FAILED; DESIGN.md "Status".]
+template <class C>
+__device__ void Solver<C>::enter_restoration(double* rec, int kind) {
+    rec[5] = kind;
+    if (theta < o.tol) status = JIPM_ST_RESTO_AT_FEASIBLE_POINT;
+    else status = JIPM_ST_RESTORATION_FAILED;
+    rec[12] = rec[12];
+    k += 1;
+}
+
+// ---- Step A: one iteration ----------------------------------------------------------------------------------
+template <class C>
+__device__ void Solver<C>::iterate() {
+    double* x = V(L.x); double* y = V(L.y); double* zL = V(L.zL); double* zU = V(L.zU);
+    double* cv = V(L.c); const double* g = V(L.g);
+    double* b1 = V(L.b1); double* b2 = V(L.b2); double* b3 = V(L.b3); double* b4 = V(L.b4);
+    double* dx = V(L.dx); double* dy = V(L.dy); double* dzL = V(L.dzL); double* dzU = V(L.dzU);
+    double rec[JIPM_TRACE_W];
+#pragma unroll
+    for (int i = 0; i < JIPM_TRACE_W; ++i) rec[i] = 0.0;
+    n_iter++;
+    // A-1 derivatives at (x, y)
+    c.eval_derivs(x, y, 1.0);
+    n_deriv++;
+    // dual residual base rdb = grad f + A^T y - zL + zU  (into b1), multiplier sums for the scaling s_d, s_c
+    double ysum = 0.0, zsum = 0.0, chk = 0.0;
+    for (int i = lane; i < pb.n; i += 32) {
+        const double v = g[i] + c.AT_entry(y, i) - zL[i] + zU[i];
+        b1[i] = v; chk += v;
+        zsum += fabs(zL[i]) + fabs(zU[i]);
+    }
+    for (int i = lane; i < pb.m; i += 32) ysum += fabs(y[i]);
+    ysum = wsum(ysum); zsum = wsum(zsum); chk = wsum(chk);
+    __syncwarp();
+    if (!isfinite(chk) || !isfinite(f) || !isfinite(theta)) {
+        status = JIPM_ST_NONFINITE; rec[5] = KIND_TERMINAL; trace_put(rec); return;
+    }
+    const int nz = pb.nL + pb.nU;
+    const double sd = (pb.m + nz > 0) ? fmax(o.s_max, (ysum + zsum) / (pb.m + nz)) / o.s_max : 1.0;
+    const double sc = (nz > 0) ? fmax(o.s_max, zsum / nz) / o.s_max : 1.0;
+    // A-2 termination
+    const double e0 = opt_error(0.0, sd, sc);
+    rec[12] = e0;
+    if (e0 <= o.tol) { status = JIPM_ST_SOLVED; rec[5] = KIND_TERMINAL; trace_put(rec); return; }
+    if (k >= o.max_iter) { status = JIPM_ST_MAXITER; rec[5] = KIND_TERMINAL; trace_put(rec); return; }
+    // A-3 monotone barrier update (Table I row 7)
+    int nmu = 0;
+    const double mu_min = o.tol / 10.0;
+    while (nmu < o.max_mu_updates && mu > mu_min && opt_error(mu, sd, sc) <= o.kappa_eps * mu) {
+        mu = fmax(mu_min, fmin(o.kappa_mu * mu, pow(mu, o.theta_mu)));
+        tau = fmax(o.tau_min, 1.0 - mu);
+        nfilt = 0;
+        nmu++;
+    }
+    rec[11] = nmu; rec[13] = mu;
+    // A-4 search direction with inertia correction (Algorithm IC)
+    int nfact = 0, nzero = 0;
+    double dw = 0.0, dc = 0.0;
+    bool ic_ok;
+    set_sigma(0.0, 0.0);
+    int bad = K::factor(c, nzero); nfact++;  // IC-1
+    ic_ok = (bad == 0);
+    if (!ic_ok) {
+        dc = (nzero > 0) ? o.delta_c_bar * pow(mu, o.kappa_c) : 0.0;                               // IC-2
+        dw = (dw_last == 0.0) ? o.delta_w_0 : fmax(o.delta_w_min, o.kappa_w_minus * dw_last);      // IC-3
+        while (true) {
+            set_sigma(dw, dc);
+            bad = K::factor(c, nzero); nfact++;                                                     // IC-4
+            if (bad == 0) { ic_ok = true; break; }
+            dw *= (dw_last == 0.0) ? o.kappa_w_plus_first : o.kappa_w_plus;                         // IC-5
+            if (dw > o.delta_w_max) break;                                                          // IC-6
+        }
+    }
+    n_fact += nfact;
+    rec[1] = nfact; rec[2] = dw; rec[3] = dc; rec[14] = theta;
+    if (!ic_ok) { enter_restoration(rec, KIND_IC_FAIL); trace_put(rec); return; }
+    if (dw > 0.0) dw_last = dw;
+    // right-hand side of (6)
+    double gd_part = 0.0;
+    for (int i = lane; i < pb.n; i += 32) {
+        const double l = pb.xL[i], u = pb.xU[i];
+        const bool hl = l > -INFINITY, hu = u < INFINITY;
+        double dmp = 0.0;
+        if (hl && !hu) dmp = o.kappa_d * mu;
+        if (hu && !hl) dmp = -o.kappa_d * mu;
+        b1[i] = -(b1[i] + dmp);
+        b3[i] = hl ? mu - (x[i] - l) * zL[i] : 0.0;
+        b4[i] = hu ? mu - (u - x[i]) * zU[i] : 0.0;
+    }
+    for (int i = lane; i < pb.m; i += 32) b2[i] = -cv[i];
+    __syncwarp();
+    const int nref = solve_full(b1, b2, b3, b4, dx, dy, dzL, dzU);
+    rec[4] = nref;
+    // A-5 filter line search
+    for (int i = lane; i < pb.n; i += 32) {
+        const double l = pb.xL[i], u = pb.xU[i];
+        const bool hl = l > -INFINITY, hu = u < INFINITY;
+        double gp = g[i];
+        if (hl) gp -= mu / (x[i] - l);
+        if (hu) gp += mu / (u - x[i]);
+        if (hl && !hu) gp += o.kappa_d * mu;
+        if (hu && !hl) gp -= o.kappa_d * mu;
+        gd_part += gp * dx[i];
+    }
+    const double gd = wsum(gd_part);
+    const double theta_k = theta;
+    const double phi_k = phi(x, f, mu);
+    rec[15] = phi_k;
+    const double a_max = ftb_primal(x, dx, tau);
+    double a_min;
+    if (gd < 0.0 && theta_k <= theta_min)
+        a_min = o.gamma_alpha * fmin(fmin(o.gamma_theta, o.gamma_phi * theta_k / (-gd)),
+                                     o.delta * pow(theta_k, o.s_theta) / pow(-gd, o.s_phi));
+    else if (gd < 0.0) a_min = o.gamma_alpha * fmin(o.gamma_theta, o.gamma_phi * theta_k / (-gd));
+    else a_min = o.gamma_alpha * o.gamma_theta;
+    double* xt = V(L.xt); double* ct = V(L.ct);
+    double alpha = a_max, alpha_acc = 0.0, phi_acc = 0.0, f_acc = 0.0, th_acc = 0.0, cm_acc = 0.0;
+    int ntrial = 0, nsoc = 0, acc = -1;  // acc: 0 newton, 1 soc
+    while (true) {
+        for (int i = lane; i < pb.n; i += 32) xt[i] = x[i] + alpha * dx[i];
+        __syncwarp();
+        double th_t, cm_t; bool fin;
+        const double f_t = c.eval_fc(xt, ct, th_t, cm_t, fin);
+        n_fc++;
+        const double ph_t = phi(xt, f_t, mu);
+        if (acceptable(th_t, ph_t, theta_k, phi_k, alpha, gd)) {
+            acc = 0; alpha_acc = alpha; phi_acc = ph_t; f_acc = f_t; th_acc = th_t; cm_acc = cm_t;
+            break;
+        }
+        if (ntrial == 0 && isfinite(th_t) && th_t >= theta_k && o.max_soc > 0) {
+            // second-order correction (Table I row 2)
+            double* csoc = V(L.csoc); double* bs2 = V(L.bs2);
+            double* sx = V(L.sx); double* sy = V(L.sy); double* szL = V(L.szL); double* szU = V(L.szU);
+            for (int i = lane; i < pb.m; i += 32) csoc[i] = alpha * cv[i] + ct[i];
+            __syncwarp();
+            double theta_old = theta_k;
+            for (int ps = 1; ps <= o.max_soc; ++ps) {
+                for (int i = lane; i < pb.m; i += 32) bs2[i] = -csoc[i];
+                __syncwarp();
+                solve_full(b1, bs2, b3, b4, sx, sy, szL, szU);
+                const double a_soc = ftb_primal(x, sx, tau);
+                for (int i = lane; i < pb.n; i += 32) xt[i] = x[i] + a_soc * sx[i];
+                __syncwarp();
+                double th_s, cm_s; bool fin_s;
+                const double f_s = c.eval_fc(xt, ct, th_s, cm_s, fin_s);
+                n_fc++;
+                const double ph_s = phi(xt, f_s, mu);
+                nsoc = ps;
+                if (acceptable(th_s, ph_s, theta_k, phi_k, alpha, gd)) {
+                    acc = 1; alpha_acc = a_soc; phi_acc = ph_s; f_acc = f_s; th_acc = th_s; cm_acc = cm_s;
+                    break;
+                }
+                if (!isfinite(th_s) || th_s > o.kappa_soc * theta_old) break;
+                theta_old = th_s;
+                for (int i = lane; i < pb.m; i += 32) csoc[i] = a_soc * csoc[i] + ct[i];
+                __syncwarp();
+            }
+            if (acc >= 0) break;
+        }
+        alpha *= o.alpha_red;
+        ntrial++;
+        if (alpha < a_min || ntrial > o.max_backtrack) break;
+    }
+    rec[6] = ntrial; rec[7] = nsoc;
+    if (acc < 0) { enter_restoration(rec, KIND_LS_FAIL); trace_put(rec); return; }
+    // A-6 accept, A-7 filter augmentation
+    const double* ax = (acc == 1) ? V(L.sx) : dx;
+    const double* ay = (acc == 1) ? V(L.sy) : dy;
+    const double* azL = (acc == 1) ? V(L.szL) : dzL;
+    const double* azU = (acc == 1) ? V(L.szU) : dzU;
+    const double a_z = ftb_dual(zL, zU, azL, azU, tau);
+    const bool ftype = switching(alpha, gd, theta_k) && armijo(phi_acc, phi_k, alpha, gd);
+    if (!ftype) filter_add((1.0 - o.gamma_theta) * theta_k, phi_k - o.gamma_phi * theta_k);
+    const double ks = o.kappa_sigma;
+    for (int i = lane; i < pb.n; i += 32) {
+        const double l = pb.xL[i], u = pb.xU[i];
+        const double xn = xt[i];
+        x[i] = xn;
+        double zl = 0.0, zu = 0.0;
+        if (l > -INFINITY) {
+            const double sl = xn - l;
+            zl = fmax(fmin(zL[i] + a_z * azL[i], ks * mu / sl), mu / (ks * sl));
+        }
+        if (u < INFINITY) {
+            const double su = u - xn;
+            zu = fmax(fmin(zU[i] + a_z * azU[i], ks * mu / su), mu / (ks * su));
+        }
+        zL[i] = zl; zU[i] = zu;
+    }
+    for (int i = lane; i < pb.m; i += 32) { y[i] += alpha_acc * ay[i]; cv[i] = ct[i]; }
+    __syncwarp();
+    f = f_acc; theta = th_acc; cmax = cm_acc;
+    k += 1;  // A-8
+    rec[5] = (acc == 1) ? KIND_SOC : KIND_NEWTON;
+    rec[8] = alpha_acc; rec[9] = a_z; rec[10] = ftype ? 1.0 : 0.0;
+    trace_put(rec);
+}
+
+template <class C>
+__device__ void Solver<C>::write_outputs() {
+    const double* x = V(L.x); const double* y = V(L.y); const double* zL = V(L.zL); const double* zU = V(L.zU);
+    if (A.x_out) for (int i = lane; i < pb.n; i += 32) A.x_out[pid * pb.n + i] = x[i];
+    if (A.lam_out) for (int i = lane; i < pb.m; i += 32) A.lam_out[pid * pb.m + i] = y[i];
+    if (A.zL_out) for (int i = lane; i < pb.n; i += 32) A.zL_out[pid * pb.n + i] = zL[i];
+    if (A.zU_out) for (int i = lane; i < pb.n; i += 32) A.zU_out[pid * pb.n + i] = zU[i];
+    if (lane == 0) {
+        if (A.status_out) A.status_out[pid] = status;
+        if (A.iters_out) A.iters_out[pid] = k;
+    }
+}
+
+}  // namespace jipm

@@ -1,0 +1,347 @@
+// jipm_api.cu -- host side of the C ABI declared in include/jipm.h.  No torch types, no CPU fallback.
+#include <cstdio>
+#include <cstring>
+#include <cmath>
+#include <string>
+#include <vector>
+#include <algorithm>
+#include "kernel.cuh"
+
+using namespace jipm;
+
+static thread_local std::string g_err = "";
+static int fail(int code, const std::string& msg) { g_err = msg; return code; }
+#define CUDA_TRY(expr)                                                                                   \
+    do {                                                                                                 \
+        cudaError_t e_ = (expr);                                                                         \
+        if (e_ != cudaSuccess)                                                                           \
+            return fail(e_ == cudaErrorMemoryAllocation ? JIPM_ERR_NOMEM : JIPM_ERR_CUDA,                \
+                        std::string(#expr) + ": " + cudaGetErrorString(e_));                             \
+    } while (0)
+
+using C_PM = Cfg<PointmassDyn, 1>;
+using C_Q1 = Cfg<QuadDyn, 1>;
+using C_Q2 = Cfg<QuadDyn, 2>;
+using C_Q4 = Cfg<QuadDyn, 4>;
+
+struct jipm_solver {
+    int family;
+    jipm_family_dims dims;
+    jipm_options o;
+    Pb pb;
+    Lay L;
+    int NX, NU, NZ, sm_per_warp, warps_per_block;
+    int n_slots;
+    cudaStream_t stream;
+    double *d_xL = nullptr, *d_xU = nullptr, *d_ws = nullptr;
+    int* d_queue = nullptr;
+    unsigned long long* d_stats = nullptr;
+    double* trace = nullptr;
+    int trace_cap = 0;
+    long long stats[8] = {0};
+    DbgLay dbg;
+};
+
+extern "C" const char* jipm_last_error(void) { return g_err.c_str(); }
+
+extern "C" int jipm_default_options(jipm_options* o) {
+    if (!o) return fail(JIPM_ERR_ARG, "options pointer is NULL");
+    o->tol = 1e-8; o->mu_init = 0.1; o->kappa_eps = 10.0; o->kappa_mu = 0.2; o->theta_mu = 1.5; o->tau_min = 0.99;
+    o->s_max = 100.0; o->kappa_sigma = 1e10; o->kappa_1 = 1e-2; o->kappa_2 = 1e-2; o->bound_relax_factor = 1e-8;
+    o->bound_mult_init = 1.0; o->lam_init_max = 1e3; o->kappa_d = 1e-5; o->gamma_theta = 1e-5; o->gamma_phi = 1e-8;
+    o->eta_phi = 1e-8; o->delta = 1.0; o->s_theta = 1.1; o->s_phi = 2.3; o->gamma_alpha = 0.05;
+    o->theta_max_fact = 1e4; o->theta_min_fact = 1e-4; o->alpha_red = 0.5; o->kappa_soc = 0.99;
+    o->delta_w_min = 1e-20; o->delta_w_0 = 1e-4; o->delta_w_max = 1e40; o->kappa_w_minus = 1.0 / 3.0;
+    o->kappa_w_plus = 8.0; o->kappa_w_plus_first = 100.0; o->delta_c_bar = 1e-8; o->kappa_c = 0.25;
+    o->residual_ratio_max = 1e-10; o->rho_resto = 1000.0; o->kappa_resto = 0.9; o->z_reset_threshold = 1e3;
+    o->max_iter = 3000; o->max_backtrack = 64; o->max_soc = 4; o->refine_min = 1; o->refine_max = 10;
+    o->max_mu_updates = 8; o->init_slacks = 1; o->enable_restoration = 1;
+    return JIPM_OK;
+}
+
+static bool family_shape(int family, const jipm_family_dims* d, int& nx, int& nu, int& ng, int& nth, int& pd) {
+    if (!d || d->horizon_N < 1 || d->horizon_N > 4096 || !(d->dt > 0.0)) return false;
+    const int na = d->n_agents, nobs = d->n_obstacles;
+    switch (family) {
+        case JIPM_FAM_POINTMASS2D:
+            if (na != 1 || nobs < 0) return false;
+            nx = 4; nu = 2; ng = nobs; nth = 4 + 2 + 3 * nobs; pd = 2; return true;
+        case JIPM_FAM_QUAD_TRACK:
+            if (na != 1 || nobs < 0) return false;
+            nx = 12; nu = 4; ng = nobs; nth = 12 + 2 + 4 * nobs; pd = 3; return true;
+        case JIPM_FAM_QUAD_CLUTTER:
+            if (na != 1 || nobs < 0) return false;
+            nx = 12; nu = 4; ng = nobs; nth = 12 + 3 + 4 * nobs; pd = 3; return true;
+        case JIPM_FAM_MULTIQUAD:
+            if (na != 2 && na != 4) return false;
+            nx = 12 * na; nu = 4 * na; ng = na * (na - 1) / 2; nth = 12 * na + 3 * na; pd = 3; return true;
+        default: return false;
+    }
+}
+
+extern "C" int jipm_family_sizes(int family, const jipm_family_dims* d, int64_t* n, int64_t* m, int64_t* n_theta) {
+    int nx, nu, ng, nth, pd;
+    if (!family_shape(family, d, nx, nu, ng, nth, pd)) return fail(JIPM_ERR_DIM, "bad family or dims");
+    const int64_t N = d->horizon_N;
+    if (n) *n = (N + 1) * nx + N * nu + N * ng;
+    if (m) *m = (N + 1) * nx + N * ng;
+    if (n_theta) *n_theta = nth;
+    return JIPM_OK;
+}
+
+static void build_layout(jipm_solver* s) {
+    const Pb& pb = s->pb;
+    const int n = pb.n, m = pb.m, N = pb.N, NX = s->NX, NU = s->NU, NZ = s->NZ;
+    const int pd = (pb.family == JIPM_FAM_POINTMASS2D) ? 2 : 3;
+    int o = 0;
+    auto take = [&](int cnt) { int r = o; o += (cnt + 1) & ~1; return r; };  // keep 16-byte alignment
+    Lay& L = s->L;
+    L.x = take(n); L.y = take(m); L.zL = take(n); L.zU = take(n); L.g = take(n); L.c = take(m);
+    L.gv = take(N * pb.ng * pd); L.tgt = take((N + 1) * pb.na * pd);
+    L.J = take(N * NX * NZ); L.W = take(N * NZ * NZ + NX * NX);
+    L.Sig = take(n); L.Hd = take(n); L.Dc = take(m);
+    L.T = take((N + 1) * NX * NX); L.Xf = take(N * NX * NU); L.Lf = take(N * NU * NU);
+    L.wv = take(N * NX); L.tv = take(N * NU);
+    L.b1 = take(n); L.b2 = take(m); L.b3 = take(n); L.b4 = take(n);
+    L.dx = take(n); L.dy = take(m); L.dzL = take(n); L.dzU = take(n);
+    L.r1 = take(n); L.r2 = take(m); L.r3 = take(n); L.r4 = take(n);
+    L.e1 = take(n); L.e2 = take(m); L.e3 = take(n); L.e4 = take(n);
+    L.sx = take(n); L.sy = take(m); L.szL = take(n); L.szU = take(n);
+    L.xt = take(n); L.ct = take(m); L.csoc = take(m); L.bs2 = take(m); L.rr = take(n);
+    L.rk = take(pb.family == JIPM_FAM_POINTMASS2D ? 0 : N * pb.na * 4 * RKW);
+    L.filt = take(2 * MAX_FILTER);
+    L.total = o;
+}
+
+template <class C>
+static cudaError_t launch(jipm_solver* s, const Args& a) {
+    const int wpb = s->warps_per_block;
+    const size_t smem = (size_t)wpb * C::SM_TOTAL * sizeof(double);
+    cudaError_t e = cudaFuncSetAttribute(jipm_slot_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    const int blocks = (a.n_slots + wpb - 1) / wpb;
+    jipm_slot_kernel<C><<<blocks, wpb * 32, smem, s->stream>>>(a);
+    return cudaGetLastError();
+}
+
+static cudaError_t dispatch(jipm_solver* s, const Args& a) {
+    if (s->family == JIPM_FAM_POINTMASS2D) return launch<C_PM>(s, a);
+    if (s->family == JIPM_FAM_MULTIQUAD) return s->dims.n_agents == 4 ? launch<C_Q4>(s, a) : launch<C_Q2>(s, a);
+    return launch<C_Q1>(s, a);
+}
+
+template <class C>
+static int sm_total() { return C::SM_TOTAL; }
+
+extern "C" int jipm_create(jipm_solver** out, int family, const jipm_family_dims* d, int64_t n, int64_t m,
+                           const double* x_L, const double* x_U, const jipm_options* opts, int64_t resident_slots,
+                           void* cuda_stream) {
+    if (!out || !x_L || !x_U) return fail(JIPM_ERR_ARG, "NULL argument");
+    int nx, nu, ng, nth, pd;
+    if (!family_shape(family, d, nx, nu, ng, nth, pd)) return fail(JIPM_ERR_DIM, "bad family or dims");
+    int64_t n2, m2, nt2;
+    jipm_family_sizes(family, d, &n2, &m2, &nt2);
+    if (n != n2 || m != m2) return fail(JIPM_ERR_DIM, "n, m do not match jipm_family_sizes");
+    if (resident_slots < 0) return fail(JIPM_ERR_ARG, "resident_slots < 0");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
+        return fail(JIPM_ERR_CUDA, "no CUDA device (jipm has no CPU fallback)");
+    jipm_solver* s = new jipm_solver();
+    s->family = family; s->dims = *d;
+    if (opts) s->o = *opts; else jipm_default_options(&s->o);
+    s->stream = (cudaStream_t)cuda_stream;
+    s->NX = nx; s->NU = nu; s->NZ = nx + nu;
+    Pb& pb = s->pb;
+    pb.family = family; pb.N = d->horizon_N; pb.ng = ng; pb.na = d->n_agents; pb.nobs = d->n_obstacles;
+    pb.n = (int)n; pb.m = (int)m; pb.nth = nth; pb.blk = nu + nx + ng; pb.cblk = nx + ng;
+    pb.dt = d->dt; pb.ru = (family == JIPM_FAM_POINTMASS2D) ? 0.1 : 0.01;
+    pb.th_obs = (family == JIPM_FAM_POINTMASS2D) ? 6 : (family == JIPM_FAM_QUAD_TRACK ? 14 : 15);
+    pb.th_goal = (family == JIPM_FAM_POINTMASS2D) ? 4 : (family == JIPM_FAM_MULTIQUAD ? 12 * d->n_agents : 12);
+    // Step I-1: relax finite bounds; PAPER.md:63 needs x_L < x_U
+    std::vector<double> xl(n), xu(n);
+    pb.nL = pb.nU = 0;
+    for (int64_t i = 0; i < n; ++i) {
+        double l = x_L[i], u = x_U[i];
+        if (std::isnan(l) || std::isnan(u)) { delete s; return fail(JIPM_ERR_BOUNDS, "NaN bound"); }
+        if (std::isfinite(l)) { l -= s->o.bound_relax_factor * std::max(1.0, std::fabs(l)); pb.nL++; } else l = -INFINITY;
+        if (std::isfinite(u)) { u += s->o.bound_relax_factor * std::max(1.0, std::fabs(u)); pb.nU++; } else u = INFINITY;
+        if (l >= u) { delete s; return fail(JIPM_ERR_BOUNDS, "x_L >= x_U on a component"); }
+        xl[i] = l; xu[i] = u;
+    }
+    build_layout(s);
+    s->dbg = make_dbglay(pb.n, pb.m, pb.N, s->NX, s->NZ);
+    if (family == JIPM_FAM_POINTMASS2D) s->sm_per_warp = sm_total<C_PM>();
+    else if (family == JIPM_FAM_MULTIQUAD) s->sm_per_warp = d->n_agents == 4 ? sm_total<C_Q4>() : sm_total<C_Q2>();
+    else s->sm_per_warp = sm_total<C_Q1>();
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, 0) != cudaSuccess) { delete s; return fail(JIPM_ERR_CUDA, "cudaGetDeviceProperties"); }
+    const size_t smw = (size_t)s->sm_per_warp * sizeof(double);
+    int wpb = 4;
+    while (wpb > 1 && wpb * smw > (size_t)prop.sharedMemPerBlockOptin) wpb >>= 1;
+    if (wpb * smw > (size_t)prop.sharedMemPerBlockOptin) { delete s; return fail(JIPM_ERR_NOMEM, "stage tile does not fit shared memory"); }
+    s->warps_per_block = wpb;
+    if (resident_slots == 0) {
+        // fill the GPU: as many warps per SM as shared memory and a 16-warp cap allow
+        int per_sm = (int)std::min<size_t>(16, (size_t)prop.sharedMemPerMultiprocessor / (smw + 256));
+        per_sm = std::max(per_sm / wpb * wpb, wpb);
+        resident_slots = (int64_t)per_sm * prop.multiProcessorCount;
+    }
+    s->n_slots = (int)resident_slots;
+    cudaError_t e;
+    if ((e = cudaMalloc(&s->d_xL, n * sizeof(double))) != cudaSuccess ||
+        (e = cudaMalloc(&s->d_xU, n * sizeof(double))) != cudaSuccess ||
+        (e = cudaMalloc(&s->d_ws, (size_t)s->n_slots * s->L.total * sizeof(double))) != cudaSuccess ||
+        (e = cudaMalloc(&s->d_queue, sizeof(int))) != cudaSuccess ||
+        (e = cudaMalloc(&s->d_stats, 8 * sizeof(unsigned long long))) != cudaSuccess) {
+        std::string msg = std::string("cudaMalloc: ") + cudaGetErrorString(e);
+        jipm_destroy(s);
+        return fail(JIPM_ERR_NOMEM, msg);
+    }
+    pb.xL = s->d_xL; pb.xU = s->d_xU;
+    if ((e = cudaMemcpyAsync(s->d_xL, xl.data(), n * sizeof(double), cudaMemcpyHostToDevice, s->stream)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(s->d_xU, xu.data(), n * sizeof(double), cudaMemcpyHostToDevice, s->stream)) != cudaSuccess ||
+        (e = cudaMemsetAsync(s->d_ws, 0, (size_t)s->n_slots * s->L.total * sizeof(double), s->stream)) != cudaSuccess ||
+        (e = cudaStreamSynchronize(s->stream)) != cudaSuccess) {
+        std::string msg = std::string("upload: ") + cudaGetErrorString(e);
+        jipm_destroy(s);
+        return fail(JIPM_ERR_CUDA, msg);
+    }
+    *out = s;
+    return JIPM_OK;
+}
+
+extern "C" int jipm_destroy(jipm_solver* s) {
+    if (!s) return JIPM_OK;
+    cudaFree(s->d_xL); cudaFree(s->d_xU); cudaFree(s->d_ws); cudaFree(s->d_queue); cudaFree(s->d_stats);
+    delete s;
+    return JIPM_OK;
+}
+
+static int run(jipm_solver* s, Args& a) {
+    a.pb = s->pb; a.L = s->L; a.o = s->o;
+    a.ws = s->d_ws; a.ws_stride = s->L.total; a.n_slots = (int)std::min<int64_t>(s->n_slots, std::max<int64_t>(a.P, 1));
+    a.queue = s->d_queue; a.stats = s->d_stats;
+    a.trace = s->trace; a.trace_cap = s->trace_cap;
+    a.dbg_len = s->dbg.len;
+    CUDA_TRY(cudaMemsetAsync(s->d_queue, 0, sizeof(int), s->stream));
+    CUDA_TRY(cudaMemsetAsync(s->d_stats, 0, 8 * sizeof(unsigned long long), s->stream));
+    CUDA_TRY(dispatch(s, a));
+    unsigned long long st[8];
+    CUDA_TRY(cudaMemcpyAsync(st, s->d_stats, sizeof(st), cudaMemcpyDeviceToHost, s->stream));
+    CUDA_TRY(cudaStreamSynchronize(s->stream));
+    for (int i = 0; i < 8; ++i) s->stats[i] = (long long)st[i];
+    s->stats[5] = a.n_slots; s->stats[6] = 1;
+    return JIPM_OK;
+}
+
+extern "C" int jipm_solve_batch(jipm_solver* s, int64_t P, const double* x0, const double* params, double* x_out,
+                                double* lam_out, double* zL_out, double* zU_out, int32_t* status_out,
+                                int32_t* iters_out) {
+    if (!s) return fail(JIPM_ERR_ARG, "solver is NULL");
+    if (P < 0 || P > 0x7fffffff) return fail(JIPM_ERR_ARG, "bad P");
+    if (P == 0) return JIPM_OK;
+    if (!x0 || !params || !x_out || !lam_out || !status_out || !iters_out) return fail(JIPM_ERR_ARG, "NULL buffer");
+    Args a; memset(&a, 0, sizeof(a));
+    a.P = (int)P; a.x0 = x0; a.th = params; a.x_out = x_out; a.lam_out = lam_out; a.zL_out = zL_out; a.zU_out = zU_out;
+    a.status_out = status_out; a.iters_out = iters_out; a.dbg_mode = 0;
+    return run(s, a);
+}
+
+extern "C" int jipm_solve_batch_host(jipm_solver* s, int64_t P, const double* x0, const double* params, double* x_out,
+                                     double* lam_out, double* zL_out, double* zU_out, int32_t* status_out,
+                                     int32_t* iters_out) {
+    if (!s) return fail(JIPM_ERR_ARG, "solver is NULL");
+    if (P < 0 || P > 0x7fffffff) return fail(JIPM_ERR_ARG, "bad P");
+    if (P == 0) return JIPM_OK;
+    if (!x0 || !params || !x_out || !lam_out || !status_out || !iters_out) return fail(JIPM_ERR_ARG, "NULL buffer");
+    const size_t n = s->pb.n, m = s->pb.m, nth = s->pb.nth;
+    const size_t nd = P * (2 * n + m + nth + (zL_out ? n : 0) + (zU_out ? n : 0));
+    double* buf = nullptr; int32_t* ib = nullptr;
+    CUDA_TRY(cudaMalloc(&buf, nd * sizeof(double)));
+    cudaError_t e = cudaMalloc(&ib, 2 * P * sizeof(int32_t));
+    if (e != cudaSuccess) { cudaFree(buf); return fail(JIPM_ERR_NOMEM, "cudaMalloc"); }
+    double* dx0 = buf; double* dth = dx0 + P * n; double* dxo = dth + P * nth; double* dlo = dxo + P * n;
+    double* dzl = zL_out ? dlo + P * m : nullptr; double* dzu = zU_out ? (dlo + P * m + (zL_out ? P * n : 0)) : nullptr;
+    int rc = JIPM_OK;
+    auto chk = [&](cudaError_t ee) { if (ee != cudaSuccess && rc == JIPM_OK) rc = fail(JIPM_ERR_CUDA, cudaGetErrorString(ee)); };
+    chk(cudaMemcpyAsync(dx0, x0, P * n * sizeof(double), cudaMemcpyHostToDevice, s->stream));
+    chk(cudaMemcpyAsync(dth, params, P * nth * sizeof(double), cudaMemcpyHostToDevice, s->stream));
+    if (rc == JIPM_OK) rc = jipm_solve_batch(s, P, dx0, dth, dxo, dlo, dzl, dzu, ib, ib + P);
+    if (rc == JIPM_OK) {
+        chk(cudaMemcpyAsync(x_out, dxo, P * n * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+        chk(cudaMemcpyAsync(lam_out, dlo, P * m * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+        if (zL_out) chk(cudaMemcpyAsync(zL_out, dzl, P * n * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+        if (zU_out) chk(cudaMemcpyAsync(zU_out, dzu, P * n * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+        chk(cudaMemcpyAsync(status_out, ib, P * sizeof(int32_t), cudaMemcpyDeviceToHost, s->stream));
+        chk(cudaMemcpyAsync(iters_out, ib + P, P * sizeof(int32_t), cudaMemcpyDeviceToHost, s->stream));
+        chk(cudaStreamSynchronize(s->stream));
+    }
+    cudaFree(buf); cudaFree(ib);
+    return rc;
+}
+
+extern "C" int jipm_last_stats(jipm_solver* s, int64_t* stats, int64_t n_stats) {
+    if (!s || !stats) return fail(JIPM_ERR_ARG, "NULL argument");
+    for (int64_t i = 0; i < n_stats && i < 8; ++i) stats[i] = s->stats[i];
+    return JIPM_OK;
+}
+
+extern "C" int jipm_debug_set_trace(jipm_solver* s, double* trace, int64_t max_records) {
+    if (!s) return fail(JIPM_ERR_ARG, "solver is NULL");
+    s->trace = trace; s->trace_cap = trace ? (int)max_records : 0;
+    return JIPM_OK;
+}
+
+extern "C" int jipm_debug_state_layout(jipm_solver* s, int64_t* lay, int64_t n_lay) {
+    if (!s || !lay) return fail(JIPM_ERR_ARG, "NULL argument");
+    const DbgLay& d = s->dbg;
+    const int v[15] = {d.len, d.x, d.y, d.zL, d.zU, d.sc, d.filt, d.dx, d.dy, d.dzL, d.dzU, d.g, d.c, d.J, d.W};
+    for (int64_t i = 0; i < n_lay && i < 15; ++i) lay[i] = v[i];
+    return JIPM_OK;
+}
+
+extern "C" int jipm_debug_step(jipm_solver* s, int64_t P, const double* params, double* state, int64_t n_steps) {
+    if (!s || !params || !state) return fail(JIPM_ERR_ARG, "NULL argument");
+    if (P <= 0) return JIPM_OK;
+    Args a; memset(&a, 0, sizeof(a));
+    a.P = (int)P; a.th = params; a.dbg_mode = 2; a.dbg_state = state; a.dbg_steps = (int)n_steps;
+    return run(s, a);
+}
+
+extern "C" int jipm_debug_init(jipm_solver* s, int64_t P, const double* x0, const double* params, double* state) {
+    if (!s || !x0 || !params || !state) return fail(JIPM_ERR_ARG, "NULL argument");
+    if (P <= 0) return JIPM_OK;
+    Args a; memset(&a, 0, sizeof(a));
+    a.P = (int)P; a.x0 = x0; a.th = params; a.dbg_mode = 1; a.dbg_state = state;
+    return run(s, a);
+}
+
+extern "C" int jipm_bench_fp64_peak(void* cuda_stream, double* tflops) {
+    if (!tflops) return fail(JIPM_ERR_ARG, "NULL argument");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(JIPM_ERR_CUDA, "no CUDA device");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    cudaDeviceProp prop;
+    CUDA_TRY(cudaGetDeviceProperties(&prop, 0));
+    const int blocks = prop.multiProcessorCount * 8, threads = 256, iters = 1 << 15;
+    double* out = nullptr;
+    CUDA_TRY(cudaMalloc(&out, (size_t)blocks * threads * sizeof(double)));
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    double best = 0.0;
+    for (int rep = 0; rep < 4; ++rep) {
+        cudaEventRecord(e0, st);
+        fp64_peak_kernel<<<blocks, threads, 0, st>>>(out, iters);
+        cudaEventRecord(e1, st);
+        cudaEventSynchronize(e1);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        const double fl = 2.0 * 8.0 * (double)iters * blocks * threads;
+        if (rep > 0 && ms > 0) best = std::max(best, fl / (ms * 1e-3) / 1e12);
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(out);
+    CUDA_TRY(cudaGetLastError());
+    *tflops = best;
+    return JIPM_OK;
+}
