@@ -1,0 +1,322 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the batched interior-point hot path (BASELINE.json metric) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl jipm|reference]
+
+A "step" is one pass of the whole hot path over one batch of synthetic problems: one jipm_solve_batch call
+(Step I for every problem, then fused IPM iterations with iteration-level batching until every problem of the
+batch has a final status).  Default workload: BASELINE.json configs[1] (single-quadrotor tracking, batch 4096,
+fp64, tol 1e-8).  `value` = SOLVED problems per second with inputs resident in HBM; `e2e` = the same through
+jipm_solve_batch_host (pinned host buffers, H2D/D2H inside the timed region).
+
+N > 1 (torchrun): the problem queue is sharded, every rank solves its own batch of the same size (weak scaling),
+no collective on the data path; time = max over ranks.
+
+--impl reference times the ORACLE (oracle/, plain numpy fp64) on the host cores on a bounded sample of the same
+workload; it is a deliberately slow checker, reported as a baseline, not a target.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2606_26341_b200 import workloads as wl  # noqa: E402
+
+METRIC = "converged NLPs/sec (fp64, tol 1e-8)"
+UNIT = "NLPs/s"
+WORKLOAD_NAMES = {0: "C0 2-D point-mass NMPC N=10, batch 256",
+                  1: "C1 single-quadrotor tracking RK4 N=20 3 obstacles, batch 4096",
+                  2: "C2 4-quadrotor collision-free navigation N=20, batch 2048",
+                  3: "C3 quadrotor in clutter N=30 32 obstacles, batch 8192"}
+
+
+# ---------------------------------------------------------------------------------------------------------
+# algorithmic FP64 work per operation of the structured algorithm (flops = 2 per FMA)
+# ---------------------------------------------------------------------------------------------------------
+def algorithmic_flops(d: wl.Dims) -> dict:
+    N, nx, nu, ng, na = d.horizon_N, d.nx, d.nu, d.ng, d.n_agents
+    nz, n, m = nx + nu, d.n, d.m
+    pd = 2 if d.family == wl.FAM_POINTMASS2D else 3
+    # stage-block LDL^T: per stage  T*[A B] (2 nx^2 nz), [A B]^T (T [A B]) (2 nx nz^2,
+    # symmetric half counted: nx nz^2), control-block elimination (nu pivots, rank-1 updates of an nz x nz tile:
+    # ~ nu nz^2), condensation of the (slack, multiplier) pairs (ng * pd^2 * 2)
+    fact = N * (2 * nx * nx * nz + nx * nz * nz + nu * nz * nz + 2 * ng * pd * pd * na)
+    # one solve: backward + forward sweeps: T (2 nx^2), [A B] twice (4 nx nz), X/L (2 nx nu + nu^2), x2 passes
+    solve = N * 2 * (2 * nx * nx + 4 * nx * nz + 2 * nx * nu + nu * nu) + 8 * (n + m)
+    if d.family == wl.FAM_POINTMASS2D:
+        fc = N * 12 + (N + 1) * 6 + N * ng * 8
+        deriv = fc + 4 * n
+    else:
+        ode = 110  # flops of one continuous-dynamics evaluation (sincos counted as 2 x 20)
+        fc = N * na * (4 * ode + 12 * 10) + (N + 1) * na * 9 + N * ng * 10
+        # analytic chain: 4 RK points x (Df entries ~120 + contracted 7x7 Hessian ~250 + adjoint 60) and the 16
+        # columns x 4 points x (Df column 60 + Hq v 45 + 7x16 accumulation 224)
+        deriv = N * na * (4 * (ode + 120 + 250 + 60) + 16 * 4 * (60 + 45 + 224)) + 6 * n
+    resid = 2 * (N * (nz * nz + 2 * nx * nz)) + 12 * (n + m)  # one residual of the unreduced system (6)
+    return dict(fact=fact, solve=solve, deriv=deriv, fc=fc, resid=resid)
+
+
+def flops_from_stats(d: wl.Dims, st: dict) -> float:
+    a = algorithmic_flops(d)
+    # every KKT solve inside solve_full is paired with one residual evaluation of (6)
+    return (st["factorisations"] * a["fact"] + st["kkt_solves"] * (a["solve"] + a["resid"])
+            + st["deriv_evals"] * a["deriv"] + st["fc_evals"] * a["fc"])
+
+
+# ---------------------------------------------------------------------------------------------------------
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        super().__init__(daemon=True)
+        self.gpu, self.rows, self.stop_flag, self.proc = gpu_index, [], False, None
+
+    def run(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(self.gpu)], stdout=subprocess.PIPE, text=True)
+            for line in self.proc.stdout:
+                if self.stop_flag:
+                    break
+                self.rows.append([c.strip() for c in line.split(",")])
+        except Exception:
+            pass
+
+    def finish(self) -> dict:
+        self.stop_flag = True
+        if self.proc is not None:
+            self.proc.terminate()
+        sm, smax, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[1])); smax.append(float(r[2]))
+            except (ValueError, IndexError):
+                continue
+            for name, col in (("hw_slowdown", 5), ("hw_thermal_slowdown", 6), ("sw_thermal_slowdown", 7),
+                              ("sw_power_cap", 8)):
+                if len(r) > col and r[col].lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"], "samples": 0}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(smax)), "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def _oracle_worker(args):
+    cfg, idx = args
+    os.environ["OMP_NUM_THREADS"] = "1"
+    from oracle import families as ofam, ipm as oipm
+    d, theta, x0 = wl.generate(cfg, 1, first_id=idx)
+    xL, xU = wl.bounds(d)
+    prob = ofam.Problem(d.family, d.horizon_N, d.n_agents, d.n_obstacles, d.dt)
+    st = oipm.Solver(prob, xL, xU).solve(x0[0], theta[0])
+    return int(st.status), int(st.k)
+
+
+def time_oracle(cfg: int, first: int, count: int, cores: int):
+    """The oracle as it stands, one problem per process over `cores` host cores; returns (seconds, solved, iters)."""
+    from multiprocessing import get_context
+    t0 = time.perf_counter()
+    with get_context("fork").Pool(cores) as pool:
+        res = pool.map(_oracle_worker, [(cfg, first + i) for i in range(count)], chunksize=1)
+    dt = time.perf_counter() - t0
+    return dt, sum(1 for s, _ in res if s == 0), sum(k for _, k in res)
+
+
+ORACLE_SAMPLE = {0: 256, 1: 16, 2: 2, 3: 2}  # problems per timed sample (about 10-30 s of CPU work)
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cfg = args.config
+    cores = os.cpu_count() or 1
+    count = ORACLE_SAMPLE[cfg]
+    for _ in range(min(args.warmup, 1)):
+        time_oracle(cfg, 0, min(count, cores), cores)
+    tot_t, tot_solved, tot_it = 0.0, 0, 0
+    for s in range(args.steps):
+        dt, solved, its = time_oracle(cfg, s * count, count, cores)
+        tot_t += dt; tot_solved += solved; tot_it += its
+    val = tot_solved / tot_t
+    sample = f"{count} problems of {WORKLOAD_NAMES[cfg]} per step (ids step*{count}..), one process per problem"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD_NAMES[cfg], "sample": sample},
+            "iterations_per_s": tot_it / tot_t,
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def run_jipm(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_26341_b200 import jipm
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (jipm has no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    cfg = args.config
+    P = args.batch or wl.CONFIG_BATCH[cfg]
+    d, theta, x0 = wl.generate(cfg, P, first_id=rank * P)  # queue sharded by rank: disjoint problem ids
+    xL, xU = wl.bounds(d)
+    s = jipm.Solver(d.family, d.horizon_N, d.n_agents, d.n_obstacles, d.dt, xL, xU, resident_slots=args.slots)
+    dev = torch.device("cuda", local)
+    x0_d = torch.as_tensor(x0, device=dev)
+    th_d = torch.as_tensor(theta, device=dev)
+    out = dict(x=torch.empty((P, d.n), dtype=torch.float64, device=dev),
+               lam=torch.empty((P, d.m), dtype=torch.float64, device=dev),
+               zL=torch.empty((P, d.n), dtype=torch.float64, device=dev),
+               zU=torch.empty((P, d.n), dtype=torch.float64, device=dev),
+               status=torch.empty((P,), dtype=torch.int32, device=dev),
+               iters=torch.empty((P,), dtype=torch.int32, device=dev))
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # > 126 MB L2
+    # pinned host buffers of the end-to-end leg
+    hx0 = torch.as_tensor(x0).pin_memory(); hth = torch.as_tensor(theta).pin_memory()
+    hout = dict(x=torch.empty((P, d.n), dtype=torch.float64).pin_memory(),
+                lam=torch.empty((P, d.m), dtype=torch.float64).pin_memory(),
+                zL=torch.empty((P, d.n), dtype=torch.float64).pin_memory(),
+                zU=torch.empty((P, d.n), dtype=torch.float64).pin_memory(),
+                status=torch.empty((P,), dtype=torch.int32).pin_memory(),
+                iters=torch.empty((P,), dtype=torch.int32).pin_memory())
+    hnp = {k: v.numpy() for k, v in hout.items()}
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        s.solve_batch_into(x0_d, th_d, out)
+    peak_fp64 = jipm.fp64_peak_tflops()  # roofline denominator measured on this GPU, outside the timed region
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.3)
+    # ---- timed region: K steps, device-resident inputs, CUDA events on the launching stream -------------
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    stats_sum = {}
+    t_wall0 = time.perf_counter()
+    for a, b in ev:
+        flush.fill_(1)  # L2 flush between timed iterations (not inside an event pair)
+        a.record(stream)
+        s.solve_batch_into(x0_d, th_d, out)
+        b.record(stream)
+        for k, v in s.stats().items():
+            stats_sum[k] = stats_sum.get(k, 0) + v
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    dev_ms = sum(a.elapsed_time(b) for a, b in ev)
+    clocks = sampler.finish() if rank == 0 else None
+    status = out["status"].cpu().numpy()
+    iters = out["iters"].cpu().numpy()
+    solved = int((status == 0).sum())
+    # ---- end-to-end leg: host buffers through jipm_solve_batch_host -------------------------------------
+    s.solve_batch_host(hx0.numpy(), hth.numpy(), hnp)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        s.solve_batch_host(hx0.numpy(), hth.numpy(), hnp)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    e2e_solved = int((hnp["status"] == 0).sum())
+    # ---- reduce over ranks ---------------------------------------------------------------------------------
+    red = torch.tensor([dev_ms, e2e_s, t_wall], dtype=torch.float64, device=dev)
+    cnt = torch.tensor([solved, e2e_solved, int(iters.sum()), P], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(red, op=dist.ReduceOp.MAX)
+        dist.all_reduce(cnt, op=dist.ReduceOp.SUM)
+    dev_ms, e2e_s, t_wall = red.tolist()
+    solved_all, e2e_solved_all, iters_all, P_all = cnt.tolist()
+    if rank == 0:
+        K = args.steps
+        secs = dev_ms * 1e-3
+        value = solved_all * K / secs
+        flops = flops_from_stats(d, stats_sum)  # rank 0's launches
+        my_secs = sum(a.elapsed_time(b) for a, b in ev) * 1e-3
+        achieved = flops / my_secs / 1e12
+        hist = {int(k): int((status == k).sum()) for k in np.unique(status)}
+        h2d = (x0.nbytes + theta.nbytes)
+        d2h = sum(v.nbytes for v in hnp.values())
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
+            "ms_per_step": dev_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD_NAMES[cfg], "batch_per_gpu": P, "n": d.n, "m": d.m,
+                       "resident_slots": s.stats()["slots"], "l2": "flushed between timed steps (256 MiB fill)",
+                       "parallelism": f"queue sharded over {world} GPU(s), no collective"},
+            "iterations_per_s": iters_all * K / secs,
+            "iters_mean": float(iters.mean()), "iters_max": int(iters.max()),
+            "status_hist_rank0": hist, "converged_fraction": solved_all / P_all,
+            "wall_s_timed_region": t_wall,
+            "e2e": {"value": e2e_solved_all * K / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                    "d2h_bytes_per_step": d2h},
+            "gpu_launches": int(stats_sum["launches"]),
+            "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_fp64, "unit": "TFLOP/s",
+                         "frac": achieved / peak_fp64, "traffic": None,
+                         "kernel": "jipm_slot_kernel (persistent, one launch per step)",
+                         "peak_source": "DFMA microbenchmark jipm_bench_fp64_peak measured in this run "
+                                        "(MEASURED_PEAKS.json has no FP64 entry); nominal 148 SM x 64 DFMA/clk x 2 x "
+                                        "1.965 GHz = 37.2",
+                         "algorithmic_flops_per_step": flops / K,
+                         "counts_per_step": {k: v / K for k, v in stats_sum.items()}},
+            "clocks": clocks,
+        }
+        if not args.no_cpu_baseline and world == 1:
+            cores = os.cpu_count() or 1
+            cnt_o = ORACLE_SAMPLE[cfg]
+            dt, so, it = time_oracle(cfg, 0, cnt_o, cores)
+            line["cpu_baseline"] = {"value": so / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                    "iterations_per_s": it / dt,
+                                    "sample": f"first {cnt_o} problems of the same workload, one process per problem"}
+        print(json.dumps(line))
+    s.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 3])
+    ap.add_argument("--batch", type=int, default=0, help="problems per GPU per step (default: the config's batch)")
+    ap.add_argument("--slots", type=int, default=0, help="resident slots (0: library picks)")
+    ap.add_argument("--impl", default="jipm", choices=["jipm", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_jipm(args)
+
+
+if __name__ == "__main__":
+    main()

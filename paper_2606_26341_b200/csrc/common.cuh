@@ -59,6 +59,21 @@ struct Args {
 // debug state layout (doubles) -- mirrored by jipm_debug_state_layout
 struct DbgLay { int len, x, y, zL, zU, sc, filt, dx, dy, dzL, dzU, g, c, J, W; };
 
+constexpr int RKW = 42;  // doubles of quadrotor phase-1 output per (stage, RK point); see dyn.cuh
+
+__host__ __device__ inline DbgLay make_dbglay(int n, int m, int N, int NX, int NZ) {
+    DbgLay d;
+    int o = 0;
+    d.x = o; o += n; d.y = o; o += m; d.zL = o; o += n; d.zU = o; o += n;
+    d.sc = o; o += 8; d.filt = o; o += 2 * MAX_FILTER;
+    d.dx = o; o += n; d.dy = o; o += m; d.dzL = o; o += n; d.dzU = o; o += n;
+    d.g = o; o += n; d.c = o; o += m;
+    d.J = o; o += N * NX * NZ; d.W = o; o += N * NZ * NZ + NX * NX;
+    d.len = o;
+    return d;
+}
+
+#ifdef __CUDACC__
 __device__ __forceinline__ double wsum(double v) {
 #pragma unroll
     for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(FULL, v, o);
@@ -76,5 +91,6 @@ __device__ __forceinline__ double wmin(double v) {
 }
 __device__ __forceinline__ int wor(int v) { return __any_sync(FULL, v); }
 __device__ __forceinline__ bool finite_d(double v) { return isfinite(v); }
+#endif
 
 }  // namespace jipm

@@ -17,7 +17,6 @@
 namespace jipm {
 
 constexpr double Q_G = 9.81, Q_MASS = 1.0, Q_ARM = 0.2, Q_JX = 0.01, Q_JY = 0.01, Q_JZ = 0.02, Q_KTAU = 0.02;
-constexpr int RKW = 42;  // doubles of phase-1 output per (stage, RK stage)
 
 struct PointmassDyn {
     static constexpr int AX = 4, AU = 2, PD = 2, AZ = 6;

@@ -5,7 +5,7 @@
 #include <string>
 #include <vector>
 #include <algorithm>
-#include "kernel.cuh"
+#include "launch.cuh"
 
 using namespace jipm;
 
@@ -19,10 +19,6 @@ static int fail(int code, const std::string& msg) { g_err = msg; return code; }
                         std::string(#expr) + ": " + cudaGetErrorString(e_));                             \
     } while (0)
 
-using C_PM = Cfg<PointmassDyn, 1>;
-using C_Q1 = Cfg<QuadDyn, 1>;
-using C_Q2 = Cfg<QuadDyn, 2>;
-using C_Q4 = Cfg<QuadDyn, 4>;
 
 struct jipm_solver {
     int family;
@@ -113,25 +109,13 @@ static void build_layout(jipm_solver* s) {
     L.total = o;
 }
 
-template <class C>
-static cudaError_t launch(jipm_solver* s, const Args& a) {
-    const int wpb = s->warps_per_block;
-    const size_t smem = (size_t)wpb * C::SM_TOTAL * sizeof(double);
-    cudaError_t e = cudaFuncSetAttribute(jipm_slot_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    const int blocks = (a.n_slots + wpb - 1) / wpb;
-    jipm_slot_kernel<C><<<blocks, wpb * 32, smem, s->stream>>>(a);
-    return cudaGetLastError();
-}
-
 static cudaError_t dispatch(jipm_solver* s, const Args& a) {
-    if (s->family == JIPM_FAM_POINTMASS2D) return launch<C_PM>(s, a);
-    if (s->family == JIPM_FAM_MULTIQUAD) return s->dims.n_agents == 4 ? launch<C_Q4>(s, a) : launch<C_Q2>(s, a);
-    return launch<C_Q1>(s, a);
+    const int wpb = s->warps_per_block;
+    if (s->family == JIPM_FAM_POINTMASS2D) return launch_pm(a, wpb, s->stream);
+    if (s->family == JIPM_FAM_MULTIQUAD)
+        return s->dims.n_agents == 4 ? launch_q4(a, wpb, s->stream) : launch_q2(a, wpb, s->stream);
+    return launch_q1(a, wpb, s->stream);
 }
-
-template <class C>
-static int sm_total() { return C::SM_TOTAL; }
 
 extern "C" int jipm_create(jipm_solver** out, int family, const jipm_family_dims* d, int64_t n, int64_t m,
                            const double* x_L, const double* x_U, const jipm_options* opts, int64_t resident_slots,
@@ -170,9 +154,9 @@ extern "C" int jipm_create(jipm_solver** out, int family, const jipm_family_dims
     }
     build_layout(s);
     s->dbg = make_dbglay(pb.n, pb.m, pb.N, s->NX, s->NZ);
-    if (family == JIPM_FAM_POINTMASS2D) s->sm_per_warp = sm_total<C_PM>();
-    else if (family == JIPM_FAM_MULTIQUAD) s->sm_per_warp = d->n_agents == 4 ? sm_total<C_Q4>() : sm_total<C_Q2>();
-    else s->sm_per_warp = sm_total<C_Q1>();
+    if (family == JIPM_FAM_POINTMASS2D) s->sm_per_warp = sm_doubles_pm();
+    else if (family == JIPM_FAM_MULTIQUAD) s->sm_per_warp = d->n_agents == 4 ? sm_doubles_q4() : sm_doubles_q2();
+    else s->sm_per_warp = sm_doubles_q1();
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, 0) != cudaSuccess) { delete s; return fail(JIPM_ERR_CUDA, "cudaGetDeviceProperties"); }
     const size_t smw = (size_t)s->sm_per_warp * sizeof(double);
@@ -331,7 +315,7 @@ extern "C" int jipm_bench_fp64_peak(void* cuda_stream, double* tflops) {
     double best = 0.0;
     for (int rep = 0; rep < 4; ++rep) {
         cudaEventRecord(e0, st);
-        fp64_peak_kernel<<<blocks, threads, 0, st>>>(out, iters);
+        launch_fp64_peak(out, blocks, threads, iters, st);
         cudaEventRecord(e1, st);
         cudaEventSynchronize(e1);
         float ms = 0.f;

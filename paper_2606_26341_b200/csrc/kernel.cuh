@@ -6,18 +6,6 @@
 
 namespace jipm {
 
-__host__ __device__ inline DbgLay make_dbglay(int n, int m, int N, int NX, int NZ) {
-    DbgLay d;
-    int o = 0;
-    d.x = o; o += n; d.y = o; o += m; d.zL = o; o += n; d.zU = o; o += n;
-    d.sc = o; o += 8; d.filt = o; o += 2 * MAX_FILTER;
-    d.dx = o; o += n; d.dy = o; o += m; d.dzL = o; o += n; d.dzU = o; o += n;
-    d.g = o; o += n; d.c = o; o += m;
-    d.J = o; o += N * NX * NZ; d.W = o; o += N * NZ * NZ + NX * NX;
-    d.len = o;
-    return d;
-}
-
 template <class C>
 __device__ void Solver<C>::dbg_load(const double* st) {
     const DbgLay D = make_dbglay(pb.n, pb.m, pb.N, NX, NZ);
@@ -111,17 +99,6 @@ __global__ void __launch_bounds__(128) jipm_slot_kernel(const __grid_constant__ 
         atomicAdd(&A.stats[3], (unsigned long long)S.n_deriv);
         atomicAdd(&A.stats[4], (unsigned long long)S.n_fc);
     }
-}
-
-// dependent-free DFMA chains: the FP64 roofline denominator
-__global__ void fp64_peak_kernel(double* out, int iters) {
-    double a0 = threadIdx.x * 1e-9, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
-    const double b = 1.0000001, cc = 1e-9;
-    for (int i = 0; i < iters; ++i) {
-        a0 = fma(a0, b, cc); a1 = fma(a1, b, cc); a2 = fma(a2, b, cc); a3 = fma(a3, b, cc);
-        a4 = fma(a4, b, cc); a5 = fma(a5, b, cc); a6 = fma(a6, b, cc); a7 = fma(a7, b, cc);
-    }
-    out[blockIdx.x * blockDim.x + threadIdx.x] = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
 }
 
 }  // namespace jipm
