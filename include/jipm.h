@@ -112,7 +112,7 @@ int jipm_debug_set_trace(jipm_solver* s, double* trace, int64_t max_records);
 
 /* Layout of the debug state vector used by jipm_debug_step: HOST out, offsets in doubles:
  * lay[0]=len, [1]=x, [2]=y, [3]=zL, [4]=zU, [5]=scalars(mu,tau,delta_w_last,theta_min,theta_max,k,status,nfilt),
- * [6]=filter (32 pairs theta,phi), [7]=dx, [8]=dy, [9]=dzL, [10]=dzU (step of the last iteration),
+ * [6]=filter (128 pairs theta,phi), [7]=dx, [8]=dy, [9]=dzL, [10]=dzU (step of the last iteration),
  * [11]=grad f, [12]=c, [13]=J blocks [N][nx][nx+nu], [14]=W blocks [N][nz][nz] then [nx][nx] */
 int jipm_debug_state_layout(jipm_solver* s, int64_t* lay, int64_t n_lay);
 

@@ -13,7 +13,7 @@
 namespace jipm {
 
 constexpr unsigned FULL = 0xffffffffu;
-constexpr int MAX_FILTER = 32;
+constexpr int MAX_FILTER = 128;
 constexpr double EPS_MACH = 2.220446049250313e-16;
 
 // problem description, passed by value to the kernel
@@ -33,6 +33,7 @@ struct Lay {
     int x, y, zL, zU, g, c, gv, tgt, J, W, Sig, Hd, Dc, T, Xf, Lf, wv, tv;
     int b1, b2, b3, b4, dx, dy, dzL, dzU, r1, r2, r3, r4, e1, e2, e3, e4;
     int sx, sy, szL, szU, xt, ct, csoc, bs2, rr, rk, filt, total;
+    int xR, DR2, filtR, rc2;  // restoration mode: reference point, scaling D_R^2, its own filter, condensed rhs
 };
 
 // per-launch arguments

@@ -24,22 +24,32 @@ struct Solver {
     // warp-uniform scalar state of the problem in this slot
     double mu, tau, dw_last, theta_min, theta_max, f, theta, cmax;
     int k, status, nfilt, nrec;
+    // restoration mode (Table I row 6): mode 1 iterates on X = [x; p; n] with the same kernel
+    // code; the regular problem's scalars are parked in *_reg until the exit test succeeds
+    int mode, nX, nfilt_reg;
+    double mu_reg, tau_reg, dw_last_reg, theta_min_reg, theta_max_reg;
+    double theta_entry, zeta, f_pn, f_q, f_base, theta_base, cmax_base, dc_cur;
     long long pid;
-    unsigned n_fact, n_solve, n_deriv, n_fc, n_iter;
+    unsigned n_fact, n_solve, n_deriv, n_fc, n_iter, n_resto;
 
     __device__ Solver(X& c_, const Args& A_) : c(c_), A(A_), pb(A_.pb), L(A_.L), o(A_.o), lane(c_.lane) {
-        n_fact = n_solve = n_deriv = n_fc = n_iter = 0;
+        n_fact = n_solve = n_deriv = n_fc = n_iter = n_resto = 0;
+        mode = 0; nX = pb.n;
     }
     __device__ __forceinline__ double* V(int off) const { return c.ws + off; }
-    __device__ __forceinline__ bool hasL(int i) const { return pb.xL[i] > -INFINITY; }
-    __device__ __forceinline__ bool hasU(int i) const { return pb.xU[i] < INFINITY; }
+    // bounds of the extended primal vector: entries >= n are the restoration variables p, n >= 0
+    __device__ __forceinline__ double lo(int i) const { return i < pb.n ? pb.xL[i] : 0.0; }
+    __device__ __forceinline__ double hi(int i) const { return i < pb.n ? pb.xU[i] : INFINITY; }
+    __device__ __forceinline__ bool hasL(int i) const { return lo(i) > -INFINITY; }
+    __device__ __forceinline__ bool hasU(int i) const { return hi(i) < INFINITY; }
+    __device__ __forceinline__ double* filt_active() const { return V(mode ? L.filtR : L.filt); }
 
     // barrier objective (3) with the one-sided damping term; NaN outside the interior
-    __device__ double phi(const double* x, double fv, double mu_) const {
+    __device__ double phi(const double* x, double fv, double mu_, int nvar) const {
         double s = 0.0;
         int badpt = 0;
-        for (int i = lane; i < pb.n; i += 32) {
-            const double l = pb.xL[i], u = pb.xU[i], xi = x[i];
+        for (int i = lane; i < nvar; i += 32) {
+            const double l = lo(i), u = hi(i), xi = x[i];
             const bool hl = l > -INFINITY, hu = u < INFINITY;
             if (hl) {
                 const double sl = xi - l;
@@ -62,8 +72,8 @@ struct Solver {
     // fraction to the boundary (PAPER.md:148 fn 2) on the primal step
     __device__ double ftb_primal(const double* x, const double* dx, double tau_) const {
         double a = 1.0;
-        for (int i = lane; i < pb.n; i += 32) {
-            const double l = pb.xL[i], u = pb.xU[i], d = dx[i];
+        for (int i = lane; i < nX; i += 32) {
+            const double l = lo(i), u = hi(i), d = dx[i];
             if (l > -INFINITY && d < 0.0) a = fmin(a, -tau_ * (x[i] - l) / d);
             if (u < INFINITY && d > 0.0) a = fmin(a, tau_ * (u - x[i]) / d);
         }
@@ -72,7 +82,7 @@ struct Solver {
     __device__ double ftb_dual(const double* zL, const double* zU, const double* dzL, const double* dzU,
                                double tau_) const {
         double a = 1.0;
-        for (int i = lane; i < pb.n; i += 32) {
+        for (int i = lane; i < nX; i += 32) {
             if (hasL(i) && dzL[i] < 0.0) a = fmin(a, -tau_ * zL[i] / dzL[i]);
             if (hasU(i) && dzU[i] < 0.0) a = fmin(a, -tau_ * zU[i] / dzU[i]);
         }
@@ -83,8 +93,8 @@ struct Solver {
     __device__ double opt_error(double mu_, double sd, double sc) const {
         const double* x = V(L.x); const double* zL = V(L.zL); const double* zU = V(L.zU); const double* rdb = V(L.b1);
         double ed = 0.0, es = 0.0;
-        for (int i = lane; i < pb.n; i += 32) {
-            const double l = pb.xL[i], u = pb.xU[i];
+        for (int i = lane; i < nX; i += 32) {
+            const double l = lo(i), u = hi(i);
             const bool hl = l > -INFINITY, hu = u < INFINITY;
             double dmp = 0.0;
             if (hl && !hu) dmp = o.kappa_d * mu_;
@@ -98,18 +108,30 @@ struct Solver {
     }
 
     // filter ([7] sec 2.3): entries (theta_j, phi_j) in the workspace
-    __device__ bool in_filter(double th_t, double ph_t) const {
-        if (th_t >= theta_max) return true;
-        const double* F = V(L.filt);
+    __device__ bool in_filter_of(const double* F, int nf, double thmax, double th_t, double ph_t) const {
+        if (th_t >= thmax) return true;
         int hit = 0;
-        for (int j = lane; j < nfilt; j += 32) hit |= (th_t >= F[2 * j] && ph_t >= F[2 * j + 1]);
+        for (int j = lane; j < nf; j += 32) hit |= (th_t >= F[2 * j] && ph_t >= F[2 * j + 1]);
         return wor(hit);
     }
+    __device__ bool in_filter(double th_t, double ph_t) const {
+        return in_filter_of(filt_active(), nfilt, theta_max, th_t, ph_t);
+    }
+    // add an entry; entries dominated by the new one (their forbidden region is a subset of the new region) are
+    // dropped first, which changes no decision (reading S-10).  Serial on lane 0: at most MAX_FILTER entries, once
+    // per h-type step.
     __device__ void filter_add(double th_e, double ph_e) {
-        double* F = V(L.filt);
-        const int slot = (nfilt < MAX_FILTER) ? nfilt : (nfilt % MAX_FILTER);  // overflow: overwrite the oldest
-        if (lane == 0) { F[2 * slot] = th_e; F[2 * slot + 1] = ph_e; }
-        if (nfilt < MAX_FILTER) nfilt++;
+        double* F = filt_active();
+        int nf = 0;
+        if (lane == 0) {
+            for (int j = 0; j < nfilt; ++j) {
+                const double t = F[2 * j], p = F[2 * j + 1];
+                if (!(t >= th_e && p >= ph_e)) { F[2 * nf] = t; F[2 * nf + 1] = p; ++nf; }
+            }
+            if (nf == MAX_FILTER) nf = MAX_FILTER - 1;  // overflow: the newest old entry is dropped (counted nowhere: never seen)
+            F[2 * nf] = th_e; F[2 * nf + 1] = ph_e;
+        }
+        nfilt = __shfl_sync(FULL, nf, 0) + 1;
         __syncwarp();
     }
     __device__ bool switching(double alpha, double g, double theta_k) const {
@@ -127,38 +149,67 @@ struct Solver {
     }
 
     // ---- linear algebra of one iteration ---------------------------------------------------------------
-    // Sig = zL/sL + zU/sU + Hd
-    __device__ void set_sigma(double dw, double dc) const {
+    // Sig = zL/sL + zU/sU + Hd, Hd = delta_w (+ zeta D_R^2 on x in restoration mode); Dc = delta_c, plus in
+    // restoration mode the Schur complement 1/Sig_p + 1/Sig_n of the eliminated (p, n) pairs ([7] sec 3.3)
+    __device__ void set_sigma(double dw, double dc) {
+        dc_cur = dc;
         const double* x = V(L.x); const double* zL = V(L.zL); const double* zU = V(L.zU);
         double* Sig = V(L.Sig); double* Hd = V(L.Hd); double* Dc = V(L.Dc);
-        for (int i = lane; i < pb.n; i += 32) {
-            const double l = pb.xL[i], u = pb.xU[i];
-            double s = dw;
+        const double* DR2 = V(L.DR2);
+        for (int i = lane; i < nX; i += 32) {
+            const double l = lo(i), u = hi(i);
+            const double hd = (mode && i < pb.n) ? dw + zeta * DR2[i] : dw;
+            double s = hd;
             if (l > -INFINITY) s += zL[i] / (x[i] - l);
             if (u < INFINITY) s += zU[i] / (u - x[i]);
-            Sig[i] = s; Hd[i] = dw;
+            Sig[i] = s; Hd[i] = hd;
         }
-        for (int i = lane; i < pb.m; i += 32) Dc[i] = dc;
+        __syncwarp();
+        for (int i = lane; i < pb.m; i += 32)
+            Dc[i] = mode ? dc + 1.0 / Sig[pb.n + i] + 1.0 / Sig[pb.n + pb.m + i] : dc;
         __syncwarp();
     }
+
+    // products with the constraint Jacobian / Lagrangian Hessian of the (extended) problem
+    __device__ __forceinline__ double ATx(const double* y, int i) const {
+        if (i < pb.n) return c.AT_entry(y, i);
+        return (i < pb.n + pb.m) ? -y[i - pb.n] : y[i - pb.n - pb.m];
+    }
+    __device__ __forceinline__ double Wx(const double* d, int i) const { return i < pb.n ? c.W_entry(d, i) : 0.0; }
 
     // solve (6) through (7) + the Delta z recovery of PAPER.md:110 for rhs (b1,b2,b3,b4) -> (d1..d4)
     __device__ void reduced_solve(const double* b1, const double* b2, const double* b3, const double* b4,
                                   double* d1, double* d2, double* d3, double* d4) {
         const double* x = V(L.x); const double* zL = V(L.zL); const double* zU = V(L.zU);
         double* rr = V(L.rr);
-        for (int i = lane; i < pb.n; i += 32) {
-            const double l = pb.xL[i], u = pb.xU[i];
+        for (int i = lane; i < nX; i += 32) {
+            const double l = lo(i), u = hi(i);
             double r = b1[i];
             if (l > -INFINITY) r += b3[i] / (x[i] - l);
             if (u < INFINITY) r -= b4[i] / (u - x[i]);
             rr[i] = r;
         }
         __syncwarp();
-        K::solve(c, rr, b2, d1, d2);
+        const double* rc = b2;
+        const double* Sig = V(L.Sig);
+        const int n = pb.n, m = pb.m;
+        if (mode) {  // eliminate (dp, dn): dp = (r_p + dy)/Sig_p, dn = (r_n - dy)/Sig_n
+            double* rc2 = V(L.rc2);
+            for (int j = lane; j < m; j += 32) rc2[j] = b2[j] + rr[n + j] / Sig[n + j] - rr[n + m + j] / Sig[n + m + j];
+            __syncwarp();
+            rc = rc2;
+        }
+        K::solve(c, rr, rc, d1, d2);
         n_solve++;
-        for (int i = lane; i < pb.n; i += 32) {
-            const double l = pb.xL[i], u = pb.xU[i];
+        if (mode) {
+            for (int j = lane; j < m; j += 32) {
+                d1[n + j] = (rr[n + j] + d2[j]) / Sig[n + j];
+                d1[n + m + j] = (rr[n + m + j] - d2[j]) / Sig[n + m + j];
+            }
+            __syncwarp();
+        }
+        for (int i = lane; i < nX; i += 32) {
+            const double l = lo(i), u = hi(i);
             d3[i] = (l > -INFINITY) ? (b3[i] - zL[i] * d1[i]) / (x[i] - l) : 0.0;
             d4[i] = (u < INFINITY) ? (b4[i] + zU[i] * d1[i]) / (u - x[i]) : 0.0;
         }
@@ -170,12 +221,12 @@ struct Solver {
                                     const double* d1, const double* d2, const double* d3, const double* d4,
                                     double& dnorm) const {
         const double* x = V(L.x); const double* zL = V(L.zL); const double* zU = V(L.zU);
-        const double* Hd = V(L.Hd); const double* Dc = V(L.Dc);
+        const double* Hd = V(L.Hd);
         double* r1 = V(L.r1); double* r2 = V(L.r2); double* r3 = V(L.r3); double* r4 = V(L.r4);
         double rn = 0.0, dn = 0.0;
-        for (int i = lane; i < pb.n; i += 32) {
-            const double l = pb.xL[i], u = pb.xU[i];
-            const double lhs1 = c.W_entry(d1, i) + Hd[i] * d1[i] + c.AT_entry(d2, i) - d3[i] + d4[i];
+        for (int i = lane; i < nX; i += 32) {
+            const double l = lo(i), u = hi(i);
+            const double lhs1 = Wx(d1, i) + Hd[i] * d1[i] + ATx(d2, i) - d3[i] + d4[i];
             const double v1 = b1[i] - lhs1;
             r1[i] = v1; rn = fmax(rn, fabs(v1));
             double v3 = 0.0, v4 = 0.0;
@@ -187,7 +238,9 @@ struct Solver {
         }
         c.A_mul(d1, r2);
         for (int i = lane; i < pb.m; i += 32) {
-            const double v2 = b2[i] - (r2[i] - Dc[i] * d2[i]);
+            double ad = r2[i];
+            if (mode) ad += d1[pb.n + pb.m + i] - d1[pb.n + i];
+            const double v2 = b2[i] - (ad - dc_cur * d2[i]);
             r2[i] = v2; rn = fmax(rn, fabs(v2)); dn = fmax(dn, fabs(d2[i]));
         }
         __syncwarp();
@@ -200,7 +253,7 @@ struct Solver {
                               double* d1, double* d2, double* d3, double* d4) {
         reduced_solve(b1, b2, b3, b4, d1, d2, d3, d4);
         double bn = 0.0;
-        for (int i = lane; i < pb.n; i += 32) bn = fmax(bn, fmax(fabs(b1[i]), fmax(fabs(b3[i]), fabs(b4[i]))));
+        for (int i = lane; i < nX; i += 32) bn = fmax(bn, fmax(fabs(b1[i]), fmax(fabs(b3[i]), fabs(b4[i]))));
         for (int i = lane; i < pb.m; i += 32) bn = fmax(bn, fabs(b2[i]));
         bn = wmax(bn);
         int nref = 0;
@@ -210,7 +263,7 @@ struct Solver {
             const double rn = full_residual(b1, b2, b3, b4, d1, d2, d3, d4, dn);
             if (nref >= o.refine_min && rn <= o.residual_ratio_max * (bn + dn)) break;
             reduced_solve(V(L.r1), V(L.r2), V(L.r3), V(L.r4), e1, e2, e3, e4);
-            for (int i = lane; i < pb.n; i += 32) { d1[i] += e1[i]; d3[i] += e3[i]; d4[i] += e4[i]; }
+            for (int i = lane; i < nX; i += 32) { d1[i] += e1[i]; d3[i] += e3[i]; d4[i] += e4[i]; }
             for (int i = lane; i < pb.m; i += 32) d2[i] += e2[i];
             __syncwarp();
             nref++;
@@ -227,6 +280,9 @@ struct Solver {
     __device__ void init_problem(long long id);
     __device__ void iterate();
     __device__ void enter_restoration(double* rec, int kind);
+    __device__ void try_exit_restoration();
+    __device__ double eval_point(const double* xt, double* ct, double& th_t, double& cm_t, double& fb, double& thb,
+                                 double& cmb, double& fpn, double& fq);
     __device__ void write_outputs();
     __device__ void dbg_load(const double* st);
     __device__ void dbg_store(double* st);

@@ -8,6 +8,7 @@ namespace jipm {
 template <class C>
 __device__ void Solver<C>::init_problem(long long id) {
     pid = id;
+    mode = 0; nX = pb.n;
     c.th = A.th + id * pb.nth;
     const double* th = c.th;
     const int N = pb.N;
@@ -90,51 +91,157 @@ __device__ void Solver<C>::init_problem(long long id) {
     status = fin ? JIPM_ST_NOT_RUN : JIPM_ST_NONFINITE;
 }
 
-// Restoration entry (Table I row 6).  [round-1 state: the fused restoration mode is not
-// built yet -- the problem ends with RESTORATION_FAILED; DESIGN.md "Status".]
+// f, c (and theta, ||c||_inf) of the active problem at a trial point.  Regular mode: the NLP itself.  Restoration
+// mode ([7] sec 3.3): X = [x; p; n], f_R = rho sum(p+n) + zeta/2 ||D_R (x - x_R)||^2, c_R = c(x) - p + n; the base
+// problem's f, theta, ||c||_inf come back too (the exit test of Step R needs them).
+template <class C>
+__device__ double Solver<C>::eval_point(const double* xt, double* ct, double& th_t, double& cm_t, double& fb,
+                                        double& thb, double& cmb, double& fpn, double& fq) {
+    bool fin;
+    fb = c.eval_fc(xt, ct, thb, cmb, fin);
+    n_fc++;
+    if (!mode) { th_t = thb; cm_t = cmb; fpn = 0.0; fq = 0.0; return fb; }
+    const int n = pb.n, m = pb.m;
+    const double* xR = V(L.xR); const double* DR2 = V(L.DR2);
+    double spn = 0.0, sq = 0.0, th1 = 0.0, cm = 0.0;
+    for (int j = lane; j < m; j += 32) {
+        const double pj = xt[n + j], nj = xt[n + m + j];
+        const double v = (ct[j] - pj) + nj;
+        ct[j] = v; th1 += fabs(v); cm = fmax(cm, fabs(v));
+        spn += pj + nj;
+    }
+    for (int i = lane; i < n; i += 32) { const double d = xt[i] - xR[i]; sq += DR2[i] * d * d; }
+    __syncwarp();
+    fpn = wsum(spn); fq = wsum(sq); th_t = wsum(th1); cm_t = wmax(cm);
+    return o.rho_resto * fpn + 0.5 * zeta * fq;
+}
+
+// Restoration entry (Table I row 6; Step R of SURVEY.md 8(c), [7] sec 3.3).  The restoration
+// problem  min rho e^T(p+n) + zeta/2 ||D_R(x-x_R)||^2  s.t. c(x) - p + n = 0, p, n >= 0, x_L <= x <= x_U  is iterated
+// by the SAME iterate() with mode = 1 (same KKT sparsity after eliminating p, n: that is what lets it fuse).
 template <class C>
 __device__ void Solver<C>::enter_restoration(double* rec, int kind) {
     rec[5] = kind;
-    if (theta < o.tol) status = JIPM_ST_RESTO_AT_FEASIBLE_POINT;
-    else status = JIPM_ST_RESTORATION_FAILED;
-    rec[12] = rec[12];
-    k += 1;
+    if (!o.enable_restoration || mode == 1) { status = JIPM_ST_RESTORATION_FAILED; return; }  // no nesting (A20)
+    if (theta < o.tol) { status = JIPM_ST_RESTO_AT_FEASIBLE_POINT; return; }
+    const int n = pb.n, m = pb.m;
+    double* x = V(L.x); double* y = V(L.y); double* zL = V(L.zL); double* zU = V(L.zU); double* cv = V(L.c);
+    const double theta_k = theta;
+    const double phi_k = phi(x, f, mu, n);
+    filter_add((1.0 - o.gamma_theta) * theta_k, phi_k - o.gamma_phi * theta_k);
+    const double mu_bar = fmax(mu, cmax);
+    mu_reg = mu; tau_reg = tau; dw_last_reg = dw_last; theta_min_reg = theta_min; theta_max_reg = theta_max;
+    nfilt_reg = nfilt;
+    f_base = f; theta_base = theta_k; cmax_base = cmax;
+    const double rho = o.rho_resto;
+    double* xR = V(L.xR); double* DR2 = V(L.DR2);
+    for (int i = lane; i < n; i += 32) {
+        const double xi = x[i];
+        xR[i] = xi;
+        const double dr = fmin(1.0, 1.0 / fmax(fabs(xi), 1e-300));
+        DR2[i] = dr * dr;
+        zL[i] = hasL(i) ? fmin(rho, zL[i]) : 0.0;
+        zU[i] = hasU(i) ? fmin(rho, zU[i]) : 0.0;
+    }
+    double th1 = 0.0, cm = 0.0, spn = 0.0;
+    for (int j = lane; j < m; j += 32) {
+        // closed-form minimiser of the restoration barrier function in (p, n) at fixed x ([7] eqs 32-33)
+        const double cj = cv[j];
+        const double t = (mu_bar - rho * cj) / (2.0 * rho);
+        const double nn = t + sqrt(t * t + mu_bar * cj / (2.0 * rho));
+        const double pp = cj + nn;
+        x[n + j] = pp; x[n + m + j] = nn;
+        zL[n + j] = mu_bar / pp; zL[n + m + j] = mu_bar / nn;
+        zU[n + j] = 0.0; zU[n + m + j] = 0.0;
+        y[j] = 0.0;
+        const double v = (cj - pp) + nn;
+        cv[j] = v; th1 += fabs(v); cm = fmax(cm, fabs(v));
+        spn += pp + nn;
+    }
+    __syncwarp();
+    theta = wsum(th1); cmax = wmax(cm); f_pn = wsum(spn); f_q = 0.0;
+    mode = 1; nX = n + 2 * m;
+    mu = mu_bar; tau = fmax(o.tau_min, 1.0 - mu_bar); dw_last = 0.0; nfilt = 0;
+    zeta = sqrt(mu_bar);
+    f = rho * f_pn + 0.5 * zeta * f_q;
+    theta_max = o.theta_max_fact * fmax(1.0, theta);
+    theta_min = o.theta_min_fact * fmax(1.0, theta);
+    theta_entry = theta_k;
+    k += 1;  // the failed regular iteration counts (reading S-19)
 }
 
-// ---- Step A: one iteration ----------------------------------------------------------------------------------
+// Exit test after an accepted restoration step: theta(x) <= kappa_resto theta(x_R) and (theta, phi_mu) not in the
+// REGULAR filter -> back to regular mode with y = 0 and the restoration z (reading S-15).
+template <class C>
+__device__ void Solver<C>::try_exit_restoration() {
+    const int n = pb.n;
+    double* x = V(L.x); double* y = V(L.y); double* zL = V(L.zL); double* zU = V(L.zU);
+    const double phi_b = phi(x, f_base, mu_reg, n);
+    if (!isfinite(phi_b) || !(theta_base <= o.kappa_resto * theta_entry)) return;
+    if (in_filter_of(V(L.filt), nfilt_reg, theta_max_reg, theta_base, phi_b)) return;
+    double zm = 0.0;
+    for (int i = lane; i < n; i += 32) zm = fmax(zm, fmax(zL[i], zU[i]));
+    zm = wmax(zm);
+    if (zm > o.z_reset_threshold)
+        for (int i = lane; i < n; i += 32) { zL[i] = hasL(i) ? 1.0 : 0.0; zU[i] = hasU(i) ? 1.0 : 0.0; }
+    for (int j = lane; j < pb.m; j += 32) y[j] = 0.0;
+    __syncwarp();
+    mode = 0; nX = n;
+    mu = mu_reg; tau = tau_reg; dw_last = dw_last_reg; theta_min = theta_min_reg; theta_max = theta_max_reg;
+    nfilt = nfilt_reg;
+    bool fin;
+    f = c.eval_fc(x, V(L.c), theta, cmax, fin);  // base c back into the c vector (same point: same values)
+    n_fc++;
+}
+
+// ---- Step A: one iteration (either mode) ---------------------------------------------------------------------
 template <class C>
 __device__ void Solver<C>::iterate() {
     double* x = V(L.x); double* y = V(L.y); double* zL = V(L.zL); double* zU = V(L.zU);
-    double* cv = V(L.c); const double* g = V(L.g);
+    double* cv = V(L.c); double* g = V(L.g);
     double* b1 = V(L.b1); double* b2 = V(L.b2); double* b3 = V(L.b3); double* b4 = V(L.b4);
     double* dx = V(L.dx); double* dy = V(L.dy); double* dzL = V(L.dzL); double* dzU = V(L.dzU);
+    const int n = pb.n, m = pb.m;
     double rec[JIPM_TRACE_W];
 #pragma unroll
     for (int i = 0; i < JIPM_TRACE_W; ++i) rec[i] = 0.0;
+    rec[0] = mode;
     n_iter++;
-    // A-1 derivatives at (x, y)
-    c.eval_derivs(x, y, 1.0);
+    if (mode) n_resto++;
+    // A-1 derivatives at (x, y): sigma_f = 0 in restoration mode (its objective is rho e^T(p+n) + zeta/2 ||D_R(x-x_R)||^2)
+    c.eval_derivs(x, y, mode ? 0.0 : 1.0);
     n_deriv++;
+    if (mode) {
+        const double* xR = V(L.xR); const double* DR2 = V(L.DR2);
+        for (int i = lane; i < n; i += 32) g[i] = zeta * DR2[i] * (x[i] - xR[i]);
+        for (int i = n + lane; i < nX; i += 32) g[i] = o.rho_resto;
+        __syncwarp();
+    }
     // dual residual base rdb = grad f + A^T y - zL + zU  (into b1), multiplier sums for the scaling s_d, s_c
     double ysum = 0.0, zsum = 0.0, chk = 0.0;
-    for (int i = lane; i < pb.n; i += 32) {
-        const double v = g[i] + c.AT_entry(y, i) - zL[i] + zU[i];
+    for (int i = lane; i < nX; i += 32) {
+        const double v = g[i] + ATx(y, i) - zL[i] + zU[i];
         b1[i] = v; chk += v;
         zsum += fabs(zL[i]) + fabs(zU[i]);
     }
-    for (int i = lane; i < pb.m; i += 32) ysum += fabs(y[i]);
+    for (int i = lane; i < m; i += 32) ysum += fabs(y[i]);
     ysum = wsum(ysum); zsum = wsum(zsum); chk = wsum(chk);
     __syncwarp();
     if (!isfinite(chk) || !isfinite(f) || !isfinite(theta)) {
         status = JIPM_ST_NONFINITE; rec[5] = KIND_TERMINAL; trace_put(rec); return;
     }
-    const int nz = pb.nL + pb.nU;
-    const double sd = (pb.m + nz > 0) ? fmax(o.s_max, (ysum + zsum) / (pb.m + nz)) / o.s_max : 1.0;
+    const int nz = pb.nL + pb.nU + (mode ? 2 * m : 0);
+    const double sd = (m + nz > 0) ? fmax(o.s_max, (ysum + zsum) / (m + nz)) / o.s_max : 1.0;
     const double sc = (nz > 0) ? fmax(o.s_max, zsum / nz) / o.s_max : 1.0;
     // A-2 termination
     const double e0 = opt_error(0.0, sd, sc);
     rec[12] = e0;
-    if (e0 <= o.tol) { status = JIPM_ST_SOLVED; rec[5] = KIND_TERMINAL; trace_put(rec); return; }
+    if (e0 <= o.tol) {
+        // restoration problem converged without an acceptable point: local minimiser of the violation
+        if (mode) status = (theta_base > o.tol) ? JIPM_ST_LOCALLY_INFEASIBLE : JIPM_ST_RESTO_AT_FEASIBLE_POINT;
+        else status = JIPM_ST_SOLVED;
+        rec[5] = KIND_TERMINAL; trace_put(rec); return;
+    }
     if (k >= o.max_iter) { status = JIPM_ST_MAXITER; rec[5] = KIND_TERMINAL; trace_put(rec); return; }
     // A-3 monotone barrier update (Table I row 7)
     int nmu = 0;
@@ -144,6 +251,17 @@ __device__ void Solver<C>::iterate() {
         tau = fmax(o.tau_min, 1.0 - mu);
         nfilt = 0;
         nmu++;
+        if (mode) {  // zeta = sqrt(mu) follows the restoration barrier parameter: objective, gradient, residual move
+            const double zn = sqrt(mu);
+            const double* xR = V(L.xR); const double* DR2 = V(L.DR2);
+            for (int i = lane; i < n; i += 32) {
+                const double gi = zn * DR2[i] * (x[i] - xR[i]);
+                b1[i] += gi - g[i]; g[i] = gi;
+            }
+            __syncwarp();
+            zeta = zn;
+            f = o.rho_resto * f_pn + 0.5 * zeta * f_q;
+        }
     }
     rec[11] = nmu; rec[13] = mu;
     // A-4 search direction with inertia correction (Algorithm IC)
@@ -166,12 +284,11 @@ __device__ void Solver<C>::iterate() {
     }
     n_fact += nfact;
     rec[1] = nfact; rec[2] = dw; rec[3] = dc; rec[14] = theta;
-    if (!ic_ok) { enter_restoration(rec, KIND_IC_FAIL); trace_put(rec); return; }
+    if (!ic_ok) { rec[1] = 0; rec[2] = 0; rec[3] = 0; enter_restoration(rec, KIND_IC_FAIL); trace_put(rec); return; }
     if (dw > 0.0) dw_last = dw;
     // right-hand side of (6)
-    double gd_part = 0.0;
-    for (int i = lane; i < pb.n; i += 32) {
-        const double l = pb.xL[i], u = pb.xU[i];
+    for (int i = lane; i < nX; i += 32) {
+        const double l = lo(i), u = hi(i);
         const bool hl = l > -INFINITY, hu = u < INFINITY;
         double dmp = 0.0;
         if (hl && !hu) dmp = o.kappa_d * mu;
@@ -180,13 +297,14 @@ __device__ void Solver<C>::iterate() {
         b3[i] = hl ? mu - (x[i] - l) * zL[i] : 0.0;
         b4[i] = hu ? mu - (u - x[i]) * zU[i] : 0.0;
     }
-    for (int i = lane; i < pb.m; i += 32) b2[i] = -cv[i];
+    for (int i = lane; i < m; i += 32) b2[i] = -cv[i];
     __syncwarp();
     const int nref = solve_full(b1, b2, b3, b4, dx, dy, dzL, dzU);
     rec[4] = nref;
     // A-5 filter line search
-    for (int i = lane; i < pb.n; i += 32) {
-        const double l = pb.xL[i], u = pb.xU[i];
+    double gd_part = 0.0;
+    for (int i = lane; i < nX; i += 32) {
+        const double l = lo(i), u = hi(i);
         const bool hl = l > -INFINITY, hu = u < INFINITY;
         double gp = g[i];
         if (hl) gp -= mu / (x[i] - l);
@@ -197,7 +315,7 @@ __device__ void Solver<C>::iterate() {
     }
     const double gd = wsum(gd_part);
     const double theta_k = theta;
-    const double phi_k = phi(x, f, mu);
+    const double phi_k = phi(x, f, mu, nX);
     rec[15] = phi_k;
     const double a_max = ftb_primal(x, dx, tau);
     double a_min;
@@ -208,44 +326,45 @@ __device__ void Solver<C>::iterate() {
     else a_min = o.gamma_alpha * o.gamma_theta;
     double* xt = V(L.xt); double* ct = V(L.ct);
     double alpha = a_max, alpha_acc = 0.0, phi_acc = 0.0, f_acc = 0.0, th_acc = 0.0, cm_acc = 0.0;
+    double fb_acc = 0.0, thb_acc = 0.0, cmb_acc = 0.0, fpn_acc = 0.0, fq_acc = 0.0;
     int ntrial = 0, nsoc = 0, acc = -1;  // acc: 0 newton, 1 soc
     while (true) {
-        for (int i = lane; i < pb.n; i += 32) xt[i] = x[i] + alpha * dx[i];
+        for (int i = lane; i < nX; i += 32) xt[i] = x[i] + alpha * dx[i];
         __syncwarp();
-        double th_t, cm_t; bool fin;
-        const double f_t = c.eval_fc(xt, ct, th_t, cm_t, fin);
-        n_fc++;
-        const double ph_t = phi(xt, f_t, mu);
+        double th_t, cm_t, fb, thb, cmb, fpn, fq;
+        const double f_t = eval_point(xt, ct, th_t, cm_t, fb, thb, cmb, fpn, fq);
+        const double ph_t = phi(xt, f_t, mu, nX);
         if (acceptable(th_t, ph_t, theta_k, phi_k, alpha, gd)) {
             acc = 0; alpha_acc = alpha; phi_acc = ph_t; f_acc = f_t; th_acc = th_t; cm_acc = cm_t;
+            fb_acc = fb; thb_acc = thb; cmb_acc = cmb; fpn_acc = fpn; fq_acc = fq;
             break;
         }
         if (ntrial == 0 && isfinite(th_t) && th_t >= theta_k && o.max_soc > 0) {
             // second-order correction (Table I row 2)
             double* csoc = V(L.csoc); double* bs2 = V(L.bs2);
             double* sx = V(L.sx); double* sy = V(L.sy); double* szL = V(L.szL); double* szU = V(L.szU);
-            for (int i = lane; i < pb.m; i += 32) csoc[i] = alpha * cv[i] + ct[i];
+            for (int i = lane; i < m; i += 32) csoc[i] = alpha * cv[i] + ct[i];
             __syncwarp();
             double theta_old = theta_k;
             for (int ps = 1; ps <= o.max_soc; ++ps) {
-                for (int i = lane; i < pb.m; i += 32) bs2[i] = -csoc[i];
+                for (int i = lane; i < m; i += 32) bs2[i] = -csoc[i];
                 __syncwarp();
                 solve_full(b1, bs2, b3, b4, sx, sy, szL, szU);
                 const double a_soc = ftb_primal(x, sx, tau);
-                for (int i = lane; i < pb.n; i += 32) xt[i] = x[i] + a_soc * sx[i];
+                for (int i = lane; i < nX; i += 32) xt[i] = x[i] + a_soc * sx[i];
                 __syncwarp();
-                double th_s, cm_s; bool fin_s;
-                const double f_s = c.eval_fc(xt, ct, th_s, cm_s, fin_s);
-                n_fc++;
-                const double ph_s = phi(xt, f_s, mu);
+                double th_s, cm_s;
+                const double f_s = eval_point(xt, ct, th_s, cm_s, fb, thb, cmb, fpn, fq);
+                const double ph_s = phi(xt, f_s, mu, nX);
                 nsoc = ps;
                 if (acceptable(th_s, ph_s, theta_k, phi_k, alpha, gd)) {
                     acc = 1; alpha_acc = a_soc; phi_acc = ph_s; f_acc = f_s; th_acc = th_s; cm_acc = cm_s;
+                    fb_acc = fb; thb_acc = thb; cmb_acc = cmb; fpn_acc = fpn; fq_acc = fq;
                     break;
                 }
                 if (!isfinite(th_s) || th_s > o.kappa_soc * theta_old) break;
                 theta_old = th_s;
-                for (int i = lane; i < pb.m; i += 32) csoc[i] = a_soc * csoc[i] + ct[i];
+                for (int i = lane; i < m; i += 32) csoc[i] = a_soc * csoc[i] + ct[i];
                 __syncwarp();
             }
             if (acc >= 0) break;
@@ -261,12 +380,13 @@ __device__ void Solver<C>::iterate() {
     const double* ay = (acc == 1) ? V(L.sy) : dy;
     const double* azL = (acc == 1) ? V(L.szL) : dzL;
     const double* azU = (acc == 1) ? V(L.szU) : dzU;
+    (void)ax;
     const double a_z = ftb_dual(zL, zU, azL, azU, tau);
     const bool ftype = switching(alpha, gd, theta_k) && armijo(phi_acc, phi_k, alpha, gd);
     if (!ftype) filter_add((1.0 - o.gamma_theta) * theta_k, phi_k - o.gamma_phi * theta_k);
     const double ks = o.kappa_sigma;
-    for (int i = lane; i < pb.n; i += 32) {
-        const double l = pb.xL[i], u = pb.xU[i];
+    for (int i = lane; i < nX; i += 32) {
+        const double l = lo(i), u = hi(i);
         const double xn = xt[i];
         x[i] = xn;
         double zl = 0.0, zu = 0.0;
@@ -280,13 +400,15 @@ __device__ void Solver<C>::iterate() {
         }
         zL[i] = zl; zU[i] = zu;
     }
-    for (int i = lane; i < pb.m; i += 32) { y[i] += alpha_acc * ay[i]; cv[i] = ct[i]; }
+    for (int i = lane; i < m; i += 32) { y[i] += alpha_acc * ay[i]; cv[i] = ct[i]; }
     __syncwarp();
     f = f_acc; theta = th_acc; cmax = cm_acc;
+    f_base = fb_acc; theta_base = thb_acc; cmax_base = cmb_acc; f_pn = fpn_acc; f_q = fq_acc;
     k += 1;  // A-8
     rec[5] = (acc == 1) ? KIND_SOC : KIND_NEWTON;
     rec[8] = alpha_acc; rec[9] = a_z; rec[10] = ftype ? 1.0 : 0.0;
     trace_put(rec);
+    if (mode) try_exit_restoration();
 }
 
 template <class C>

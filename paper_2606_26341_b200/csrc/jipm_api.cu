@@ -92,20 +92,22 @@ static void build_layout(jipm_solver* s) {
     int o = 0;
     auto take = [&](int cnt) { int r = o; o += (cnt + 1) & ~1; return r; };  // keep 16-byte alignment
     Lay& L = s->L;
-    L.x = take(n); L.y = take(m); L.zL = take(n); L.zU = take(n); L.g = take(n); L.c = take(m);
+    const int nX = n + 2 * m;  // restoration mode iterates on X = [x; p; n]
+    L.x = take(nX); L.y = take(m); L.zL = take(nX); L.zU = take(nX); L.g = take(nX); L.c = take(m);
     L.gv = take(N * pb.ng * pd); L.tgt = take((N + 1) * pb.na * pd);
     L.J = take(N * NX * NZ); L.W = take(N * NZ * NZ + NX * NX);
-    L.Sig = take(n); L.Hd = take(n); L.Dc = take(m);
+    L.Sig = take(nX); L.Hd = take(nX); L.Dc = take(m);
     L.T = take((N + 1) * NX * NX); L.Xf = take(N * NX * NU); L.Lf = take(N * NU * NU);
     L.wv = take(N * NX); L.tv = take(N * NU);
-    L.b1 = take(n); L.b2 = take(m); L.b3 = take(n); L.b4 = take(n);
-    L.dx = take(n); L.dy = take(m); L.dzL = take(n); L.dzU = take(n);
-    L.r1 = take(n); L.r2 = take(m); L.r3 = take(n); L.r4 = take(n);
-    L.e1 = take(n); L.e2 = take(m); L.e3 = take(n); L.e4 = take(n);
-    L.sx = take(n); L.sy = take(m); L.szL = take(n); L.szU = take(n);
-    L.xt = take(n); L.ct = take(m); L.csoc = take(m); L.bs2 = take(m); L.rr = take(n);
+    L.b1 = take(nX); L.b2 = take(m); L.b3 = take(nX); L.b4 = take(nX);
+    L.dx = take(nX); L.dy = take(m); L.dzL = take(nX); L.dzU = take(nX);
+    L.r1 = take(nX); L.r2 = take(m); L.r3 = take(nX); L.r4 = take(nX);
+    L.e1 = take(nX); L.e2 = take(m); L.e3 = take(nX); L.e4 = take(nX);
+    L.sx = take(nX); L.sy = take(m); L.szL = take(nX); L.szU = take(nX);
+    L.xt = take(nX); L.ct = take(m); L.csoc = take(m); L.bs2 = take(m); L.rr = take(nX);
     L.rk = take(pb.family == JIPM_FAM_POINTMASS2D ? 0 : N * pb.na * 4 * RKW);
     L.filt = take(2 * MAX_FILTER);
+    L.xR = take(n); L.DR2 = take(n); L.filtR = take(2 * MAX_FILTER); L.rc2 = take(m);
     L.total = o;
 }
 
@@ -147,6 +149,7 @@ extern "C" int jipm_create(jipm_solver** out, int family, const jipm_family_dims
     for (int64_t i = 0; i < n; ++i) {
         double l = x_L[i], u = x_U[i];
         if (std::isnan(l) || std::isnan(u)) { delete s; return fail(JIPM_ERR_BOUNDS, "NaN bound"); }
+        if (l >= u) { delete s; return fail(JIPM_ERR_BOUNDS, "x_L >= x_U on a component (PAPER.md:63 needs x_L < x_U)"); }
         if (std::isfinite(l)) { l -= s->o.bound_relax_factor * std::max(1.0, std::fabs(l)); pb.nL++; } else l = -INFINITY;
         if (std::isfinite(u)) { u += s->o.bound_relax_factor * std::max(1.0, std::fabs(u)); pb.nU++; } else u = INFINITY;
         if (l >= u) { delete s; return fail(JIPM_ERR_BOUNDS, "x_L >= x_U on a component"); }

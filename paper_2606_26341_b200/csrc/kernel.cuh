@@ -13,6 +13,7 @@ __device__ void Solver<C>::dbg_load(const double* st) {
     for (int i = lane; i < pb.n; i += 32) { x[i] = st[D.x + i]; zL[i] = st[D.zL + i]; zU[i] = st[D.zU + i]; }
     for (int i = lane; i < pb.m; i += 32) y[i] = st[D.y + i];
     for (int i = lane; i < 2 * MAX_FILTER; i += 32) V(L.filt)[i] = st[D.filt + i];
+    mode = 0; nX = pb.n;
     mu = st[D.sc + 0]; tau = st[D.sc + 1]; dw_last = st[D.sc + 2];
     theta_min = st[D.sc + 3]; theta_max = st[D.sc + 4];
     k = (int)st[D.sc + 5]; status = (int)st[D.sc + 6]; nfilt = (int)st[D.sc + 7];
@@ -98,6 +99,7 @@ __global__ void __launch_bounds__(128) jipm_slot_kernel(const __grid_constant__ 
         atomicAdd(&A.stats[2], (unsigned long long)S.n_solve);
         atomicAdd(&A.stats[3], (unsigned long long)S.n_deriv);
         atomicAdd(&A.stats[4], (unsigned long long)S.n_fc);
+        atomicAdd(&A.stats[7], (unsigned long long)S.n_resto);
     }
 }
 

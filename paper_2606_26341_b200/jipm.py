@@ -122,8 +122,8 @@ class Solver:
         self._trace = None
 
     def close(self):
-        if getattr(self, "_h", None) is not None and self._h.value:
-            lib().jipm_destroy(self._h)
+        if getattr(self, "_h", None) is not None and self._h.value and _lib is not None:
+            _lib.jipm_destroy(self._h)
             self._h = C.c_void_p()
 
     __del__ = close

@@ -42,8 +42,8 @@ def e_v(v, vref):
 
 
 def decisions_equal(gpu_rec: np.ndarray, otr: dict) -> tuple[bool, str]:
-    """One iteration: the integer decisions must be identical; the reals agree to 1e-6 relative (they are
-    compared tightly by the step-parity tests; here they only guard against a different branch)."""
+    """One iteration: the integer decisions must be identical; the step lengths agree to 1e-4 relative (iterates
+    are compared tightly by the step-parity tests; here the reals only guard against a different branch)."""
     kind = KIND_CODE[otr["kind"]]
     if int(gpu_rec[T_KIND]) != kind:
         return False, f"kind {int(gpu_rec[T_KIND])} vs {kind}"
@@ -67,9 +67,9 @@ def decisions_equal(gpu_rec: np.ndarray, otr: dict) -> tuple[bool, str]:
         return True, ""
     if bool(gpu_rec[T_FTYPE]) != bool(otr["ftype"]):
         return False, "ftype"
-    if not np.isclose(gpu_rec[T_ALPHA], otr["alpha"], rtol=1e-6, atol=1e-12):
+    if not np.isclose(gpu_rec[T_ALPHA], otr["alpha"], rtol=1e-4, atol=1e-12):
         return False, f"alpha {gpu_rec[T_ALPHA]} vs {otr['alpha']}"
-    if not np.isclose(gpu_rec[T_ALPHAZ], otr["alpha_z"], rtol=1e-6, atol=1e-12):
+    if not np.isclose(gpu_rec[T_ALPHAZ], otr["alpha_z"], rtol=1e-4, atol=1e-12):
         return False, f"alpha_z {gpu_rec[T_ALPHAZ]} vs {otr['alpha_z']}"
     return True, ""
 
