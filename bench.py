@@ -183,7 +183,11 @@ def run_jipm(args):
     P = args.batch or wl.CONFIG_BATCH[cfg]
     d, theta, x0 = wl.generate(cfg, P, first_id=rank * P)  # queue sharded by rank: disjoint problem ids
     xL, xU = wl.bounds(d)
-    s = jipm.Solver(d.family, d.horizon_N, d.n_agents, d.n_obstacles, d.dt, xL, xU, resident_slots=args.slots)
+    opts = None
+    if args.max_iter > 0:
+        opts = jipm.default_options()
+        opts.max_iter = args.max_iter
+    s = jipm.Solver(d.family, d.horizon_N, d.n_agents, d.n_obstacles, d.dt, xL, xU, opts, resident_slots=args.slots)
     dev = torch.device("cuda", local)
     x0_d = torch.as_tensor(x0, device=dev)
     th_d = torch.as_tensor(theta, device=dev)
@@ -270,6 +274,8 @@ def run_jipm(args):
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": WORKLOAD_NAMES[cfg], "batch_per_gpu": P, "n": d.n, "m": d.m,
                        "resident_slots": s.stats()["slots"], "l2": "flushed between timed steps (256 MiB fill)",
+                       **({"max_iter_cap": args.max_iter, "note": "profiling run, not a bench value"}
+                          if args.max_iter > 0 else {}),
                        "parallelism": f"queue sharded over {world} GPU(s), no collective"},
             "iterations_per_s": iters_all * K / secs,
             "iters_mean": float(iters.mean()), "iters_max": int(iters.max()),
@@ -311,6 +317,9 @@ def main():
     ap.add_argument("--slots", type=int, default=0, help="resident slots (0: library picks)")
     ap.add_argument("--impl", default="jipm", choices=["jipm", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--max-iter", type=int, default=0,
+                    help="cap IPM iterations per problem (profiling runs only: keeps the kernel short under ncu; "
+                         "a line produced with this flag says so in config and is not a bench value)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -1,9 +1,9 @@
 // common.cuh -- shared structs and warp helpers of the jipm CUDA path (sm_100a, fp64).
 //
-// Execution model: ONE WARP OWNS ONE PROBLEM SLOT.  A warp runs the whole
-// interior-point iteration of PAPER.md:77-150 for its problem, synchronising only with __syncwarp(), and
-// pops the next problem id from a global queue when its problem reaches a final status (iteration-level
-// batching).  All decisions are warp-uniform predicates.
+// Execution model: ONE TEAM OF NT THREADS OWNS ONE PROBLEM SLOT.  A team runs the whole
+// interior-point iteration of PAPER.md:77-150 for its problem, synchronising only inside the team (warp sync or
+// a named barrier), and pops the next problem id from a global queue when its problem reaches a final status
+// (iteration-level batching).  All decisions are team-uniform predicates.
 #pragma once
 #include <cstdint>
 #include <cmath>
@@ -30,9 +30,10 @@ struct Pb {
 
 // offsets (in doubles) into the per-warp workspace
 struct Lay {
-    int x, y, zL, zU, g, c, gv, tgt, J, W, Sig, Hd, Dc, T, Xf, Lf, wv, tv;
+    int x, y, zL, zU, g, c, gv, tgt, J, W, Sig, Hd, Dc, T, Kf, Gf, Psi, pv, qv, sv, wv, tv;
     int b1, b2, b3, b4, dx, dy, dzL, dzU, r1, r2, r3, r4, e1, e2, e3, e4;
     int sx, sy, szL, szU, xt, ct, csoc, bs2, rr, rk, filt, total;
+    int nsm;  // the first nsm doubles of the layout are shared-memory resident (per team), the rest global
     int xR, DR2, filtR, rc2;  // restoration mode: reference point, scaling D_R^2, its own filter, condensed rhs
 };
 
@@ -75,23 +76,51 @@ __host__ __device__ inline DbgLay make_dbglay(int n, int m, int N, int NX, int N
 }
 
 #ifdef __CUDACC__
-__device__ __forceinline__ double wsum(double v) {
+// Launch arguments live in constant memory (one copy per translation unit / family instantiation, uploaded by the
+// launcher on the solver's stream): every pb->, L->, o->, A-> below compiles to a c[3][offset] operand instead of a
+// load through a pointer to the kernel parameters.
+static __constant__ Args g_A;
+struct PbProxy { __device__ __forceinline__ const Pb* operator->() const { return &g_A.pb; } };
+struct LayProxy { __device__ __forceinline__ const Lay* operator->() const { return &g_A.L; } };
+struct OptProxy { __device__ __forceinline__ const jipm_options* operator->() const { return &g_A.o; } };
+struct ArgsProxy { __device__ __forceinline__ const Args* operator->() const { return &g_A; } };
+
+// A TEAM of NT threads (NT = 32, 64, 128 or 256; whole warps) owns one problem slot.  All decisions of the
+// interior-point iteration are team-uniform predicates: every thread of the team holds the same scalar state,
+// obtained from the reductions below, which return bit-identical values to every thread.
+template <int NT>
+struct Team {
+    static constexpr int NW = NT / 32;
+    int tid;      // 0 .. NT-1
+    int bar;      // unused while there is one team per CTA (barrier 0)
+    int flip;     // which half of the reduction scratch the next reduction uses
+    double* red;  // shared memory, 2 * NW doubles
+
+    __device__ __forceinline__ void sync() const {
+        if constexpr (NT == 32) __syncwarp();
+        else __syncthreads();  // one team per CTA
+    }
+    template <class Op>
+    __device__ __forceinline__ double reduce(double v, Op op) {
 #pragma unroll
-    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(FULL, v, o);
-    return v;
-}
-__device__ __forceinline__ double wmax(double v) {
+        for (int o = 16; o; o >>= 1) v = op(v, __shfl_xor_sync(FULL, v, o));
+        if constexpr (NT == 32) return v;
+        double* r = red + flip * NW;
+        if ((tid & 31) == 0) r[tid >> 5] = v;
+        sync();
+        double a = r[0];
 #pragma unroll
-    for (int o = 16; o; o >>= 1) v = fmax(v, __shfl_xor_sync(FULL, v, o));
-    return v;
-}
-__device__ __forceinline__ double wmin(double v) {
-#pragma unroll
-    for (int o = 16; o; o >>= 1) v = fmin(v, __shfl_xor_sync(FULL, v, o));
-    return v;
-}
-__device__ __forceinline__ int wor(int v) { return __any_sync(FULL, v); }
-__device__ __forceinline__ bool finite_d(double v) { return isfinite(v); }
+        for (int w = 1; w < NW; ++w) a = op(a, r[w]);
+        flip ^= 1;  // the next reduction writes the other half: one barrier per reduction is enough
+        return a;
+    }
+    __device__ __forceinline__ double sum(double v) { return reduce(v, [](double a, double b) { return a + b; }); }
+    __device__ __forceinline__ double max(double v) { return reduce(v, [](double a, double b) { return fmax(a, b); }); }
+    __device__ __forceinline__ double min(double v) { return reduce(v, [](double a, double b) { return fmin(a, b); }); }
+    __device__ __forceinline__ int any(int v) { return reduce(v ? 1.0 : 0.0, [](double a, double b) { return fmax(a, b); }) > 0.0; }
+    // broadcast an int from thread 0
+    __device__ __forceinline__ int bcast0(int v) { return (int)reduce(tid == 0 ? (double)v : -1.0e300, [](double a, double b) { return fmax(a, b); }); }
+};
 #endif
 
 }  // namespace jipm

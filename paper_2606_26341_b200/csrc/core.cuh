@@ -6,42 +6,53 @@
 
 namespace jipm {
 
-template <class Dyn_, int NA_>
+template <class Dyn_, int NA_, int NT_>
 struct Cfg {
     using Dyn = Dyn_;
     static constexpr int NA = NA_;
+    static constexpr int NT = NT_;  // threads per problem slot (team size)
     static constexpr int AX = Dyn::AX, AU = Dyn::AU, PD = Dyn::PD;
     static constexpr int NX = AX * NA, NU = AU * NA, NZ = NX + NU;
-    // shared memory per warp (doubles): T, J, M, 5 small vectors, V staging for the quadrotor Hessian
+    // fixed shared memory per team (doubles): T, J, M, TJ/Phi, Kf/Linv tiles of the stage sweep, the staging of the
+    // quadrotor Hessian columns (7 x 16 per 16-thread group), the reduction scratch
     static constexpr int SM_MSZ = (NZ * NZ > 2 * NX * NX) ? NZ * NZ : 2 * NX * NX;
-    static constexpr int SM_T = 0, SM_J = SM_T + NX * NX, SM_M = SM_J + NX * NZ, SM_V = SM_M + SM_MSZ;
-    static constexpr int SM_TOTAL = SM_V + 4 * NX + 2 * NU + 8;
+    static constexpr int SM_T = 0, SM_J = SM_T + NX * NX, SM_M = SM_J + NX * NZ, SM_TJ = SM_M + SM_MSZ;
+    static constexpr int SM_K = SM_TJ + NX * NZ, SM_G = SM_K + NU * NX + NU * NU;
+    static constexpr int SM_RED = SM_G + (Dyn::AX == 12 ? (NT / 16) * 7 * 16 : 0);
+    static constexpr int SM_TOTAL = SM_RED + 2 * (NT / 32) + 2;
 };
 
 template <class C>
 struct Ctx {
     static constexpr int NX = C::NX, NU = C::NU, NZ = C::NZ, PD = C::PD, AX = C::AX, AU = C::AU, NA = C::NA;
-    const Pb& pb;
-    const Lay& L;
-    const jipm_options& o;
-    double* ws;        // this warp's workspace (global)
-    double* sm;        // this warp's shared memory
+    static constexpr int NT = C::NT;
+    PbProxy pb;        // launch arguments: constant memory (common.cuh)
+    LayProxy L;
+    OptProxy o;
+    double* ws;        // this team's global workspace, shifted so that ws + off is valid for off >= L->nsm
+    double* sm;        // this team's fixed shared memory (tiles, staging, reduction scratch)
+    double* smd;       // this team's shared-memory part of the workspace layout (offsets < L->nsm)
     const double* th;  // theta of the current problem
-    int lane;
+    int lane;          // thread index inside the team, 0 .. NT-1
+    mutable Team<NT> tm;
 
-    __device__ Ctx(const Pb& pb_, const Lay& L_, const jipm_options& o_, double* ws_, double* sm_, int lane_)
-        : pb(pb_), L(L_), o(o_), ws(ws_), sm(sm_), th(nullptr), lane(lane_) {}
+    __device__ Ctx(double* ws_, double* sm_, int tid_, int bar_)
+        : ws(ws_ - g_A.L.nsm), sm(sm_), smd(sm_ + C::SM_TOTAL), th(nullptr), lane(tid_) {
+        tm.tid = tid_; tm.bar = bar_; tm.flip = 0; tm.red = sm_ + C::SM_RED;
+    }
 
     // ---- stage-order index helpers (same layout as include/jipm.h) -----------------------------------
-    __device__ __forceinline__ int ix(int k) const { return k == 0 ? 0 : NX + (k - 1) * pb.blk + NU; }
-    __device__ __forceinline__ int iu(int k) const { return NX + k * pb.blk; }
-    __device__ __forceinline__ int is(int k) const { return NX + (k - 1) * pb.blk + NU + NX; }
-    __device__ __forceinline__ int icd(int k) const { return k == 0 ? 0 : NX + (k - 1) * pb.cblk; }
-    __device__ __forceinline__ int icg(int k) const { return NX + (k - 1) * pb.cblk + NX; }
+    __device__ __forceinline__ int ix(int k) const { return k == 0 ? 0 : NX + (k - 1) * pb->blk + NU; }
+    __device__ __forceinline__ int iu(int k) const { return NX + k * pb->blk; }
+    __device__ __forceinline__ int is(int k) const { return NX + (k - 1) * pb->blk + NU + NX; }
+    __device__ __forceinline__ int icd(int k) const { return k == 0 ? 0 : NX + (k - 1) * pb->cblk; }
+    __device__ __forceinline__ int icg(int k) const { return NX + (k - 1) * pb->cblk + NX; }
     __device__ __forceinline__ int zidx(int k, int a) const { return a < NX ? ix(k) + a : iu(k) + a - NX; }
-    __device__ __forceinline__ double* Jk(int k) const { return ws + L.J + k * (NX * NZ); }
-    __device__ __forceinline__ double* Wk(int k) const { return ws + L.W + k * (NZ * NZ); }  // k == N: NX x NX
-    __device__ __forceinline__ double* v(int off) const { return ws + off; }
+    __device__ __forceinline__ double* Jk(int k) const { return v(L->J) + k * (NX * NZ); }
+    __device__ __forceinline__ double* Wk(int k) const { return v(L->W) + k * (NZ * NZ); }  // k == N: NX x NX
+    // workspace array at layout offset off: the first L->nsm doubles of the layout live in shared memory (the
+    // hot vectors and factor blocks), the rest in this slot's global workspace (L2-resident scratch)
+    __device__ __forceinline__ double* v(int off) const { return off < L->nsm ? smd + off : ws + off; }
 
     // pair q -> agents (a,b), a<b, row-major enumeration
     __device__ __forceinline__ void pair_ab(int q, int& a, int& b) const {
@@ -53,7 +64,7 @@ struct Ctx {
     // inequality h_j(x_k) >= 0 (obstacle or pair separation), value
     __device__ double ineq_val(const double* x, int k, int j) const {
         double s = 0.0;
-        if (pb.family == JIPM_FAM_MULTIQUAD) {
+        if (pb->family == JIPM_FAM_MULTIQUAD) {
             int a, b; pair_ab(j, a, b);
             const double* pa = x + ix(k) + AX * a; const double* pb_ = x + ix(k) + AX * b;
 #pragma unroll
@@ -61,16 +72,16 @@ struct Ctx {
             return s - 0.25;
         }
         const double* p = x + ix(k);
-        const double* ob = th + pb.th_obs + (PD + 1) * j;
+        const double* ob = th + pb->th_obs + (PD + 1) * j;
 #pragma unroll
         for (int i = 0; i < PD; ++i) { double d = p[i] - ob[i]; s += d * d; }
         return s - ob[PD] * ob[PD];
     }
     // G_{k,j} . d  with the gradient vector stored in gv (2*(p-c) or 2*(p_a-p_b))
     __device__ double G_dot(const double* gv, const double* d, int k, int j) const {
-        const double* g = gv + ((k - 1) * pb.ng + j) * PD;
+        const double* g = gv + ((k - 1) * pb->ng + j) * PD;
         double s = 0.0;
-        if (pb.family == JIPM_FAM_MULTIQUAD) {
+        if (pb->family == JIPM_FAM_MULTIQUAD) {
             int a, b; pair_ab(j, a, b);
             const double* da = d + ix(k) + AX * a; const double* db = d + ix(k) + AX * b;
 #pragma unroll
@@ -84,16 +95,16 @@ struct Ctx {
     }
     // (G_k^T s)_(agent a, coordinate i) for a per-constraint weight vector sv (indexed [j], stage k)
     __device__ double GT_entry(const double* gv, const double* sv, int k, int a, int i) const {
-        const double* g = gv + (k - 1) * pb.ng * PD;
+        const double* g = gv + (k - 1) * pb->ng * PD;
         double s = 0.0;
-        if (pb.family == JIPM_FAM_MULTIQUAD) {
-            for (int j = 0; j < pb.ng; ++j) {
+        if (pb->family == JIPM_FAM_MULTIQUAD) {
+            for (int j = 0; j < pb->ng; ++j) {
                 int pa, pb2; pair_ab(j, pa, pb2);
                 if (pa == a) s += g[j * PD + i] * sv[j];
                 else if (pb2 == a) s -= g[j * PD + i] * sv[j];
             }
         } else {
-            for (int j = 0; j < pb.ng; ++j) s += g[j * PD + i] * sv[j];
+            for (int j = 0; j < pb->ng; ++j) s += g[j * PD + i] * sv[j];
         }
         return s;
     }
@@ -101,10 +112,10 @@ struct Ctx {
     // ---- f, c at a point (line-search trial evaluation) --------------------------------
     // returns f; writes c[m]; theta = ||c||_1, cmax = ||c||_inf; fin = all finite
     __device__ double eval_fc(const double* x, double* c, double& theta, double& cmax, bool& fin) const {
-        const int N = pb.N;
+        const int N = pb->N;
         double f = 0.0;
-        const double* tgt = ws + L.tgt;
-        for (int it = lane; it < (N + 1) * NA; it += 32) {
+        const double* tgt = v(L->tgt);
+        for (int it = lane; it < (N + 1) * NA; it += NT) {
             const int k = it / NA, a = it % NA;
             const double* p = x + ix(k) + AX * a;
             double s = 0.0;
@@ -112,50 +123,50 @@ struct Ctx {
             for (int i = 0; i < PD; ++i) { double d = p[i] - tgt[it * PD + i]; s += d * d; }
             f += s;
         }
-        for (int it = lane; it < N * NU; it += 32) {
+        for (int it = lane; it < N * NU; it += NT) {
             const double u = x[iu(it / NU) + it % NU];
-            f += pb.ru * (u * u);
+            f += pb->ru * (u * u);
         }
-        f = wsum(f);
+        f = tm.sum(f);
         double th1 = 0.0, cm = 0.0;
-        for (int i = lane; i < NX; i += 32) {
+        for (int i = lane; i < NX; i += NT) {
             const double v = x[i] - th[i];
             c[i] = v; th1 += fabs(v); cm = fmax(cm, fabs(v));
         }
-        for (int it = lane; it < N * NA; it += 32) {
+        for (int it = lane; it < N * NA; it += NT) {
             const int k = it / NA, a = it % NA;
             double xa[AX], ua[AU], Fv[AX];
 #pragma unroll
             for (int i = 0; i < AX; ++i) xa[i] = x[ix(k) + AX * a + i];
 #pragma unroll
             for (int i = 0; i < AU; ++i) ua[i] = x[iu(k) + AU * a + i];
-            C::Dyn::F(xa, ua, pb.dt, Fv);
+            C::Dyn::F(xa, ua, pb->dt, Fv);
 #pragma unroll
             for (int i = 0; i < AX; ++i) {
                 const double v = x[ix(k + 1) + AX * a + i] - Fv[i];
                 c[icd(k + 1) + AX * a + i] = v; th1 += fabs(v); cm = fmax(cm, fabs(v));
             }
         }
-        for (int it = lane; it < N * pb.ng; it += 32) {
-            const int k = it / pb.ng + 1, j = it % pb.ng;
+        for (int it = lane; it < N * pb->ng; it += NT) {
+            const int k = it / pb->ng + 1, j = it % pb->ng;
             const double v = ineq_val(x, k, j) - x[is(k) + j];
             c[icg(k) + j] = v; th1 += fabs(v); cm = fmax(cm, fabs(v));
         }
-        theta = wsum(th1);
-        cmax = wmax(cm);
+        theta = tm.sum(th1);
+        cmax = tm.max(cm);
         fin = isfinite(f) && isfinite(theta);
-        __syncwarp();
+        tm.sync();
         return f;
     }
 
     // ---- A d (m-vector) and A^T y (n-vector) with the stage blocks J_k and the inequality gradients -----
     __device__ void A_mul(const double* d, double* out) const {
-        const double* gv = ws + L.gv;
-        for (int r = lane; r < pb.m; r += 32) {
+        const double* gv = v(L->gv);
+        for (int r = lane; r < pb->m; r += NT) {
             double s;
             if (r < NX) s = d[r];
             else {
-                const int q = r - NX, k = q / pb.cblk, rr = q % pb.cblk;
+                const int q = r - NX, k = q / pb->cblk, rr = q % pb->cblk;
                 if (rr < NX) {
                     const double* Jr = Jk(k) + rr * NZ;
                     s = d[ix(k + 1) + rr];
@@ -171,20 +182,20 @@ struct Ctx {
             }
             out[r] = s;
         }
-        __syncwarp();
+        tm.sync();
     }
     __device__ double AT_entry(const double* y, int idx) const {
-        const double* gv = ws + L.gv;
+        const double* gv = v(L->gv);
         int k, a;  // x_k[a] or u_k[a-NX]
         if (idx < NX) { k = 0; a = idx; }
         else {
-            const int q = idx - NX, kk = q / pb.blk, r = q % pb.blk;
+            const int q = idx - NX, kk = q / pb->blk, r = q % pb->blk;
             if (r < NU) { k = kk; a = NX + r; }
             else if (r < NU + NX) { k = kk + 1; a = r - NU; }
             else return -y[icg(kk + 1) + (r - NU - NX)];
         }
         double s = 0.0;
-        if (k < pb.N) {
+        if (k < pb->N) {
             const double* Jc = Jk(k) + a; const double* yn = y + icd(k + 1);
 #pragma unroll 4
             for (int l = 0; l < NX; ++l) s -= Jc[l * NZ] * yn[l];
@@ -201,13 +212,13 @@ struct Ctx {
         int k, a;
         if (idx < NX) { k = 0; a = idx; }
         else {
-            const int q = idx - NX, kk = q / pb.blk, r = q % pb.blk;
+            const int q = idx - NX, kk = q / pb->blk, r = q % pb->blk;
             if (r < NU) { k = kk; a = NX + r; }
             else if (r < NU + NX) { k = kk + 1; a = r - NU; }
             else return 0.0;
         }
         double s = 0.0;
-        if (k < pb.N) {
+        if (k < pb->N) {
             const double* Wr = Wk(k) + a * NZ; const double* dxk = d + ix(k); const double* duk = d + iu(k);
 #pragma unroll 4
             for (int b = 0; b < NX; ++b) s += Wr[b] * dxk[b];

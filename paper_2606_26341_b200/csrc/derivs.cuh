@@ -9,11 +9,11 @@ namespace jipm {
 
 template <class C>
 __device__ void Ctx<C>::dyn_derivs(const double* x, const double* y) {
-    const int N = pb.N;
+    const int N = pb->N;
     if constexpr (std::is_same<typename C::Dyn, PointmassDyn>::value) {
         // linear dynamics: constant Jacobian, zero Hessian
-        const double h = pb.dt;
-        for (int it = lane; it < N * NX * NZ; it += 32) {
+        const double h = pb->dt;
+        for (int it = lane; it < N * NX * NZ; it += NT) {
             const int k = it / (NX * NZ), e = it % (NX * NZ), r = e / NZ, cidx = e % NZ;
             double v = 0.0;
             if (cidx == r) v = 1.0;
@@ -22,16 +22,16 @@ __device__ void Ctx<C>::dyn_derivs(const double* x, const double* y) {
             else if (r >= 2 && cidx == r + 2) v = h;
             Jk(k)[e] = v;
         }
-        for (int it = lane; it < N * NZ * NZ + NX * NX; it += 32) (ws + L.W)[it] = 0.0;
-        __syncwarp();
+        for (int it = lane; it < N * NZ * NZ + NX * NX; it += NT) v(L->W)[it] = 0.0;
+        tm.sync();
     } else {
-        const double h = pb.dt;
-        double* rk = ws + L.rk;
+        const double h = pb->dt;
+        double* rk = v(L->rk);
         if (NA > 1) {
-            for (int it = lane; it < N * NZ * NZ; it += 32) (ws + L.W)[it] = 0.0;
+            for (int it = lane; it < N * NZ * NZ; it += NT) v(L->W)[it] = 0.0;
         }
         // ---- phase 1: lane <-> (stage, agent): RK points, Df entries, adjoints, contracted 7x7 Hessians ----
-        for (int it = lane; it < N * NA; it += 32) {
+        for (int it = lane; it < N * NA; it += NT) {
             const int k = it / NA, a = it % NA;
             double xa[12], ua[4], lam[12], kk[12], xi[12];
             QuadBasics bs[4];
@@ -72,14 +72,15 @@ __device__ void Ctx<C>::dyn_derivs(const double* x, const double* y) {
                 }
             }
         }
-        __syncwarp();
-        // ---- phase 2: half-warp <-> (stage, agent), lane <-> column j of z = (x(12), u(4)) -----------------
-        const int hw = lane >> 4, j = lane & 15;
-        double* sV = sm + C::SM_V - 0;  // staging aliases the M tile region start (M is not live here)
-        sV = sm + C::SM_M + hw * (7 * 16);
+        tm.sync();
+        // ---- phase 2: 16-thread group <-> (stage, agent), thread <-> column j of z = (x(12), u(4)) ----------
+        // (two groups share a warp and run the same instruction stream: __syncwarp orders the staging)
+        const int grp = lane >> 4, j = lane & 15;
+        constexpr int NGRP = NT / 16;
+        double* sV = sm + C::SM_G + grp * (7 * 16);
         const int nit = N * NA;
-        for (int it0 = 0; it0 < nit; it0 += 2) {
-            const int it = it0 + hw;
+        for (int it0 = 0; it0 < nit; it0 += NGRP) {
+            const int it = it0 + grp;
             const bool valid = it < nit;
             const int itc = valid ? it : nit - 1;
             const int k = itc / NA, a = itc % NA;
@@ -134,51 +135,51 @@ __device__ void Ctx<C>::dyn_derivs(const double* x, const double* y) {
                 }
             }
         }
-        for (int it = lane; it < NX * NX; it += 32) Wk(N)[it] = 0.0;
-        __syncwarp();
+        for (int it = lane; it < NX * NX; it += NT) Wk(N)[it] = 0.0;
+        tm.sync();
     }
 }
 
 // grad f, J, W (+ objective and inequality curvature), inequality gradient vectors gv
 template <class C>
 __device__ void Ctx<C>::eval_derivs(const double* x, const double* y, double sigma_f) {
-    const int N = pb.N;
-    double* g = ws + L.g;
-    const double* tgt = ws + L.tgt;
-    for (int i = lane; i < pb.n; i += 32) g[i] = 0.0;
-    __syncwarp();
-    for (int it = lane; it < (N + 1) * NA * PD; it += 32) {
+    const int N = pb->N;
+    double* g = v(L->g);
+    const double* tgt = v(L->tgt);
+    for (int i = lane; i < pb->n; i += NT) g[i] = 0.0;
+    tm.sync();
+    for (int it = lane; it < (N + 1) * NA * PD; it += NT) {
         const int ka = it / PD, i = it % PD, k = ka / NA, a = ka % NA;
         g[ix(k) + AX * a + i] = sigma_f * 2.0 * (x[ix(k) + AX * a + i] - tgt[it]);
     }
-    for (int it = lane; it < N * NU; it += 32) {
+    for (int it = lane; it < N * NU; it += NT) {
         const int idx = iu(it / NU) + it % NU;
-        g[idx] = sigma_f * 2.0 * pb.ru * x[idx];
+        g[idx] = sigma_f * 2.0 * pb->ru * x[idx];
     }
     // inequality gradient vectors
-    double* gv = ws + L.gv;
-    for (int it = lane; it < N * pb.ng; it += 32) {
-        const int k = it / pb.ng + 1, j = it % pb.ng;
-        if (pb.family == JIPM_FAM_MULTIQUAD) {
+    double* gv = v(L->gv);
+    for (int it = lane; it < N * pb->ng; it += NT) {
+        const int k = it / pb->ng + 1, j = it % pb->ng;
+        if (pb->family == JIPM_FAM_MULTIQUAD) {
             int a, b; pair_ab(j, a, b);
 #pragma unroll
             for (int i = 0; i < PD; ++i) gv[it * PD + i] = 2.0 * (x[ix(k) + AX * a + i] - x[ix(k) + AX * b + i]);
         } else {
-            const double* ob = th + pb.th_obs + (PD + 1) * j;
+            const double* ob = th + pb->th_obs + (PD + 1) * j;
 #pragma unroll
             for (int i = 0; i < PD; ++i) gv[it * PD + i] = 2.0 * (x[ix(k) + i] - ob[i]);
         }
     }
     dyn_derivs(x, y);
     // objective curvature (diagonal) and inequality curvature 2 y_g I on positions
-    for (int it = lane; it < (N + 1) * NA * PD; it += 32) {
+    for (int it = lane; it < (N + 1) * NA * PD; it += NT) {
         const int ka = it / PD, i = it % PD, k = ka / NA, a = ka % NA;
         const int r = AX * a + i, ld = (k < N) ? NZ : NX;
         double add = sigma_f * 2.0;
         if (k >= 1) {
             const double* yg = y + icg(k);
-            if (pb.family == JIPM_FAM_MULTIQUAD) {
-                for (int q = 0; q < pb.ng; ++q) {
+            if (pb->family == JIPM_FAM_MULTIQUAD) {
+                for (int q = 0; q < pb->ng; ++q) {
                     int pa, pb2; pair_ab(q, pa, pb2);
                     if (pa == a || pb2 == a) {
                         add += 2.0 * yg[q];
@@ -187,16 +188,16 @@ __device__ void Ctx<C>::eval_derivs(const double* x, const double* y, double sig
                     }
                 }
             } else {
-                for (int q = 0; q < pb.ng; ++q) add += 2.0 * yg[q];
+                for (int q = 0; q < pb->ng; ++q) add += 2.0 * yg[q];
             }
         }
         Wk(k)[r * ld + r] += add;
     }
-    for (int it = lane; it < N * NU; it += 32) {
+    for (int it = lane; it < N * NU; it += NT) {
         const int k = it / NU, r = NX + it % NU;
-        Wk(k)[r * NZ + r] += sigma_f * 2.0 * pb.ru;
+        Wk(k)[r * NZ + r] += sigma_f * 2.0 * pb->ru;
     }
-    __syncwarp();
+    tm.sync();
 }
 
 }  // namespace jipm

@@ -1,9 +1,7 @@
-// inst_pm.cu -- slot kernel instantiation: Cfg<PointmassDyn, 1>.
+// inst_pm.cu -- slot kernel instantiation: PointmassDyn, 1 agent(s), 32 threads per problem slot, >= 16 CTA(s) per SM.
 #include "inst.cuh"
 namespace jipm {
-using C_ = Cfg<PointmassDyn, 1>;
-cudaError_t launch_pm(const Args& a, int wpb, cudaStream_t st) { return launch_cfg<C_>(a, wpb, st); }
-int sm_doubles_pm() { return C_::SM_TOTAL; }
+Inst inst_pm() { return make_inst<Cfg<PointmassDyn, 1, 32>, 16>(); }
 }  // namespace jipm
 
 namespace jipm {

@@ -1,7 +1,5 @@
-// inst_q1.cu -- slot kernel instantiation: Cfg<QuadDyn, 1>.
+// inst_q1.cu -- slot kernel instantiation: QuadDyn, 1 agent(s), 128 threads per problem slot, >= 3 CTA(s) per SM.
 #include "inst.cuh"
 namespace jipm {
-using C_ = Cfg<QuadDyn, 1>;
-cudaError_t launch_q1(const Args& a, int wpb, cudaStream_t st) { return launch_cfg<C_>(a, wpb, st); }
-int sm_doubles_q1() { return C_::SM_TOTAL; }
+Inst inst_q1() { return make_inst<Cfg<QuadDyn, 1, 128>, 3>(); }
 }  // namespace jipm

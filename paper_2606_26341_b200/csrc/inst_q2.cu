@@ -1,7 +1,5 @@
-// inst_q2.cu -- slot kernel instantiation: Cfg<QuadDyn, 2>.
+// inst_q2.cu -- slot kernel instantiation: QuadDyn, 2 agent(s), 128 threads per problem slot, >= 2 CTA(s) per SM.
 #include "inst.cuh"
 namespace jipm {
-using C_ = Cfg<QuadDyn, 2>;
-cudaError_t launch_q2(const Args& a, int wpb, cudaStream_t st) { return launch_cfg<C_>(a, wpb, st); }
-int sm_doubles_q2() { return C_::SM_TOTAL; }
+Inst inst_q2() { return make_inst<Cfg<QuadDyn, 2, 128>, 2>(); }
 }  // namespace jipm

@@ -1,7 +1,5 @@
-// inst_q4.cu -- slot kernel instantiation: Cfg<QuadDyn, 4>.
+// inst_q4.cu -- slot kernel instantiation: QuadDyn, 4 agent(s), 256 threads per problem slot, >= 1 CTA(s) per SM.
 #include "inst.cuh"
 namespace jipm {
-using C_ = Cfg<QuadDyn, 4>;
-cudaError_t launch_q4(const Args& a, int wpb, cudaStream_t st) { return launch_cfg<C_>(a, wpb, st); }
-int sm_doubles_q4() { return C_::SM_TOTAL; }
+Inst inst_q4() { return make_inst<Cfg<QuadDyn, 4, 256>, 1>(); }
 }  // namespace jipm

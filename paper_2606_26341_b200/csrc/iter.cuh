@@ -14,12 +14,12 @@ template <class C>
 struct Solver {
     using X = Ctx<C>;
     using K = Kkt<C>;
-    static constexpr int NX = C::NX, NU = C::NU, NZ = C::NZ, PD = C::PD, AX = C::AX, NA = C::NA;
+    static constexpr int NX = C::NX, NU = C::NU, NZ = C::NZ, PD = C::PD, AX = C::AX, NA = C::NA, NT = C::NT;
     X& c;
-    const Args& A;
-    const Pb& pb;
-    const Lay& L;
-    const jipm_options& o;
+    ArgsProxy A;
+    PbProxy pb;
+    LayProxy L;
+    OptProxy o;
     int lane;
     // warp-uniform scalar state of the problem in this slot
     double mu, tau, dw_last, theta_min, theta_max, f, theta, cmax;
@@ -32,78 +32,78 @@ struct Solver {
     long long pid;
     unsigned n_fact, n_solve, n_deriv, n_fc, n_iter, n_resto;
 
-    __device__ Solver(X& c_, const Args& A_) : c(c_), A(A_), pb(A_.pb), L(A_.L), o(A_.o), lane(c_.lane) {
+    __device__ Solver(X& c_) : c(c_), lane(c_.lane) {
         n_fact = n_solve = n_deriv = n_fc = n_iter = n_resto = 0;
-        mode = 0; nX = pb.n;
+        mode = 0; nX = pb->n;
     }
-    __device__ __forceinline__ double* V(int off) const { return c.ws + off; }
+    __device__ __forceinline__ double* V(int off) const { return c.v(off); }
     // bounds of the extended primal vector: entries >= n are the restoration variables p, n >= 0
-    __device__ __forceinline__ double lo(int i) const { return i < pb.n ? pb.xL[i] : 0.0; }
-    __device__ __forceinline__ double hi(int i) const { return i < pb.n ? pb.xU[i] : INFINITY; }
+    __device__ __forceinline__ double lo(int i) const { return i < pb->n ? pb->xL[i] : 0.0; }
+    __device__ __forceinline__ double hi(int i) const { return i < pb->n ? pb->xU[i] : INFINITY; }
     __device__ __forceinline__ bool hasL(int i) const { return lo(i) > -INFINITY; }
     __device__ __forceinline__ bool hasU(int i) const { return hi(i) < INFINITY; }
-    __device__ __forceinline__ double* filt_active() const { return V(mode ? L.filtR : L.filt); }
+    __device__ __forceinline__ double* filt_active() const { return V(mode ? L->filtR : L->filt); }
 
     // barrier objective (3) with the one-sided damping term; NaN outside the interior
     __device__ double phi(const double* x, double fv, double mu_, int nvar) const {
         double s = 0.0;
         int badpt = 0;
-        for (int i = lane; i < nvar; i += 32) {
+        for (int i = lane; i < nvar; i += NT) {
             const double l = lo(i), u = hi(i), xi = x[i];
             const bool hl = l > -INFINITY, hu = u < INFINITY;
             if (hl) {
                 const double sl = xi - l;
                 if (!(sl > 0.0)) badpt = 1;
                 s -= mu_ * log(sl);
-                if (!hu) s += o.kappa_d * mu_ * sl;
+                if (!hu) s += o->kappa_d * mu_ * sl;
             }
             if (hu) {
                 const double su = u - xi;
                 if (!(su > 0.0)) badpt = 1;
                 s -= mu_ * log(su);
-                if (!hl) s += o.kappa_d * mu_ * su;
+                if (!hl) s += o->kappa_d * mu_ * su;
             }
         }
-        s = wsum(s);
-        if (wor(badpt)) return NAN;
+        s = c.tm.sum(s);
+        if (c.tm.any(badpt)) return NAN;
         return fv + s;
     }
 
     // fraction to the boundary (PAPER.md:148 fn 2) on the primal step
     __device__ double ftb_primal(const double* x, const double* dx, double tau_) const {
         double a = 1.0;
-        for (int i = lane; i < nX; i += 32) {
+        for (int i = lane; i < nX; i += NT) {
             const double l = lo(i), u = hi(i), d = dx[i];
             if (l > -INFINITY && d < 0.0) a = fmin(a, -tau_ * (x[i] - l) / d);
             if (u < INFINITY && d > 0.0) a = fmin(a, tau_ * (u - x[i]) / d);
         }
-        return wmin(a);
+        return c.tm.min(a);
     }
     __device__ double ftb_dual(const double* zL, const double* zU, const double* dzL, const double* dzU,
                                double tau_) const {
         double a = 1.0;
-        for (int i = lane; i < nX; i += 32) {
+        for (int i = lane; i < nX; i += NT) {
             if (hasL(i) && dzL[i] < 0.0) a = fmin(a, -tau_ * zL[i] / dzL[i]);
             if (hasU(i) && dzU[i] < 0.0) a = fmin(a, -tau_ * zU[i] / dzU[i]);
         }
-        return wmin(a);
+        return c.tm.min(a);
     }
 
     // optimality error E_mu from the dual residual base in b1 (= grad f + A^T y - zL + zU)
     __device__ double opt_error(double mu_, double sd, double sc) const {
-        const double* x = V(L.x); const double* zL = V(L.zL); const double* zU = V(L.zU); const double* rdb = V(L.b1);
+        const double* x = V(L->x); const double* zL = V(L->zL); const double* zU = V(L->zU); const double* rdb = V(L->b1);
         double ed = 0.0, es = 0.0;
-        for (int i = lane; i < nX; i += 32) {
+        for (int i = lane; i < nX; i += NT) {
             const double l = lo(i), u = hi(i);
             const bool hl = l > -INFINITY, hu = u < INFINITY;
             double dmp = 0.0;
-            if (hl && !hu) dmp = o.kappa_d * mu_;
-            if (hu && !hl) dmp = -o.kappa_d * mu_;
+            if (hl && !hu) dmp = o->kappa_d * mu_;
+            if (hu && !hl) dmp = -o->kappa_d * mu_;
             ed = fmax(ed, fabs(rdb[i] + dmp));
             if (hl) es = fmax(es, fabs((x[i] - l) * zL[i] - mu_));
             if (hu) es = fmax(es, fabs((u - x[i]) * zU[i] - mu_));
         }
-        ed = wmax(ed); es = wmax(es);
+        ed = c.tm.max(ed); es = c.tm.max(es);
         return fmax(fmax(ed / sd, cmax), es / sc);
     }
 
@@ -111,8 +111,8 @@ struct Solver {
     __device__ bool in_filter_of(const double* F, int nf, double thmax, double th_t, double ph_t) const {
         if (th_t >= thmax) return true;
         int hit = 0;
-        for (int j = lane; j < nf; j += 32) hit |= (th_t >= F[2 * j] && ph_t >= F[2 * j + 1]);
-        return wor(hit);
+        for (int j = lane; j < nf; j += NT) hit |= (th_t >= F[2 * j] && ph_t >= F[2 * j + 1]);
+        return c.tm.any(hit);
     }
     __device__ bool in_filter(double th_t, double ph_t) const {
         return in_filter_of(filt_active(), nfilt, theta_max, th_t, ph_t);
@@ -131,21 +131,20 @@ struct Solver {
             if (nf == MAX_FILTER) nf = MAX_FILTER - 1;  // overflow: the newest old entry is dropped (counted nowhere: never seen)
             F[2 * nf] = th_e; F[2 * nf + 1] = ph_e;
         }
-        nfilt = __shfl_sync(FULL, nf, 0) + 1;
-        __syncwarp();
+        nfilt = c.tm.bcast0(nf) + 1;  // (the reduction's barrier also publishes lane 0's writes)
     }
     __device__ bool switching(double alpha, double g, double theta_k) const {
-        return g < 0.0 && alpha * pow(-g, o.s_phi) > o.delta * pow(theta_k, o.s_theta);
+        return g < 0.0 && alpha * pow(-g, o->s_phi) > o->delta * pow(theta_k, o->s_theta);
     }
     __device__ bool armijo(double phi_t, double phi_k, double alpha, double g) const {
-        return phi_t - phi_k - 10.0 * EPS_MACH * fabs(phi_k) <= o.eta_phi * alpha * g;
+        return phi_t - phi_k - 10.0 * EPS_MACH * fabs(phi_k) <= o->eta_phi * alpha * g;
     }
     __device__ bool acceptable(double th_t, double ph_t, double th_k, double ph_k, double alpha, double g) const {
         if (!(isfinite(th_t) && isfinite(ph_t))) return false;
         if (in_filter(th_t, ph_t)) return false;
         if (th_k <= theta_min && switching(alpha, g, th_k)) return armijo(ph_t, ph_k, alpha, g);
-        return th_t <= (1.0 - o.gamma_theta) * th_k ||
-               ph_t - ph_k - 10.0 * EPS_MACH * fabs(ph_k) <= -o.gamma_phi * th_k;
+        return th_t <= (1.0 - o->gamma_theta) * th_k ||
+               ph_t - ph_k - 10.0 * EPS_MACH * fabs(ph_k) <= -o->gamma_phi * th_k;
     }
 
     // ---- linear algebra of one iteration ---------------------------------------------------------------
@@ -153,78 +152,78 @@ struct Solver {
     // restoration mode the Schur complement 1/Sig_p + 1/Sig_n of the eliminated (p, n) pairs ([7] sec 3.3)
     __device__ void set_sigma(double dw, double dc) {
         dc_cur = dc;
-        const double* x = V(L.x); const double* zL = V(L.zL); const double* zU = V(L.zU);
-        double* Sig = V(L.Sig); double* Hd = V(L.Hd); double* Dc = V(L.Dc);
-        const double* DR2 = V(L.DR2);
-        for (int i = lane; i < nX; i += 32) {
+        const double* x = V(L->x); const double* zL = V(L->zL); const double* zU = V(L->zU);
+        double* Sig = V(L->Sig); double* Hd = V(L->Hd); double* Dc = V(L->Dc);
+        const double* DR2 = V(L->DR2);
+        for (int i = lane; i < nX; i += NT) {
             const double l = lo(i), u = hi(i);
-            const double hd = (mode && i < pb.n) ? dw + zeta * DR2[i] : dw;
+            const double hd = (mode && i < pb->n) ? dw + zeta * DR2[i] : dw;
             double s = hd;
             if (l > -INFINITY) s += zL[i] / (x[i] - l);
             if (u < INFINITY) s += zU[i] / (u - x[i]);
             Sig[i] = s; Hd[i] = hd;
         }
-        __syncwarp();
-        for (int i = lane; i < pb.m; i += 32)
-            Dc[i] = mode ? dc + 1.0 / Sig[pb.n + i] + 1.0 / Sig[pb.n + pb.m + i] : dc;
-        __syncwarp();
+        c.tm.sync();
+        for (int i = lane; i < pb->m; i += NT)
+            Dc[i] = mode ? dc + 1.0 / Sig[pb->n + i] + 1.0 / Sig[pb->n + pb->m + i] : dc;
+        c.tm.sync();
     }
 
     // products with the constraint Jacobian / Lagrangian Hessian of the (extended) problem
     __device__ __forceinline__ double ATx(const double* y, int i) const {
-        if (i < pb.n) return c.AT_entry(y, i);
-        return (i < pb.n + pb.m) ? -y[i - pb.n] : y[i - pb.n - pb.m];
+        if (i < pb->n) return c.AT_entry(y, i);
+        return (i < pb->n + pb->m) ? -y[i - pb->n] : y[i - pb->n - pb->m];
     }
-    __device__ __forceinline__ double Wx(const double* d, int i) const { return i < pb.n ? c.W_entry(d, i) : 0.0; }
+    __device__ __forceinline__ double Wx(const double* d, int i) const { return i < pb->n ? c.W_entry(d, i) : 0.0; }
 
     // solve (6) through (7) + the Delta z recovery of PAPER.md:110 for rhs (b1,b2,b3,b4) -> (d1..d4)
     __device__ void reduced_solve(const double* b1, const double* b2, const double* b3, const double* b4,
                                   double* d1, double* d2, double* d3, double* d4) {
-        const double* x = V(L.x); const double* zL = V(L.zL); const double* zU = V(L.zU);
-        double* rr = V(L.rr);
-        for (int i = lane; i < nX; i += 32) {
+        const double* x = V(L->x); const double* zL = V(L->zL); const double* zU = V(L->zU);
+        double* rr = V(L->rr);
+        for (int i = lane; i < nX; i += NT) {
             const double l = lo(i), u = hi(i);
             double r = b1[i];
             if (l > -INFINITY) r += b3[i] / (x[i] - l);
             if (u < INFINITY) r -= b4[i] / (u - x[i]);
             rr[i] = r;
         }
-        __syncwarp();
+        c.tm.sync();
         const double* rc = b2;
-        const double* Sig = V(L.Sig);
-        const int n = pb.n, m = pb.m;
+        const double* Sig = V(L->Sig);
+        const int n = pb->n, m = pb->m;
         if (mode) {  // eliminate (dp, dn): dp = (r_p + dy)/Sig_p, dn = (r_n - dy)/Sig_n
-            double* rc2 = V(L.rc2);
-            for (int j = lane; j < m; j += 32) rc2[j] = b2[j] + rr[n + j] / Sig[n + j] - rr[n + m + j] / Sig[n + m + j];
-            __syncwarp();
+            double* rc2 = V(L->rc2);
+            for (int j = lane; j < m; j += NT) rc2[j] = b2[j] + rr[n + j] / Sig[n + j] - rr[n + m + j] / Sig[n + m + j];
+            c.tm.sync();
             rc = rc2;
         }
-        K::solve(c, rr, rc, d1, d2);
+        K::solve(c, rr, rc, d1, d2, mode != 0 || dc_cur != 0.0);
         n_solve++;
         if (mode) {
-            for (int j = lane; j < m; j += 32) {
+            for (int j = lane; j < m; j += NT) {
                 d1[n + j] = (rr[n + j] + d2[j]) / Sig[n + j];
                 d1[n + m + j] = (rr[n + m + j] - d2[j]) / Sig[n + m + j];
             }
-            __syncwarp();
+            c.tm.sync();
         }
-        for (int i = lane; i < nX; i += 32) {
+        for (int i = lane; i < nX; i += NT) {
             const double l = lo(i), u = hi(i);
             d3[i] = (l > -INFINITY) ? (b3[i] - zL[i] * d1[i]) / (x[i] - l) : 0.0;
             d4[i] = (u < INFINITY) ? (b4[i] + zU[i] * d1[i]) / (u - x[i]) : 0.0;
         }
-        __syncwarp();
+        c.tm.sync();
     }
 
     // residual of the unreduced system (6): r = b - M d; returns ||r||_inf; dnorm = ||d||_inf
     __device__ double full_residual(const double* b1, const double* b2, const double* b3, const double* b4,
                                     const double* d1, const double* d2, const double* d3, const double* d4,
                                     double& dnorm) const {
-        const double* x = V(L.x); const double* zL = V(L.zL); const double* zU = V(L.zU);
-        const double* Hd = V(L.Hd);
-        double* r1 = V(L.r1); double* r2 = V(L.r2); double* r3 = V(L.r3); double* r4 = V(L.r4);
+        const double* x = V(L->x); const double* zL = V(L->zL); const double* zU = V(L->zU);
+        const double* Hd = V(L->Hd);
+        double* r1 = V(L->r1); double* r2 = V(L->r2); double* r3 = V(L->r3); double* r4 = V(L->r4);
         double rn = 0.0, dn = 0.0;
-        for (int i = lane; i < nX; i += 32) {
+        for (int i = lane; i < nX; i += NT) {
             const double l = lo(i), u = hi(i);
             const double lhs1 = Wx(d1, i) + Hd[i] * d1[i] + ATx(d2, i) - d3[i] + d4[i];
             const double v1 = b1[i] - lhs1;
@@ -237,15 +236,15 @@ struct Solver {
             dn = fmax(dn, fmax(fabs(d1[i]), fmax(fabs(d3[i]), fabs(d4[i]))));
         }
         c.A_mul(d1, r2);
-        for (int i = lane; i < pb.m; i += 32) {
+        for (int i = lane; i < pb->m; i += NT) {
             double ad = r2[i];
-            if (mode) ad += d1[pb.n + pb.m + i] - d1[pb.n + i];
+            if (mode) ad += d1[pb->n + pb->m + i] - d1[pb->n + i];
             const double v2 = b2[i] - (ad - dc_cur * d2[i]);
             r2[i] = v2; rn = fmax(rn, fabs(v2)); dn = fmax(dn, fabs(d2[i]));
         }
-        __syncwarp();
-        dnorm = wmax(dn);
-        return wmax(rn);
+        c.tm.sync();
+        dnorm = c.tm.max(dn);
+        return c.tm.max(rn);
     }
 
     // solve (6) with iterative refinement on the unreduced system (reading S-7); returns #refinements
@@ -253,27 +252,27 @@ struct Solver {
                               double* d1, double* d2, double* d3, double* d4) {
         reduced_solve(b1, b2, b3, b4, d1, d2, d3, d4);
         double bn = 0.0;
-        for (int i = lane; i < nX; i += 32) bn = fmax(bn, fmax(fabs(b1[i]), fmax(fabs(b3[i]), fabs(b4[i]))));
-        for (int i = lane; i < pb.m; i += 32) bn = fmax(bn, fabs(b2[i]));
-        bn = wmax(bn);
+        for (int i = lane; i < nX; i += NT) bn = fmax(bn, fmax(fabs(b1[i]), fmax(fabs(b3[i]), fabs(b4[i]))));
+        for (int i = lane; i < pb->m; i += NT) bn = fmax(bn, fabs(b2[i]));
+        bn = c.tm.max(bn);
         int nref = 0;
-        double* e1 = V(L.e1); double* e2 = V(L.e2); double* e3 = V(L.e3); double* e4 = V(L.e4);
-        while (nref < o.refine_max) {
+        double* e1 = V(L->e1); double* e2 = V(L->e2); double* e3 = V(L->e3); double* e4 = V(L->e4);
+        while (nref < o->refine_max) {
             double dn;
             const double rn = full_residual(b1, b2, b3, b4, d1, d2, d3, d4, dn);
-            if (nref >= o.refine_min && rn <= o.residual_ratio_max * (bn + dn)) break;
-            reduced_solve(V(L.r1), V(L.r2), V(L.r3), V(L.r4), e1, e2, e3, e4);
-            for (int i = lane; i < nX; i += 32) { d1[i] += e1[i]; d3[i] += e3[i]; d4[i] += e4[i]; }
-            for (int i = lane; i < pb.m; i += 32) d2[i] += e2[i];
-            __syncwarp();
+            if (nref >= o->refine_min && rn <= o->residual_ratio_max * (bn + dn)) break;
+            reduced_solve(V(L->r1), V(L->r2), V(L->r3), V(L->r4), e1, e2, e3, e4);
+            for (int i = lane; i < nX; i += NT) { d1[i] += e1[i]; d3[i] += e3[i]; d4[i] += e4[i]; }
+            for (int i = lane; i < pb->m; i += NT) d2[i] += e2[i];
+            c.tm.sync();
             nref++;
         }
         return nref;
     }
 
     __device__ void trace_put(const double* rec) {
-        if (A.trace != nullptr && nrec < A.trace_cap && lane < JIPM_TRACE_W)
-            A.trace[(pid * A.trace_cap + nrec) * JIPM_TRACE_W + lane] = rec[lane];
+        if (A->trace != nullptr && nrec < A->trace_cap && lane < JIPM_TRACE_W)
+            A->trace[(pid * A->trace_cap + nrec) * JIPM_TRACE_W + lane] = rec[lane];
         nrec++;
     }
 

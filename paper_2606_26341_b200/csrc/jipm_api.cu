@@ -26,7 +26,9 @@ struct jipm_solver {
     jipm_options o;
     Pb pb;
     Lay L;
-    int NX, NU, NZ, sm_per_warp, warps_per_block;
+    int NX, NU, NZ;
+    Inst inst;
+    int teams_per_sm;
     int n_slots;
     cudaStream_t stream;
     double *d_xL = nullptr, *d_xU = nullptr, *d_ws = nullptr;
@@ -85,39 +87,47 @@ extern "C" int jipm_family_sizes(int family, const jipm_family_dims* d, int64_t*
     return JIPM_OK;
 }
 
-static void build_layout(jipm_solver* s) {
+// Workspace layout of one slot.  Arrays are laid out in PRIORITY order; the first L.nsm doubles (as many whole
+// arrays as the shared-memory budget holds) live in shared memory, the rest in the slot's global scratch.
+static void build_layout(jipm_solver* s, int sm_budget_doubles) {
     const Pb& pb = s->pb;
     const int n = pb.n, m = pb.m, N = pb.N, NX = s->NX, NU = s->NU, NZ = s->NZ;
     const int pd = (pb.family == JIPM_FAM_POINTMASS2D) ? 2 : 3;
-    int o = 0;
-    auto take = [&](int cnt) { int r = o; o += (cnt + 1) & ~1; return r; };  // keep 16-byte alignment
-    Lay& L = s->L;
     const int nX = n + 2 * m;  // restoration mode iterates on X = [x; p; n]
-    L.x = take(nX); L.y = take(m); L.zL = take(nX); L.zU = take(nX); L.g = take(nX); L.c = take(m);
-    L.gv = take(N * pb.ng * pd); L.tgt = take((N + 1) * pb.na * pd);
-    L.J = take(N * NX * NZ); L.W = take(N * NZ * NZ + NX * NX);
-    L.Sig = take(nX); L.Hd = take(nX); L.Dc = take(m);
-    L.T = take((N + 1) * NX * NX); L.Xf = take(N * NX * NU); L.Lf = take(N * NU * NU);
-    L.wv = take(N * NX); L.tv = take(N * NU);
-    L.b1 = take(nX); L.b2 = take(m); L.b3 = take(nX); L.b4 = take(nX);
-    L.dx = take(nX); L.dy = take(m); L.dzL = take(nX); L.dzU = take(nX);
-    L.r1 = take(nX); L.r2 = take(m); L.r3 = take(nX); L.r4 = take(nX);
-    L.e1 = take(nX); L.e2 = take(m); L.e3 = take(nX); L.e4 = take(nX);
-    L.sx = take(nX); L.sy = take(m); L.szL = take(nX); L.szU = take(nX);
-    L.xt = take(nX); L.ct = take(m); L.csoc = take(m); L.bs2 = take(m); L.rr = take(nX);
-    L.rk = take(pb.family == JIPM_FAM_POINTMASS2D ? 0 : N * pb.na * 4 * RKW);
-    L.filt = take(2 * MAX_FILTER);
-    L.xR = take(n); L.DR2 = take(n); L.filtR = take(2 * MAX_FILTER); L.rc2 = take(m);
+    Lay& L = s->L;
+    struct Ent { int Lay::*f; int cnt; };
+    const int rkn = pb.family == JIPM_FAM_POINTMASS2D ? 0 : N * pb.na * 4 * RKW;
+    const Ent order[] = {
+        // the factor and what every solve streams through
+        {&Lay::Psi, N * NX * NX}, {&Lay::pv, (N + 1) * NX}, {&Lay::qv, N * NX}, {&Lay::wv, N * NX}, {&Lay::sv, N * NX}, {&Lay::tv, N * NU},
+        {&Lay::T, (N + 1) * NX * NX}, {&Lay::Kf, N * NU * NX}, {&Lay::Gf, N * NU * NU},
+        {&Lay::J, N * NX * NZ}, {&Lay::Dc, m}, {&Lay::gv, N * pb.ng * pd}, {&Lay::tgt, (N + 1) * pb.na * pd},
+        {&Lay::filt, 2 * MAX_FILTER}, {&Lay::filtR, 2 * MAX_FILTER},
+        // m-vectors
+        {&Lay::y, m}, {&Lay::c, m}, {&Lay::b2, m}, {&Lay::dy, m}, {&Lay::rc2, m}, {&Lay::ct, m}, {&Lay::r2, m}, {&Lay::e2, m},
+        {&Lay::W, N * NZ * NZ + NX * NX},
+        // primal-sized vectors (n + 2m entries: the tail is only touched in restoration mode)
+        {&Lay::x, nX}, {&Lay::rr, nX}, {&Lay::dx, nX}, {&Lay::Sig, nX}, {&Lay::xt, nX}, {&Lay::zL, nX}, {&Lay::zU, nX},
+        {&Lay::b1, nX}, {&Lay::b3, nX}, {&Lay::b4, nX}, {&Lay::dzL, nX}, {&Lay::dzU, nX}, {&Lay::g, nX}, {&Lay::Hd, nX},
+        {&Lay::r1, nX}, {&Lay::r3, nX}, {&Lay::r4, nX}, {&Lay::e1, nX}, {&Lay::e3, nX}, {&Lay::e4, nX},
+        {&Lay::rk, rkn},
+        {&Lay::sx, nX}, {&Lay::sy, m}, {&Lay::szL, nX}, {&Lay::szU, nX}, {&Lay::csoc, m}, {&Lay::bs2, m},
+        {&Lay::xR, n}, {&Lay::DR2, n},
+    };
+    int o = 0;
+    L.nsm = 0;
+    bool in_sm = true;
+    for (const Ent& e : order) {
+        const int cnt = (e.cnt + 1) & ~1;  // keep 16-byte alignment
+        if (in_sm && o + cnt > sm_budget_doubles) { in_sm = false; L.nsm = o; }
+        L.*(e.f) = o;
+        o += cnt;
+    }
+    if (in_sm) L.nsm = o;
     L.total = o;
 }
 
-static cudaError_t dispatch(jipm_solver* s, const Args& a) {
-    const int wpb = s->warps_per_block;
-    if (s->family == JIPM_FAM_POINTMASS2D) return launch_pm(a, wpb, s->stream);
-    if (s->family == JIPM_FAM_MULTIQUAD)
-        return s->dims.n_agents == 4 ? launch_q4(a, wpb, s->stream) : launch_q2(a, wpb, s->stream);
-    return launch_q1(a, wpb, s->stream);
-}
+static cudaError_t dispatch(jipm_solver* s, const Args& a) { return s->inst.launch(a, s->stream); }
 
 extern "C" int jipm_create(jipm_solver** out, int family, const jipm_family_dims* d, int64_t n, int64_t m,
                            const double* x_L, const double* x_U, const jipm_options* opts, int64_t resident_slots,
@@ -155,29 +165,26 @@ extern "C" int jipm_create(jipm_solver** out, int family, const jipm_family_dims
         if (l >= u) { delete s; return fail(JIPM_ERR_BOUNDS, "x_L >= x_U on a component"); }
         xl[i] = l; xu[i] = u;
     }
-    build_layout(s);
-    s->dbg = make_dbglay(pb.n, pb.m, pb.N, s->NX, s->NZ);
-    if (family == JIPM_FAM_POINTMASS2D) s->sm_per_warp = sm_doubles_pm();
-    else if (family == JIPM_FAM_MULTIQUAD) s->sm_per_warp = d->n_agents == 4 ? sm_doubles_q4() : sm_doubles_q2();
-    else s->sm_per_warp = sm_doubles_q1();
+    if (family == JIPM_FAM_POINTMASS2D) s->inst = inst_pm();
+    else if (family == JIPM_FAM_MULTIQUAD) s->inst = d->n_agents == 4 ? inst_q4() : inst_q2();
+    else s->inst = inst_q1();
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, 0) != cudaSuccess) { delete s; return fail(JIPM_ERR_CUDA, "cudaGetDeviceProperties"); }
-    const size_t smw = (size_t)s->sm_per_warp * sizeof(double);
-    int wpb = 4;
-    while (wpb > 1 && wpb * smw > (size_t)prop.sharedMemPerBlockOptin) wpb >>= 1;
-    if (wpb * smw > (size_t)prop.sharedMemPerBlockOptin) { delete s; return fail(JIPM_ERR_NOMEM, "stage tile does not fit shared memory"); }
-    s->warps_per_block = wpb;
-    if (resident_slots == 0) {
-        // fill the GPU: as many warps per SM as shared memory and a 16-warp cap allow
-        int per_sm = (int)std::min<size_t>(16, (size_t)prop.sharedMemPerMultiprocessor / (smw + 256));
-        per_sm = std::max(per_sm / wpb * wpb, wpb);
-        resident_slots = (int64_t)per_sm * prop.multiProcessorCount;
-    }
+    // shared-memory budget per team: the SM's shared memory split over the CTAs the kernel was compiled to co-run
+    // (register budget of __launch_bounds__), minus the fixed tiles and 1 KB of per-CTA reservation
+    s->teams_per_sm = std::max(1, std::min(s->inst.info.min_blocks, 2048 / s->inst.info.nt));
+    const long per_team = std::min<long>((long)prop.sharedMemPerMultiprocessor / s->teams_per_sm - 1024,
+                                         (long)prop.sharedMemPerBlockOptin);
+    const long budget = per_team / (long)sizeof(double) - s->inst.info.sm_fixed;
+    if (budget < 0) { delete s; return fail(JIPM_ERR_NOMEM, "stage tiles do not fit shared memory"); }
+    build_layout(s, (int)budget);
+    s->dbg = make_dbglay(pb.n, pb.m, pb.N, s->NX, s->NZ);
+    if (resident_slots == 0) resident_slots = (int64_t)s->teams_per_sm * prop.multiProcessorCount;  // fill the GPU
     s->n_slots = (int)resident_slots;
     cudaError_t e;
     if ((e = cudaMalloc(&s->d_xL, n * sizeof(double))) != cudaSuccess ||
         (e = cudaMalloc(&s->d_xU, n * sizeof(double))) != cudaSuccess ||
-        (e = cudaMalloc(&s->d_ws, (size_t)s->n_slots * s->L.total * sizeof(double))) != cudaSuccess ||
+        (e = cudaMalloc(&s->d_ws, (size_t)s->n_slots * (s->L.total - s->L.nsm + 2) * sizeof(double))) != cudaSuccess ||
         (e = cudaMalloc(&s->d_queue, sizeof(int))) != cudaSuccess ||
         (e = cudaMalloc(&s->d_stats, 8 * sizeof(unsigned long long))) != cudaSuccess) {
         std::string msg = std::string("cudaMalloc: ") + cudaGetErrorString(e);
@@ -187,7 +194,7 @@ extern "C" int jipm_create(jipm_solver** out, int family, const jipm_family_dims
     pb.xL = s->d_xL; pb.xU = s->d_xU;
     if ((e = cudaMemcpyAsync(s->d_xL, xl.data(), n * sizeof(double), cudaMemcpyHostToDevice, s->stream)) != cudaSuccess ||
         (e = cudaMemcpyAsync(s->d_xU, xu.data(), n * sizeof(double), cudaMemcpyHostToDevice, s->stream)) != cudaSuccess ||
-        (e = cudaMemsetAsync(s->d_ws, 0, (size_t)s->n_slots * s->L.total * sizeof(double), s->stream)) != cudaSuccess ||
+        (e = cudaMemsetAsync(s->d_ws, 0, (size_t)s->n_slots * (s->L.total - s->L.nsm + 2) * sizeof(double), s->stream)) != cudaSuccess ||
         (e = cudaStreamSynchronize(s->stream)) != cudaSuccess) {
         std::string msg = std::string("upload: ") + cudaGetErrorString(e);
         jipm_destroy(s);
@@ -206,7 +213,7 @@ extern "C" int jipm_destroy(jipm_solver* s) {
 
 static int run(jipm_solver* s, Args& a) {
     a.pb = s->pb; a.L = s->L; a.o = s->o;
-    a.ws = s->d_ws; a.ws_stride = s->L.total; a.n_slots = (int)std::min<int64_t>(s->n_slots, std::max<int64_t>(a.P, 1));
+    a.ws = s->d_ws; a.ws_stride = s->L.total - s->L.nsm + 2; a.n_slots = (int)std::min<int64_t>(s->n_slots, std::max<int64_t>(a.P, 1));
     a.queue = s->d_queue; a.stats = s->d_stats;
     a.trace = s->trace; a.trace_cap = s->trace_cap;
     a.dbg_len = s->dbg.len;

@@ -1,4 +1,4 @@
-// kernel.cuh -- the persistent slot kernel: one warp per resident slot; a slot pops problem ids from the queue
+// kernel.cuh -- the persistent slot kernel: one team (CTA) per resident slot; a slot pops problem ids from the queue
 // until it is empty (iteration-level batching: a finished problem is replaced at once, no
 // slot ever waits for a straggler).  Also the debug load/store used by the parity tests.
 #pragma once
@@ -8,98 +8,100 @@ namespace jipm {
 
 template <class C>
 __device__ void Solver<C>::dbg_load(const double* st) {
-    const DbgLay D = make_dbglay(pb.n, pb.m, pb.N, NX, NZ);
-    double* x = V(L.x); double* y = V(L.y); double* zL = V(L.zL); double* zU = V(L.zU);
-    for (int i = lane; i < pb.n; i += 32) { x[i] = st[D.x + i]; zL[i] = st[D.zL + i]; zU[i] = st[D.zU + i]; }
-    for (int i = lane; i < pb.m; i += 32) y[i] = st[D.y + i];
-    for (int i = lane; i < 2 * MAX_FILTER; i += 32) V(L.filt)[i] = st[D.filt + i];
-    mode = 0; nX = pb.n;
+    const DbgLay D = make_dbglay(pb->n, pb->m, pb->N, NX, NZ);
+    double* x = V(L->x); double* y = V(L->y); double* zL = V(L->zL); double* zU = V(L->zU);
+    for (int i = lane; i < pb->n; i += NT) { x[i] = st[D.x + i]; zL[i] = st[D.zL + i]; zU[i] = st[D.zU + i]; }
+    for (int i = lane; i < pb->m; i += NT) y[i] = st[D.y + i];
+    for (int i = lane; i < 2 * MAX_FILTER; i += NT) V(L->filt)[i] = st[D.filt + i];
+    mode = 0; nX = pb->n;
     mu = st[D.sc + 0]; tau = st[D.sc + 1]; dw_last = st[D.sc + 2];
     theta_min = st[D.sc + 3]; theta_max = st[D.sc + 4];
     k = (int)st[D.sc + 5]; status = (int)st[D.sc + 6]; nfilt = (int)st[D.sc + 7];
-    __syncwarp();
+    c.tm.sync();
     bool fin;
-    f = c.eval_fc(x, V(L.c), theta, cmax, fin);
+    f = c.eval_fc(x, V(L->c), theta, cmax, fin);
 }
 
 template <class C>
 __device__ void Solver<C>::dbg_store(double* st) {
-    const DbgLay D = make_dbglay(pb.n, pb.m, pb.N, NX, NZ);
-    __syncwarp();
-    for (int i = lane; i < pb.n; i += 32) {
-        st[D.x + i] = V(L.x)[i]; st[D.zL + i] = V(L.zL)[i]; st[D.zU + i] = V(L.zU)[i];
-        st[D.dx + i] = V(L.dx)[i]; st[D.dzL + i] = V(L.dzL)[i]; st[D.dzU + i] = V(L.dzU)[i];
-        st[D.g + i] = V(L.g)[i];
+    const DbgLay D = make_dbglay(pb->n, pb->m, pb->N, NX, NZ);
+    c.tm.sync();
+    for (int i = lane; i < pb->n; i += NT) {
+        st[D.x + i] = V(L->x)[i]; st[D.zL + i] = V(L->zL)[i]; st[D.zU + i] = V(L->zU)[i];
+        st[D.dx + i] = V(L->dx)[i]; st[D.dzL + i] = V(L->dzL)[i]; st[D.dzU + i] = V(L->dzU)[i];
+        st[D.g + i] = V(L->g)[i];
     }
-    for (int i = lane; i < pb.m; i += 32) {
-        st[D.y + i] = V(L.y)[i]; st[D.dy + i] = V(L.dy)[i]; st[D.c + i] = V(L.c)[i];
+    for (int i = lane; i < pb->m; i += NT) {
+        st[D.y + i] = V(L->y)[i]; st[D.dy + i] = V(L->dy)[i]; st[D.c + i] = V(L->c)[i];
     }
-    for (int i = lane; i < 2 * MAX_FILTER; i += 32) st[D.filt + i] = V(L.filt)[i];
-    for (int i = lane; i < pb.N * NX * NZ; i += 32) st[D.J + i] = V(L.J)[i];
-    for (int i = lane; i < pb.N * NZ * NZ + NX * NX; i += 32) st[D.W + i] = V(L.W)[i];
+    for (int i = lane; i < 2 * MAX_FILTER; i += NT) st[D.filt + i] = V(L->filt)[i];
+    for (int i = lane; i < pb->N * NX * NZ; i += NT) st[D.J + i] = V(L->J)[i];
+    for (int i = lane; i < pb->N * NZ * NZ + NX * NX; i += NT) st[D.W + i] = V(L->W)[i];
     if (lane == 0) {
         st[D.sc + 0] = mu; st[D.sc + 1] = tau; st[D.sc + 2] = dw_last; st[D.sc + 3] = theta_min;
         st[D.sc + 4] = theta_max; st[D.sc + 5] = k; st[D.sc + 6] = status; st[D.sc + 7] = nfilt;
     }
 }
 
-template <class C>
-__global__ void __launch_bounds__(128) jipm_slot_kernel(const __grid_constant__ Args A) {
+template <class C, int MINB>
+__global__ void __launch_bounds__(C::NT, MINB) jipm_slot_kernel() {
     extern __shared__ double smem[];
-    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-    const int slot = blockIdx.x * (blockDim.x >> 5) + wib;
-    if (slot >= A.n_slots) return;
-    double* ws = A.ws + (int64_t)slot * A.ws_stride;
-    Ctx<C> ctx(A.pb, A.L, A.o, ws, smem + wib * C::SM_TOTAL, lane);
-    Solver<C> S(ctx, A);
+    constexpr int NT = C::NT;
+    const ArgsProxy A;
+    const int lane = threadIdx.x;  // one team per CTA
+    const int slot = blockIdx.x;
+    double* ws = A->ws + (int64_t)slot * A->ws_stride;
+    Ctx<C> ctx(ws, smem, lane, 1);
+    Solver<C> S(ctx);
     while (true) {
         int id = 0;
-        if (lane == 0) id = atomicAdd(A.queue, 1);
-        id = __shfl_sync(FULL, id, 0);
-        if (id >= A.P) break;
-        if (A.dbg_mode == 2) {
+        if (lane == 0) id = atomicAdd(A->queue, 1);
+        id = ctx.tm.bcast0(id);
+        if (id >= A->P) break;
+        if (A->dbg_mode == 2) {
             S.pid = id; S.nrec = 0;
-            ctx.th = A.th + (int64_t)id * A.pb.nth;
+            ctx.th = A->th + (int64_t)id * A->pb.nth;
             // targets and J zeroing as in init
             {
-                const Pb& pb = A.pb;
-                double* tgt = ws + A.L.tgt;
-                for (int it = lane; it < (pb.N + 1) * C::NA; it += 32) {
+                const PbProxy pb;
+                double* tgt = ctx.v(A->L.tgt);
+                for (int it = lane; it < (pb->N + 1) * C::NA; it += NT) {
                     const int kk = it / C::NA, a = it % C::NA;
-                    if (pb.family == JIPM_FAM_QUAD_TRACK) {
+                    if (pb->family == JIPM_FAM_QUAD_TRACK) {
                         const double rho = ctx.th[12], phase = ctx.th[13];
-                        const double ang = phase + 1.5 * (kk * pb.dt) / rho;
+                        const double ang = phase + 1.5 * (kk * pb->dt) / rho;
                         tgt[it * C::PD + 0] = rho * cos(ang); tgt[it * C::PD + 1] = rho * sin(ang);
                         if (C::PD > 2) tgt[it * C::PD + 2] = 0.0;
                     } else {
-                        for (int i = 0; i < C::PD; ++i) tgt[it * C::PD + i] = ctx.th[pb.th_goal + C::PD * a + i];
+                        for (int i = 0; i < C::PD; ++i) tgt[it * C::PD + i] = ctx.th[pb->th_goal + C::PD * a + i];
                     }
                 }
                 if (C::NA > 1)
-                    for (int it = lane; it < pb.N * C::NX * C::NZ; it += 32) (ws + A.L.J)[it] = 0.0;
-                __syncwarp();
+                    for (int it = lane; it < pb->N * C::NX * C::NZ; it += NT) ctx.v(A->L.J)[it] = 0.0;
+                ctx.tm.sync();
             }
-            S.dbg_load(A.dbg_state + (int64_t)id * A.dbg_len);
-            for (int s = 0; s < A.dbg_steps && S.status == JIPM_ST_NOT_RUN; ++s) S.iterate();
-            S.dbg_store(A.dbg_state + (int64_t)id * A.dbg_len);
+            ctx.tm.sync();
+            S.dbg_load(A->dbg_state + (int64_t)id * A->dbg_len);
+            for (int s = 0; s < A->dbg_steps && S.status == JIPM_ST_NOT_RUN; ++s) S.iterate();
+            S.dbg_store(A->dbg_state + (int64_t)id * A->dbg_len);
         } else {
             S.init_problem(id);
-            if (A.dbg_mode == 1) {
-                S.dbg_store(A.dbg_state + (int64_t)id * A.dbg_len);
+            if (A->dbg_mode == 1) {
+                S.dbg_store(A->dbg_state + (int64_t)id * A->dbg_len);
             } else {
                 while (S.status == JIPM_ST_NOT_RUN) S.iterate();
                 S.write_outputs();
             }
         }
-        __syncwarp();
+        ctx.tm.sync();
     }
     if (lane == 0) {
-        atomicAdd(&A.stats[0], (unsigned long long)S.n_iter);
-        atomicAdd(&A.stats[1], (unsigned long long)S.n_fact);
-        atomicAdd(&A.stats[2], (unsigned long long)S.n_solve);
-        atomicAdd(&A.stats[3], (unsigned long long)S.n_deriv);
-        atomicAdd(&A.stats[4], (unsigned long long)S.n_fc);
-        atomicAdd(&A.stats[7], (unsigned long long)S.n_resto);
+        atomicAdd(&A->stats[0], (unsigned long long)S.n_iter);
+        atomicAdd(&A->stats[1], (unsigned long long)S.n_fact);
+        atomicAdd(&A->stats[2], (unsigned long long)S.n_solve);
+        atomicAdd(&A->stats[3], (unsigned long long)S.n_deriv);
+        atomicAdd(&A->stats[4], (unsigned long long)S.n_fc);
+        atomicAdd(&A->stats[7], (unsigned long long)S.n_resto);
     }
 }
 

@@ -12,6 +12,14 @@
 //   3. the control block Rt_k = R_k + B^T T_{k+1} B by an unpivoted LDL^T: its pivot signs carry the inertia test.
 // By Haynsworth additivity the KKT matrix has inertia (n, m, 0) iff every Rt_k pivot (and every pivot of
 // I + E P E when D != 0) is positive.
+//
+// What the factor stores per stage k (so that a solve is two sweeps of ONE nx-by-nx product per stage plus
+// stage-parallel work):
+//   T_k   = (I + P_k D_k)^{-1} P_k                       nx x nx, k = 0..N
+//   Kf_k  = Rt_k^{-1} M_ux            (feedback)         nu x nx
+//   G_k   = Rt_k^{-1}                                    nu x nu
+//   Psi_k = (I - D_{k+1} T_{k+1}) (A_k - B_k Kf_k)       nx x nx   (closed-loop transition)
+// All loops are element-parallel over the team (thread <-> tile element), one barrier per dependent phase.
 #pragma once
 #include "core.cuh"
 
@@ -19,198 +27,237 @@ namespace jipm {
 
 template <class C>
 struct Kkt {
-    static constexpr int NX = C::NX, NU = C::NU, NZ = C::NZ, PD = C::PD, AX = C::AX, NA = C::NA;
+    static constexpr int NX = C::NX, NU = C::NU, NZ = C::NZ, PD = C::PD, AX = C::AX, NA = C::NA, NT = C::NT;
     using X = Ctx<C>;
 
-    // Dg weights of the condensed (slack, multiplier) pairs of stage k into sv-style scratch: returns for (k,j)
+    // dot product of length n with 4 independent partial sums (dependent-chain latency / 4)
+    __device__ static __forceinline__ double dot4(const double* a, int sa, const double* b, int sb, int n) {
+        double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+        int l = 0;
+        for (; l + 3 < n; l += 4) {
+            s0 = fma(a[l * sa], b[l * sb], s0);
+            s1 = fma(a[(l + 1) * sa], b[(l + 1) * sb], s1);
+            s2 = fma(a[(l + 2) * sa], b[(l + 2) * sb], s2);
+            s3 = fma(a[(l + 3) * sa], b[(l + 3) * sb], s3);
+        }
+        for (; l < n; ++l) s0 = fma(a[l * sa], b[l * sb], s0);
+        return (s0 + s1) + (s2 + s3);
+    }
+
+    // Dg weight of the condensed (slack, multiplier) pair (k, j)
     __device__ static __forceinline__ double Dg(const X& c, int k, int j) {
-        const double sig = c.ws[c.L.Sig + c.is(k) + j], dcg = c.ws[c.L.Dc + c.icg(k) + j];
+        const double sig = c.v(c.L->Sig)[c.is(k) + j], dcg = c.v(c.L->Dc)[c.icg(k) + j];
         return 1.0 / (1.0 / sig + dcg);
     }
 
     // add sum_j Dg_j G_j^T G_j of stage k (k>=1) to the position entries of the tile M (leading dim ld)
     __device__ static void add_cond(const X& c, int k, double* M, int ld) {
-        const Pb& pb = c.pb;
-        const double* gv = c.ws + c.L.gv + (k - 1) * pb.ng * PD;
+        const PbProxy pb;
+        const double* gv = c.v(c.L->gv) + (k - 1) * pb->ng * PD;
         constexpr int NPOS = NA * PD;
-        for (int e = c.lane; e < NPOS * NPOS; e += 32) {
+        for (int e = c.lane; e < NPOS * NPOS; e += NT) {
             const int r = e / NPOS, q = e % NPOS;
             const int a = r / PD, i = r % PD, b = q / PD, i2 = q % PD;
             double s = 0.0;
-            if (pb.family == JIPM_FAM_MULTIQUAD) {
-                for (int j = 0; j < pb.ng; ++j) {
+            if (pb->family == JIPM_FAM_MULTIQUAD) {
+                for (int j = 0; j < pb->ng; ++j) {
                     int pa, pb2; c.pair_ab(j, pa, pb2);
                     const double sa = (pa == a) ? 1.0 : (pb2 == a ? -1.0 : 0.0);
                     const double sb = (pa == b) ? 1.0 : (pb2 == b ? -1.0 : 0.0);
                     if (sa != 0.0 && sb != 0.0) s += sa * sb * Dg(c, k, j) * gv[j * PD + i] * gv[j * PD + i2];
                 }
             } else {
-                for (int j = 0; j < pb.ng; ++j) s += Dg(c, k, j) * gv[j * PD + i] * gv[j * PD + i2];
+                for (int j = 0; j < pb->ng; ++j) s += Dg(c, k, j) * gv[j * PD + i] * gv[j * PD + i2];
             }
             M[(AX * a + i) * ld + AX * b + i2] += s;
         }
-        __syncwarp();
+        c.tm.sync();
     }
 
     // T <- (I + P D)^{-1} P in place on the NX x NX tile sT (symmetric), D = Dc at rows [row0, row0+NX).
-    // Returns the number of non-positive pivots of I + E P E (0 when D == 0).  Uses sM as scratch.
-    __device__ static int transform_T(const X& c, double* sT, double* sM, int row0) {
-        const double* Dc = c.ws + c.L.Dc + row0;
-        double dmax = 0.0;
-        for (int i = c.lane; i < NX; i += 32) dmax = fmax(dmax, Dc[i]);
-        dmax = wmax(dmax);
-        if (dmax == 0.0) return 0;
-        // G = I + E P E -> sM (NX x NX), E = sqrt(D);   Y = E P -> rows scaled copy in sM second half is avoided:
-        // solve G Z = E P by LDL^T of G, then T = P - (P E) Z.
-        double* G = sM;              // NX*NX
-        double* Z = sM + NX * NX;    // NX*NX  (needs NZ*NZ >= 2 NX*NX; guaranteed by SM layout check at launch)
-        for (int e = c.lane; e < NX * NX; e += 32) {
+    // Returns the number of non-positive pivots of I + E P E (0 when D == 0).  Uses sM (>= 2 NX^2) as scratch.
+    __device__ static int transform_T(const X& c, double* sT, double* sM, int row0, bool any_dc) {
+        if (!any_dc) return 0;
+        const double* Dc = c.v(c.L->Dc) + row0;
+        // G = I + E P E (NX x NX), E = sqrt(D); solve G Z = E P by an unpivoted LDL^T of G, then T = P - (P E) Z
+        double* G = sM;
+        double* Z = sM + NX * NX;
+        for (int e = c.lane; e < NX * NX; e += NT) {
             const int r = e / NX, q = e % NX;
             const double er = sqrt(Dc[r]), eq = sqrt(Dc[q]);
             G[e] = er * sT[e] * eq + (r == q ? 1.0 : 0.0);
             Z[e] = er * sT[e];
         }
-        __syncwarp();
+        c.tm.sync();
         int bad = 0;
-        // unpivoted LDL^T of G applied to the right-hand sides Z (column q of Z handled by lane q)
+        // elimination: thread <-> element (r, q) of [G | Z], rows r > p
         for (int p = 0; p < NX; ++p) {
             double d = G[p * NX + p];
             if (!(d > 0.0)) { bad++; if (d == 0.0) d = 1.0; }
-            for (int q = c.lane; q < 2 * NX; q += 32) {
-                double* Mx = (q < NX) ? G : Z;
-                const int qq = (q < NX) ? q : q - NX;
-                if (q < NX && qq <= p) continue;
-                const double lpq = Mx[p * NX + qq] / d;
-                for (int r = p + 1; r < NX; ++r) Mx[r * NX + qq] -= G[r * NX + p] * lpq;
+            const double id = 1.0 / d;
+            for (int e = c.lane; e < (NX - 1 - p) * (2 * NX); e += NT) {
+                const int r = p + 1 + e / (2 * NX), q = e % (2 * NX);
+                if (q < NX) { if (q > p) G[r * NX + q] -= G[r * NX + p] * (G[p * NX + q] * id); }
+                else Z[r * NX + q - NX] -= G[r * NX + p] * (Z[p * NX + q - NX] * id);
             }
-            __syncwarp();
+            c.tm.sync();
         }
-        // now G holds (in its lower part, column p rows r>p) L*d ... Z holds L^{-1} E P; finish Z <- L^{-T} D^{-1} Z
+        // Z <- L^{-T} D^{-1} Z (rows from the bottom; thread <-> column q); L[r][p] = G[r][p] / d_p
         for (int p = NX - 1; p >= 0; --p) {
             double d = G[p * NX + p];
             if (d == 0.0) d = 1.0;
-            for (int q = c.lane; q < NX; q += 32) {
-                double v = Z[p * NX + q] / d;
-                for (int r = p + 1; r < NX; ++r) v -= (G[r * NX + p] / d) * Z[r * NX + q];
-                Z[p * NX + q] = v;
+            const double id = 1.0 / d;
+            for (int q = c.lane; q < NX; q += NT) {
+                double v = Z[p * NX + q];
+                for (int r = p + 1; r < NX; ++r) v -= G[r * NX + p] * Z[r * NX + q];
+                Z[p * NX + q] = v * id;
             }
-            __syncwarp();
+            c.tm.sync();
         }
-        // T = P - (P E) Z ; (P E)[i][l] = P[i][l] e_l
-        for (int q = c.lane; q < NX; q += 32) {
-            double acc[NX];
-#pragma unroll
-            for (int i = 0; i < NX; ++i) acc[i] = 0.0;
-            for (int l = 0; l < NX; ++l) {
-                const double zl = sqrt(Dc[l]) * Z[l * NX + q];
-#pragma unroll
-                for (int i = 0; i < NX; ++i) acc[i] += sT[l * NX + i] * zl;
-            }
-            // write into G region first to avoid overwriting P while other lanes read it
-#pragma unroll
-            for (int i = 0; i < NX; ++i) G[i * NX + q] = sT[i * NX + q] - acc[i];
+        // T = P - (P E) Z, (P E)[i][l] = P[i][l] e_l ; into G first (P is still being read), then symmetrised
+        for (int e = c.lane; e < NX * NX; e += NT) Z[e] *= sqrt(Dc[e / NX]);
+        c.tm.sync();
+        for (int e = c.lane; e < NX * NX; e += NT) {
+            const int i = e / NX, q = e % NX;
+            G[e] = sT[e] - dot4(sT + i, NX, Z + q, NX, NX);  // sum_l P[l][i] (e_l Z[l][q])   (P symmetric)
         }
-        __syncwarp();
-        for (int e = c.lane; e < NX * NX; e += 32) {
+        c.tm.sync();
+        for (int e = c.lane; e < NX * NX; e += NT) {
             const int r = e / NX, q = e % NX;
             sT[e] = 0.5 * (G[e] + G[q * NX + r]);
         }
-        __syncwarp();
+        c.tm.sync();
         return bad;
     }
 
-    // Factor.  Reads W, J, Sig, Dc, gv from the workspace; writes T, Xf, Lf.  Returns the number of pivots with
-    // the wrong sign (0 <=> inertia (n, m, 0)); nzero counts exactly-zero pivots.
-    __device__ static int factor(const X& c, int& nzero, bool useW = true) {
-        const Pb& pb = c.pb;
-        const int N = pb.N, lane = c.lane;
-        double* sT = c.sm + C::SM_T;
-        double* sJ = c.sm + C::SM_J;
-        double* sM = c.sm + C::SM_M;
-        const double* Sig = c.ws + c.L.Sig;
+    // Factor.  Reads W, J, Sig, Dc, gv from the workspace; writes T, Kf, Gf, Psi.  Returns the number of pivots with
+    // the wrong sign (0 <=> inertia (n, m, 0)); nzero counts exactly-zero pivots.  any_dc: some Dc entry is non-zero.
+    __device__ static __noinline__ int factor(const X& c, int& nzero, bool any_dc, bool useW) {
+        const PbProxy pb;
+        const int N = pb->N, lane = c.lane;
+        double* sT = c.sm + C::SM_T;     // NX x NX   current T_{k+1} / P_k
+        double* sJ = c.sm + C::SM_J;     // NX x NZ   J_k = [A B]
+        double* sM = c.sm + C::SM_M;     // NZ x NZ   stage tile (>= 2 NX^2: scratch of transform_T)
+        double* sTJ = c.sm + C::SM_TJ;   // NX x NZ   T J, later Phi (NX x NX)
+        double* sK = c.sm + C::SM_K;     // NU x NX   Kf ; then NU x NU Linv
+        double* sLi = sK + NU * NX;
+        const double* Sig = c.v(c.L->Sig);
+        const double* Dc = c.v(c.L->Dc);
         int bad = 0;
         nzero = 0;
         // terminal block
         {
             const double* WN = c.Wk(N);
-            for (int e = lane; e < NX * NX; e += 32) {
+            for (int e = lane; e < NX * NX; e += NT) {
                 const int r = e / NX, q = e % NX;
                 sT[e] = (useW ? WN[e] : 0.0) + (r == q ? Sig[c.ix(N) + r] : 0.0);
             }
-            __syncwarp();
-            if (pb.ng > 0) add_cond(c, N, sT, NX);
-            bad += transform_T(c, sT, sM, c.icd(N));
-            double* TN = c.ws + c.L.T + N * NX * NX;
-            for (int e = lane; e < NX * NX; e += 32) TN[e] = sT[e];
-            __syncwarp();
+            c.tm.sync();
+            if (pb->ng > 0) add_cond(c, N, sT, NX);
+            bad += transform_T(c, sT, sM, c.icd(N), any_dc);
+            double* TN = c.v(c.L->T) + N * NX * NX;
+            for (int e = lane; e < NX * NX; e += NT) TN[e] = sT[e];
+            c.tm.sync();
         }
         for (int k = N - 1; k >= 0; --k) {
             const double* Jg = c.Jk(k);
-            for (int e = lane; e < NX * NZ; e += 32) sJ[e] = Jg[e];
-            __syncwarp();
-            const double* Wg = c.Wk(k);
-            for (int j = lane; j < NZ; j += 32) {
-                double acc[NX];
-#pragma unroll
-                for (int i = 0; i < NX; ++i) acc[i] = 0.0;
-                for (int l = 0; l < NX; ++l) {
-                    const double jl = sJ[l * NZ + j];
-#pragma unroll
-                    for (int i = 0; i < NX; ++i) acc[i] += sT[l * NX + i] * jl;
-                }
-                double mcol[NZ];
-                const double sg = Sig[c.zidx(k, j)];
-#pragma unroll
-                for (int a = 0; a < NZ; ++a) mcol[a] = (useW ? Wg[a * NZ + j] : 0.0) + (a == j ? sg : 0.0);
-#pragma unroll
-                for (int l = 0; l < NX; ++l) {
-                    const double t = acc[l];
-#pragma unroll
-                    for (int a = 0; a < NZ; ++a) mcol[a] += sJ[l * NZ + a] * t;
-                }
-#pragma unroll
-                for (int a = 0; a < NZ; ++a) sM[a * NZ + j] = mcol[a];
+            for (int e = lane; e < NX * NZ; e += NT) sJ[e] = Jg[e];
+            c.tm.sync();
+            // TJ = T_{k+1} J_k
+            for (int e = lane; e < NX * NZ; e += NT) {
+                const int l = e / NZ, j = e % NZ;
+                sTJ[e] = dot4(sT + l * NX, 1, sJ + j, NZ, NX);
             }
-            __syncwarp();
-            if (k >= 1 && pb.ng > 0) add_cond(c, k, sM, NZ);
-            // eliminate the controls: pivots NX .. NZ-1
+            c.tm.sync();
+            // M = Q_k + J^T (T J)
+            const double* Wg = c.Wk(k);
+            for (int e = lane; e < NZ * NZ; e += NT) {
+                const int a = e / NZ, j = e % NZ;
+                double m = dot4(sJ + a, NZ, sTJ + j, NZ, NX);
+                if (useW) m += Wg[e];
+                if (a == j) m += Sig[c.zidx(k, j)];
+                sM[e] = m;
+            }
+            c.tm.sync();
+            if (k >= 1 && pb->ng > 0) add_cond(c, k, sM, NZ);
+            // eliminate the controls: pivots NX .. NZ-1 (element-parallel rank-1 updates)
             for (int p = 0; p < NU; ++p) {
                 const int pp = NX + p;
                 double d = sM[pp * NZ + pp];
                 if (!(d > 0.0)) { bad++; if (d == 0.0) { nzero++; d = 1.0; } }
-                for (int b = lane; b < NZ; b += 32) {
-                    if (b < NX || b > pp) {
-                        const double lb = sM[pp * NZ + b] / d;
-                        for (int a = 0; a < NX; ++a) sM[a * NZ + b] -= sM[a * NZ + pp] * lb;
-                        for (int a = pp + 1; a < NZ; ++a) sM[a * NZ + b] -= sM[a * NZ + pp] * lb;
-                    }
+                const double id = 1.0 / d;
+                for (int e = lane; e < NZ * NZ; e += NT) {
+                    const int a = e / NZ, b = e % NZ;
+                    if ((a < NX || a > pp) && (b < NX || b > pp)) sM[e] -= sM[a * NZ + pp] * (sM[pp * NZ + b] * id);
                 }
-                __syncwarp();
+                c.tm.sync();
             }
-            // store L (unit lower, D on the diagonal) and X = Mxu-columns scaled
-            double* Lg = c.ws + c.L.Lf + k * NU * NU;
-            double* Xg = c.ws + c.L.Xf + k * NX * NU;
-            for (int e = lane; e < NU * NU; e += 32) {
-                const int r = e / NU, p = e % NU;
-                double d = sM[(NX + p) * NZ + NX + p];
-                const double dd = (d == 0.0) ? 1.0 : d;
-                Lg[e] = (r == p) ? dd : (r > p ? sM[(NX + r) * NZ + NX + p] / dd : 0.0);
+            // Linv = L_uu^{-1} (unit lower; thread <-> column), pivots d_p on the diagonal of the tile
+            for (int q = lane; q < NU; q += NT) {
+                for (int r = 0; r < NU; ++r) {
+                    double v = (r == q) ? 1.0 : 0.0;
+                    if (r > q) {
+                        for (int t = q; t < r; ++t) {
+                            double dt = sM[(NX + t) * NZ + NX + t];
+                            if (dt == 0.0) dt = 1.0;
+                            v -= (sM[(NX + r) * NZ + NX + t] / dt) * sLi[t * NU + q];
+                        }
+                    }
+                    sLi[r * NU + q] = (r >= q) ? v : 0.0;
+                }
             }
-            for (int e = lane; e < NX * NU; e += 32) {
-                const int r = e / NU, p = e % NU;
-                double d = sM[(NX + p) * NZ + NX + p];
-                if (d == 0.0) d = 1.0;
-                Xg[e] = sM[r * NZ + NX + p] / d;
+            c.tm.sync();
+            // Kf = L^{-T} X^T, X[i][p] = M[i][NX+p]/d_p ;  Gf = L^{-T} D^{-1} L^{-1}
+            double* Kg = c.v(c.L->Kf) + k * NU * NX;
+            double* Gg = c.v(c.L->Gf) + k * NU * NU;
+            for (int e = lane; e < NU * NX + NU * NU; e += NT) {
+                if (e < NU * NX) {
+                    const int p = e / NX, i = e % NX;
+                    double s = 0.0;
+                    for (int q = p; q < NU; ++q) {
+                        double dq = sM[(NX + q) * NZ + NX + q];
+                        if (dq == 0.0) dq = 1.0;
+                        s += sLi[q * NU + p] * (sM[i * NZ + NX + q] / dq);
+                    }
+                    sK[e] = s; Kg[e] = s;
+                } else {
+                    const int e2 = e - NU * NX, p = e2 / NU, q = e2 % NU;
+                    double s = 0.0;
+                    for (int r = (p > q ? p : q); r < NU; ++r) {
+                        double dr = sM[(NX + r) * NZ + NX + r];
+                        if (dr == 0.0) dr = 1.0;
+                        s += sLi[r * NU + p] * sLi[r * NU + q] / dr;
+                    }
+                    Gg[e2] = s;
+                }
             }
-            for (int e = lane; e < NX * NX; e += 32) {
+            c.tm.sync();
+            // Phi = A - B Kf  (into sTJ, NX x NX)
+            for (int e = lane; e < NX * NX; e += NT) {
+                const int i = e / NX, a = e % NX;
+                sTJ[e] = sJ[i * NZ + a] - dot4(sJ + i * NZ + NX, 1, sK + a, NX, NU);
+            }
+            c.tm.sync();
+            // Psi = (I - D_{k+1} T_{k+1}) Phi
+            double* Pg = c.v(c.L->Psi) + k * NX * NX;
+            const int r0 = c.icd(k + 1);
+            for (int e = lane; e < NX * NX; e += NT) {
+                const int i = e / NX, a = e % NX;
+                double v = sTJ[e];
+                if (any_dc) v -= Dc[r0 + i] * dot4(sT + i * NX, 1, sTJ + a, NX, NX);
+                Pg[e] = v;
+            }
+            // P_k = symmetrised x-block of the tile (sT is still read by the Psi loop above: barrier first)
+            c.tm.sync();
+            for (int e = lane; e < NX * NX; e += NT) {
                 const int r = e / NX, q = e % NX;
                 sT[e] = 0.5 * (sM[r * NZ + q] + sM[q * NZ + r]);
             }
-            __syncwarp();
-            bad += transform_T(c, sT, sM, c.icd(k));
-            double* Tg = c.ws + c.L.T + k * NX * NX;
-            for (int e = lane; e < NX * NX; e += 32) Tg[e] = sT[e];
-            __syncwarp();
+            c.tm.sync();
+            bad += transform_T(c, sT, sM, c.icd(k), any_dc);
+            double* Tg = c.v(c.L->T) + k * NX * NX;
+            for (int e = lane; e < NX * NX; e += NT) Tg[e] = sT[e];
+            c.tm.sync();
         }
         return bad;
     }
@@ -218,154 +265,158 @@ struct Kkt {
     // condensed right-hand side contribution to x_k position entry (agent a, coordinate i), k >= 1:
     //   sum_j G_j^T Dg_j (rc_g,j + rp_s,j / sig_j)
     __device__ static double cond_rhs(const X& c, const double* rp, const double* rc, int k, int a, int i) {
-        const Pb& pb = c.pb;
-        const double* gv = c.ws + c.L.gv + (k - 1) * pb.ng * PD;
+        const PbProxy pb;
+        const double* gv = c.v(c.L->gv) + (k - 1) * pb->ng * PD;
         double s = 0.0;
-        for (int j = 0; j < pb.ng; ++j) {
+        for (int j = 0; j < pb->ng; ++j) {
             double sgn = 1.0;
-            if (pb.family == JIPM_FAM_MULTIQUAD) {
+            if (pb->family == JIPM_FAM_MULTIQUAD) {
                 int pa, pb2; c.pair_ab(j, pa, pb2);
                 sgn = (pa == a) ? 1.0 : (pb2 == a ? -1.0 : 0.0);
                 if (sgn == 0.0) continue;
             }
-            const double sig = c.ws[c.L.Sig + c.is(k) + j];
+            const double sig = c.v(c.L->Sig)[c.is(k) + j];
             s += sgn * gv[j * PD + i] * Dg(c, k, j) * (rc[c.icg(k) + j] + rp[c.is(k) + j] / sig);
         }
         return s;
     }
 
     // Solve with the current factor: [dx; dy] = K^{-1} [rp; rc].
-    __device__ static void solve(const X& c, const double* rp, const double* rc, double* dx, double* dy) {
-        const Pb& pb = c.pb;
-        const int N = pb.N, lane = c.lane;
-        double* sp = c.sm + C::SM_V;        // p vector  [NX]
-        double* sw = sp + NX;               // w         [NX]
-        double* sv = sw + NX;               // temp      [NX]
-        double* sx = sv + NX;               // x_k       [NX]
-        double* st = sx + NX;               // t / u     [NU]
-        const double* Dc = c.ws + c.L.Dc;
-        double* wv = c.ws + c.L.wv;
-        double* tv = c.ws + c.L.tv;
-        // ---- backward vector pass ----
-        for (int i = lane; i < NX; i += 32) {
-            double v = rp[c.ix(N) + i];
+    //   phase 0 (stage-parallel)  cr_k = rp_x,k + condensed rhs;  w_k = T_{k+1} rc_{k+1};
+    //                             h_k = rp_u,k - B_k^T w_k;  q_k = cr_k - A_k^T w_k - Kf_k^T h_k
+    //   phase 1 (sequential)      p_N = cr_N;  p_k = q_k + Psi_k^T p_{k+1}
+    //   phase 2 (stage-parallel)  sw_k = w_k - p_{k+1} + T_{k+1} (D_{k+1} p_{k+1});  uo_k = G_k (rp_u,k - B_k^T sw_k);
+    //                             e_k = (I - D T)(B_k uo_k) - D sw_k + rc_{k+1};  x_0 from the initial-condition rows
+    //   phase 3 (sequential)      x_{k+1} = Psi_k x_k + e_k
+    //   phase 4 (stage-parallel)  u_k = uo_k - Kf_k x_k;  nu_k = sw_k + T_{k+1} (A x_k + B u_k);  dy = -nu;  slacks
+    __device__ static __noinline__ void solve(const X& c, const double* rp, const double* rc, double* dx, double* dy,
+                                              bool any_dc) {
+        const PbProxy pb;
+        const int N = pb->N, lane = c.lane;
+        const double* Dc = c.v(c.L->Dc);
+        const double* Tf = c.v(c.L->T);
+        const double* Kf = c.v(c.L->Kf);
+        const double* Gf = c.v(c.L->Gf);
+        const double* Psi = c.v(c.L->Psi);
+        double* pv = c.v(c.L->pv);    // (N+1) x NX : cr_k, then p_k, then x_k
+        double* wv = c.v(c.L->wv);    // N x NX     : w_k, then sw_k
+        double* qv = c.v(c.L->qv);    // N x NX     : q_k, then e_k
+        double* hv = c.v(c.L->tv);    // N x NU     : h_k, then uo_k, then u_k
+        double* sv = c.v(c.L->sv);    // N x NX     : scratch (st_k, B uo_k, A x_k + B u_k)
+        // ---- phase 0a ----
+        for (int e = lane; e < (N + 1) * NX; e += NT) {
+            const int k = e / NX, i = e % NX;
+            double v = rp[c.ix(k) + i];
             const int ag = i / AX, ii = i % AX;
-            if (ii < PD && pb.ng > 0) v += cond_rhs(c, rp, rc, N, ag, ii);
-            sp[i] = v;
+            if (k >= 1 && ii < PD && pb->ng > 0) v += cond_rhs(c, rp, rc, k, ag, ii);
+            pv[e] = v;
         }
-        __syncwarp();
+        for (int e = lane; e < N * NX; e += NT) {
+            const int k = e / NX, i = e % NX;
+            wv[e] = dot4(Tf + (k + 1) * NX * NX + i, NX, rc + c.icd(k + 1), 1, NX);  // T symmetric
+        }
+        c.tm.sync();
+        // ---- phase 0b: h_k ----
+        for (int e = lane; e < N * NU; e += NT) {
+            const int k = e / NU, p = e % NU;
+            hv[e] = rp[c.iu(k) + p] - dot4(c.Jk(k) + NX + p, NZ, wv + k * NX, 1, NX);
+        }
+        c.tm.sync();
+        // ---- phase 0c: q_k ----
+        for (int e = lane; e < N * NX; e += NT) {
+            const int k = e / NX, i = e % NX;
+            qv[e] = pv[e] - dot4(c.Jk(k) + i, NZ, wv + k * NX, 1, NX) - dot4(Kf + k * NU * NX + i, NX, hv + k * NU, 1, NU);
+        }
+        c.tm.sync();
+        // ---- phase 1: backward sweep (threads i < NX; whole-team barrier only if NX spans several warps) ----
         for (int k = N - 1; k >= 0; --k) {
-            const double* Tn = c.ws + c.L.T + (k + 1) * NX * NX;
-            const double* Jg = c.Jk(k);
-            const double* Lg = c.ws + c.L.Lf + k * NU * NU;
-            const double* Xg = c.ws + c.L.Xf + k * NX * NU;
-            const int r0 = c.icd(k + 1);
-            for (int i = lane; i < NX; i += 32) sv[i] = rc[r0 + i] + Dc[r0 + i] * sp[i];
-            __syncwarp();
-            for (int i = lane; i < NX; i += 32) {
-                double s = -sp[i];
-#pragma unroll 4
-                for (int l = 0; l < NX; ++l) s += Tn[l * NX + i] * sv[l];
-                sw[i] = s; wv[k * NX + i] = s;
-            }
-            __syncwarp();
-            for (int p = lane; p < NU; p += 32) {
-                double s = rp[c.iu(k) + p];
-#pragma unroll 4
-                for (int l = 0; l < NX; ++l) s -= Jg[l * NZ + NX + p] * sw[l];
-                st[p] = s;
-            }
-            __syncwarp();
-            // t = L^{-1} rhat (column-oriented forward substitution)
-            for (int p = 0; p < NU - 1; ++p) {
-                const double tp = st[p];
-                __syncwarp();
-                for (int q = p + 1 + lane; q < NU; q += 32) st[q] -= Lg[q * NU + p] * tp;
-                __syncwarp();
-            }
-            for (int i = lane; i < NX; i += 32) {
-                double s = rp[c.ix(k) + i];
-                const int ag = i / AX, ii = i % AX;
-                if (k >= 1 && ii < PD && pb.ng > 0) s += cond_rhs(c, rp, rc, k, ag, ii);
-#pragma unroll 4
-                for (int l = 0; l < NX; ++l) s -= Jg[l * NZ + i] * sw[l];
-#pragma unroll 4
-                for (int p = 0; p < NU; ++p) s -= Xg[i * NU + p] * st[p];
-                sv[i] = s;
-            }
-            for (int p = lane; p < NU; p += 32) tv[k * NU + p] = st[p] / Lg[p * NU + p];
-            __syncwarp();
-            for (int i = lane; i < NX; i += 32) sp[i] = sv[i];
-            __syncwarp();
+            if (lane < NX) pv[k * NX + lane] = qv[k * NX + lane] + dot4(Psi + k * NX * NX + lane, NX, pv + (k + 1) * NX, 1, NX);
+            if (NX <= 32) __syncwarp(); else c.tm.sync();
         }
-        // ---- stage 0: nu_0 = T_0 (rc_0 + D_0 p_0) - p_0, x_0 = rc_0 - D_0 nu_0 ----
-        {
-            const double* T0 = c.ws + c.L.T;
-            for (int i = lane; i < NX; i += 32) sv[i] = rc[i] + Dc[i] * sp[i];
-            __syncwarp();
-            for (int i = lane; i < NX; i += 32) {
-                double s = -sp[i];
-#pragma unroll 4
-                for (int l = 0; l < NX; ++l) s += T0[l * NX + i] * sv[l];
-                const double x0 = rc[i] - Dc[i] * s;
-                sx[i] = x0; dx[i] = x0; dy[i] = -s;
-            }
-            __syncwarp();
-        }
-        // ---- forward pass ----
-        for (int k = 0; k < N; ++k) {
-            const double* Tn = c.ws + c.L.T + (k + 1) * NX * NX;
-            const double* Jg = c.Jk(k);
-            const double* Lg = c.ws + c.L.Lf + k * NU * NU;
-            const double* Xg = c.ws + c.L.Xf + k * NX * NU;
-            for (int p = lane; p < NU; p += 32) {
-                double s = tv[k * NU + p];
-#pragma unroll 4
-                for (int i = 0; i < NX; ++i) s -= Xg[i * NU + p] * sx[i];
-                st[p] = s;
-            }
-            __syncwarp();
-            // u = L^{-T} q (backward substitution)
-            for (int p = NU - 1; p > 0; --p) {
-                const double up = st[p];
-                __syncwarp();
-                for (int q = lane; q < p; q += 32) st[q] -= Lg[p * NU + q] * up;
-                __syncwarp();
-            }
-            for (int p = lane; p < NU; p += 32) dx[c.iu(k) + p] = st[p];
-            for (int i = lane; i < NX; i += 32) {
-                const double* Jr = Jg + i * NZ;
+        c.tm.sync();
+        // ---- phase 2 ----
+        if (any_dc) {
+            for (int e = lane; e < N * NX; e += NT) {
+                const int k = e / NX, i = e % NX, r0 = c.icd(k + 1);
                 double s = 0.0;
-#pragma unroll 4
-                for (int a = 0; a < NX; ++a) s += Jr[a] * sx[a];
-#pragma unroll 4
-                for (int a = 0; a < NU; ++a) s += Jr[NX + a] * st[a];
-                sv[i] = s;
+                const double* Tn = Tf + (k + 1) * NX * NX;
+                for (int l = 0; l < NX; ++l) s += Tn[l * NX + i] * (Dc[r0 + l] * pv[(k + 1) * NX + l]);
+                wv[e] += s - pv[(k + 1) * NX + i];
             }
-            __syncwarp();
-            const int r0 = c.icd(k + 1);
-            for (int i = lane; i < NX; i += 32) {
-                double nu = wv[k * NX + i];
-#pragma unroll 4
-                for (int l = 0; l < NX; ++l) nu += Tn[l * NX + i] * sv[l];
-                const double xn = sv[i] - Dc[r0 + i] * nu + rc[r0 + i];
-                dx[c.ix(k + 1) + i] = xn; dy[r0 + i] = -nu; sp[i] = xn;
+        } else {
+            for (int e = lane; e < N * NX; e += NT) wv[e] -= pv[e + NX];
+        }
+        c.tm.sync();
+        for (int e = lane; e < N * NU; e += NT) {
+            const int k = e / NU, p = e % NU;
+            sv[e] = rp[c.iu(k) + p] - dot4(c.Jk(k) + NX + p, NZ, wv + k * NX, 1, NX);  // st_k (N x NU fits in sv)
+        }
+        c.tm.sync();
+        for (int e = lane; e < N * NU; e += NT) {
+            const int k = e / NU, p = e % NU;
+            hv[e] = dot4(Gf + k * NU * NU + p * NU, 1, sv + k * NU, 1, NU);  // uo_k = G st_k
+        }
+        c.tm.sync();
+        for (int e = lane; e < N * NX; e += NT) {
+            const int k = e / NX, i = e % NX;
+            sv[e] = dot4(c.Jk(k) + i * NZ + NX, 1, hv + k * NU, 1, NU);  // B uo_k   (st_k is dead)
+        }
+        c.tm.sync();
+        for (int e = lane; e < N * NX; e += NT) {
+            const int k = e / NX, i = e % NX, r0 = c.icd(k + 1);
+            double v = sv[e] + rc[r0 + i];
+            if (any_dc) v -= Dc[r0 + i] * (dot4(Tf + (k + 1) * NX * NX + i, NX, sv + k * NX, 1, NX) + wv[e]);
+            qv[e] = v;  // e_k
+        }
+        // stage 0: nu_0 = T_0 (rc_0 + D_0 p_0) - p_0, x_0 = rc_0 - D_0 nu_0
+        double x0 = 0.0;
+        if (lane < NX) {
+            double s = -pv[lane];
+            for (int l = 0; l < NX; ++l) s += Tf[l * NX + lane] * (rc[l] + Dc[l] * pv[l]);
+            x0 = rc[lane] - Dc[lane] * s;
+            dx[lane] = x0; dy[lane] = -s;
+        }
+        c.tm.sync();
+        // ---- phase 3: forward sweep, x_k kept in pv (p_k is dead once sw_k, x_0 are formed) ----
+        if (lane < NX) pv[lane] = x0;
+        if (NX <= 32) __syncwarp(); else c.tm.sync();
+        for (int k = 0; k < N; ++k) {
+            if (lane < NX) {
+                const double xn = qv[k * NX + lane] + dot4(Psi + k * NX * NX + lane * NX, 1, pv + k * NX, 1, NX);
+                pv[(k + 1) * NX + lane] = xn;
             }
-            __syncwarp();
-            for (int i = lane; i < NX; i += 32) sx[i] = sp[i];
-            __syncwarp();
+            if (NX <= 32) __syncwarp(); else c.tm.sync();
+        }
+        c.tm.sync();
+        // ---- phase 4 ----
+        for (int e = lane; e < N * NX; e += NT) dx[c.ix(e / NX + 1) + e % NX] = pv[e + NX];
+        for (int e = lane; e < N * NU; e += NT) {
+            const int k = e / NU, p = e % NU;
+            const double u = hv[e] - dot4(Kf + k * NU * NX + p * NX, 1, pv + k * NX, 1, NX);
+            hv[e] = u; dx[c.iu(k) + p] = u;
+        }
+        c.tm.sync();
+        for (int e = lane; e < N * NX; e += NT) {
+            const int k = e / NX, i = e % NX;
+            sv[e] = dot4(c.Jk(k) + i * NZ, 1, pv + k * NX, 1, NX) + dot4(c.Jk(k) + i * NZ + NX, 1, hv + k * NU, 1, NU);
+        }
+        c.tm.sync();
+        for (int e = lane; e < N * NX; e += NT) {
+            const int k = e / NX, i = e % NX;
+            const double nu = wv[e] + dot4(Tf + (k + 1) * NX * NX + i, NX, sv + k * NX, 1, NX);
+            dy[c.icd(k + 1) + i] = -nu;
         }
         // ---- slack / inequality-multiplier recovery ----
-        const double* gv = c.ws + c.L.gv;
-        for (int it = lane; it < N * pb.ng; it += 32) {
-            const int k = it / pb.ng + 1, j = it % pb.ng;
-            const double sig = c.ws[c.L.Sig + c.is(k) + j];
+        const double* gv = c.v(c.L->gv);
+        for (int it = lane; it < N * pb->ng; it += NT) {
+            const int k = it / pb->ng + 1, j = it % pb->ng;
+            const double sig = c.v(c.L->Sig)[c.is(k) + j];
             const double rps = rp[c.is(k) + j];
             const double dyg = Dg(c, k, j) * (c.G_dot(gv, dx, k, j) - rc[c.icg(k) + j] - rps / sig);
             dy[c.icg(k) + j] = dyg;
             dx[c.is(k) + j] = (rps + dyg) / sig;
         }
-        __syncwarp();
+        c.tm.sync();
     }
 };
 

@@ -1,20 +1,24 @@
 // launch.cuh -- host-visible launchers of the slot kernel, one translation unit per family configuration
-// (inst_*.cu) so that the four template instantiations compile in parallel.
+// (inst_*.cu) so that the template instantiations compile in parallel.
 #pragma once
 #include "common.cuh"
 
 namespace jipm {
 
-struct LaunchInfo { int sm_doubles_per_warp; };
+// what the host needs to know about one instantiation
+struct InstInfo {
+    int nt;            // threads per problem slot (= CTA size: one team per CTA)
+    int sm_fixed;      // fixed shared memory per team, doubles (tiles, staging, reduction scratch)
+    int min_blocks;    // __launch_bounds__ min CTAs per SM the kernel was compiled for
+};
 
-cudaError_t launch_pm(const Args& a, int warps_per_block, cudaStream_t st);
-cudaError_t launch_q1(const Args& a, int warps_per_block, cudaStream_t st);
-cudaError_t launch_q2(const Args& a, int warps_per_block, cudaStream_t st);
-cudaError_t launch_q4(const Args& a, int warps_per_block, cudaStream_t st);
-int sm_doubles_pm();
-int sm_doubles_q1();
-int sm_doubles_q2();
-int sm_doubles_q4();
+typedef cudaError_t (*launch_fn)(const Args& a, cudaStream_t st);
+struct Inst { InstInfo info; launch_fn launch; };
+
+Inst inst_pm();
+Inst inst_q1();
+Inst inst_q2();
+Inst inst_q4();
 cudaError_t launch_fp64_peak(double* out, int blocks, int threads, int iters, cudaStream_t st);
 
 }  // namespace jipm
