@@ -263,6 +263,10 @@ def run_jipm(args):
         secs = dev_ms * 1e-3
         value = solved_all * K / secs
         flops = flops_from_stats(d, stats_sum)  # rank 0's launches
+        cyc_it = max(stats_sum.get("cyc_iterations", 0), 1)
+        phase_share = {k[4:]: round(stats_sum[k] / cyc_it, 4) for k in
+                       ("cyc_derivs", "cyc_factor", "cyc_solve", "cyc_residual", "cyc_trial_eval")}
+        us_per_iter = cyc_it / max(stats_sum["iterations"], 1) / (clocks["sm_mhz"] or 1965.0) if clocks else None
         my_secs = sum(a.elapsed_time(b) for a, b in ev) * 1e-3
         achieved = flops / my_secs / 1e12
         hist = {int(k): int((status == k).sum()) for k in np.unique(status)}
@@ -291,7 +295,9 @@ def run_jipm(args):
                                         "(MEASURED_PEAKS.json has no FP64 entry); nominal 148 SM x 64 DFMA/clk x 2 x "
                                         "1.965 GHz = 37.2",
                          "algorithmic_flops_per_step": flops / K,
-                         "counts_per_step": {k: v / K for k, v in stats_sum.items()}},
+                         "counts_per_step": {k: v / K for k, v in stats_sum.items() if not k.startswith("cyc_")},
+                         "phase_share_of_iteration_cycles": phase_share,
+                         "slot_us_per_iteration": us_per_iter},
             "clocks": clocks,
         }
         if not args.no_cpu_baseline and world == 1:

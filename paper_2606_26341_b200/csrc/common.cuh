@@ -30,9 +30,10 @@ struct Pb {
 
 // offsets (in doubles) into the per-warp workspace
 struct Lay {
-    int x, y, zL, zU, g, c, gv, tgt, J, W, Sig, Hd, Dc, T, Kf, Gf, Psi, pv, qv, sv, wv, tv;
+    int x, y, zL, zU, g, c, gv, dgv, tgt, J, W, Sig, Hd, Dc, T, Kf, Gf, Psi, pv, qv, sv, wv, tv, bl, bu;
     int b1, b2, b3, b4, dx, dy, dzL, dzU, r1, r2, r3, r4, e1, e2, e3, e4;
     int sx, sy, szL, szU, xt, ct, csoc, bs2, rr, rk, filt, total;
+    int pv0, npad, tail0, tpad;  // primal-sized vectors: contiguous block of npad-strided heads, 2m-tails (restoration) apart
     int nsm;  // the first nsm doubles of the layout are shared-memory resident (per team), the rest global
     int xR, DR2, filtR, rc2;  // restoration mode: reference point, scaling D_R^2, its own filter, condensed rhs
 };
@@ -51,7 +52,7 @@ struct Args {
     double* x_out; double* lam_out; double* zL_out; double* zU_out;
     int32_t* status_out; int32_t* iters_out;
     int* queue;          // [1] next problem id
-    unsigned long long* stats; // [8]
+    unsigned long long* stats; // [16]
     double* trace; int trace_cap;
     // debug
     int dbg_mode;        // 0 solve, 1 init only, 2 load state + step
@@ -80,10 +81,19 @@ __host__ __device__ inline DbgLay make_dbglay(int n, int m, int N, int NX, int N
 // launcher on the solver's stream): every pb->, L->, o->, A-> below compiles to a c[3][offset] operand instead of a
 // load through a pointer to the kernel parameters.
 static __constant__ Args g_A;
+extern __shared__ double jipm_smem[];  // the CTA's dynamic shared memory: fixed tiles, then the hot part of the layout
 struct PbProxy { __device__ __forceinline__ const Pb* operator->() const { return &g_A.pb; } };
 struct LayProxy { __device__ __forceinline__ const Lay* operator->() const { return &g_A.L; } };
 struct OptProxy { __device__ __forceinline__ const jipm_options* operator->() const { return &g_A.o; } };
 struct ArgsProxy { __device__ __forceinline__ const Args* operator->() const { return &g_A; } };
+
+// A primal-sized vector: entries [0, n) at a (shared memory or scratch), the restoration tail [n, n + 2m) -- the
+// p and n variables of Step R -- in the global scratch at t (pre-shifted by -n so that t[i] is entry i).
+struct Vec {
+    double* a; double* t; int n;
+    __device__ __forceinline__ double& operator[](int i) const { return i < n ? a[i] : t[i]; }
+    __device__ __forceinline__ operator double*() const { return a; }  // the head: what the base problem's code sees
+};
 
 // A TEAM of NT threads (NT = 32, 64, 128 or 256; whole warps) owns one problem slot.  All decisions of the
 // interior-point iteration are team-uniform predicates: every thread of the team holds the same scalar state,

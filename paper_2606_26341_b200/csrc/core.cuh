@@ -6,17 +6,20 @@
 
 namespace jipm {
 
-template <class Dyn_, int NA_, int NT_>
+template <class Dyn_, int NA_, int NT_, bool HOT_SM_>
 struct Cfg {
     using Dyn = Dyn_;
     static constexpr int NA = NA_;
     static constexpr int NT = NT_;  // threads per problem slot (team size)
+    // the host guarantees that the "hot" group of the layout (factor blocks, sweep vectors, J, W, m-vectors) is
+    // shared-memory resident: its accessor then yields pointers the compiler knows to be shared (LDS, not generic LD)
+    static constexpr bool HOT_SM = HOT_SM_;
     static constexpr int AX = Dyn::AX, AU = Dyn::AU, PD = Dyn::PD;
     static constexpr int NX = AX * NA, NU = AU * NA, NZ = NX + NU;
     // fixed shared memory per team (doubles): T, J, M, TJ/Phi, Kf/Linv tiles of the stage sweep, the staging of the
     // quadrotor Hessian columns (7 x 16 per 16-thread group), the reduction scratch
     static constexpr int SM_MSZ = (NZ * NZ > 2 * NX * NX) ? NZ * NZ : 2 * NX * NX;
-    static constexpr int SM_T = 0, SM_J = SM_T + NX * NX, SM_M = SM_J + NX * NZ, SM_TJ = SM_M + SM_MSZ;
+    static constexpr int SM_T = 0, SM_J = SM_T + NX * NX, SM_M = SM_J + NX * NZ, SM_M2 = SM_M + SM_MSZ, SM_TJ = SM_M2 + SM_MSZ;
     static constexpr int SM_K = SM_TJ + NX * NZ, SM_G = SM_K + NU * NX + NU * NU;
     static constexpr int SM_RED = SM_G + (Dyn::AX == 12 ? (NT / 16) * 7 * 16 : 0);
     static constexpr int SM_TOTAL = SM_RED + 2 * (NT / 32) + 2;
@@ -48,11 +51,19 @@ struct Ctx {
     __device__ __forceinline__ int icd(int k) const { return k == 0 ? 0 : NX + (k - 1) * pb->cblk; }
     __device__ __forceinline__ int icg(int k) const { return NX + (k - 1) * pb->cblk + NX; }
     __device__ __forceinline__ int zidx(int k, int a) const { return a < NX ? ix(k) + a : iu(k) + a - NX; }
-    __device__ __forceinline__ double* Jk(int k) const { return v(L->J) + k * (NX * NZ); }
-    __device__ __forceinline__ double* Wk(int k) const { return v(L->W) + k * (NZ * NZ); }  // k == N: NX x NX
+    __device__ __forceinline__ double* Jk(int k) const { return vh(L->J) + k * (NX * NZ); }
+    __device__ __forceinline__ double* Wk(int k) const { return vh(L->W) + k * (NZ * NZ); }  // k == N: NX x NX
     // workspace array at layout offset off: the first L->nsm doubles of the layout live in shared memory (the
     // hot vectors and factor blocks), the rest in this slot's global workspace (L2-resident scratch)
     __device__ __forceinline__ double* v(int off) const { return off < L->nsm ? smd + off : ws + off; }
+    // same for an array of the hot group: addressed off the CTA's shared array itself (one team per CTA), so that
+    // the compiler emits shared loads/stores (LDS/STS) instead of generic ones
+    __device__ __forceinline__ double* vh(int off) const {
+        if constexpr (C::HOT_SM) return jipm_smem + C::SM_TOTAL + off;
+        else return v(off);
+    }
+    // fixed tile at offset off of this team's shared memory
+    __device__ __forceinline__ double* smt(int off) const { return jipm_smem + off; }
 
     // pair q -> agents (a,b), a<b, row-major enumeration
     __device__ __forceinline__ void pair_ab(int q, int& a, int& b) const {
@@ -114,7 +125,7 @@ struct Ctx {
     __device__ double eval_fc(const double* x, double* c, double& theta, double& cmax, bool& fin) const {
         const int N = pb->N;
         double f = 0.0;
-        const double* tgt = v(L->tgt);
+        const double* tgt = vh(L->tgt);
         for (int it = lane; it < (N + 1) * NA; it += NT) {
             const int k = it / NA, a = it % NA;
             const double* p = x + ix(k) + AX * a;
@@ -161,7 +172,7 @@ struct Ctx {
 
     // ---- A d (m-vector) and A^T y (n-vector) with the stage blocks J_k and the inequality gradients -----
     __device__ void A_mul(const double* d, double* out) const {
-        const double* gv = v(L->gv);
+        const double* gv = vh(L->gv);
         for (int r = lane; r < pb->m; r += NT) {
             double s;
             if (r < NX) s = d[r];
@@ -185,7 +196,7 @@ struct Ctx {
         tm.sync();
     }
     __device__ double AT_entry(const double* y, int idx) const {
-        const double* gv = v(L->gv);
+        const double* gv = vh(L->gv);
         int k, a;  // x_k[a] or u_k[a-NX]
         if (idx < NX) { k = 0; a = idx; }
         else {

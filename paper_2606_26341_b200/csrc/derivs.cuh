@@ -22,13 +22,13 @@ __device__ void Ctx<C>::dyn_derivs(const double* x, const double* y) {
             else if (r >= 2 && cidx == r + 2) v = h;
             Jk(k)[e] = v;
         }
-        for (int it = lane; it < N * NZ * NZ + NX * NX; it += NT) v(L->W)[it] = 0.0;
+        for (int it = lane; it < N * NZ * NZ + NX * NX; it += NT) vh(L->W)[it] = 0.0;
         tm.sync();
     } else {
         const double h = pb->dt;
         double* rk = v(L->rk);
         if (NA > 1) {
-            for (int it = lane; it < N * NZ * NZ; it += NT) v(L->W)[it] = 0.0;
+            for (int it = lane; it < N * NZ * NZ; it += NT) vh(L->W)[it] = 0.0;
         }
         // ---- phase 1: lane <-> (stage, agent): RK points, Df entries, adjoints, contracted 7x7 Hessians ----
         for (int it = lane; it < N * NA; it += NT) {
@@ -77,7 +77,7 @@ __device__ void Ctx<C>::dyn_derivs(const double* x, const double* y) {
         // (two groups share a warp and run the same instruction stream: __syncwarp orders the staging)
         const int grp = lane >> 4, j = lane & 15;
         constexpr int NGRP = NT / 16;
-        double* sV = sm + C::SM_G + grp * (7 * 16);
+        double* sV = smt(C::SM_G) + grp * (7 * 16);
         const int nit = N * NA;
         for (int it0 = 0; it0 < nit; it0 += NGRP) {
             const int it = it0 + grp;
@@ -145,7 +145,7 @@ template <class C>
 __device__ void Ctx<C>::eval_derivs(const double* x, const double* y, double sigma_f) {
     const int N = pb->N;
     double* g = v(L->g);
-    const double* tgt = v(L->tgt);
+    const double* tgt = vh(L->tgt);
     for (int i = lane; i < pb->n; i += NT) g[i] = 0.0;
     tm.sync();
     for (int it = lane; it < (N + 1) * NA * PD; it += NT) {
@@ -157,7 +157,7 @@ __device__ void Ctx<C>::eval_derivs(const double* x, const double* y, double sig
         g[idx] = sigma_f * 2.0 * pb->ru * x[idx];
     }
     // inequality gradient vectors
-    double* gv = v(L->gv);
+    double* gv = vh(L->gv);
     for (int it = lane; it < N * pb->ng; it += NT) {
         const int k = it / pb->ng + 1, j = it % pb->ng;
         if (pb->family == JIPM_FAM_MULTIQUAD) {

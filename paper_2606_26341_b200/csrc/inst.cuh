@@ -19,7 +19,7 @@ static cudaError_t launch_cfg(const Args& a, cudaStream_t st) {
 template <class C, int MINB>
 static Inst make_inst() {
     Inst i;
-    i.info.nt = C::NT; i.info.sm_fixed = C::SM_TOTAL; i.info.min_blocks = MINB;
+    i.info.nt = C::NT; i.info.sm_fixed = C::SM_TOTAL; i.info.min_blocks = MINB; i.info.hot_sm = C::HOT_SM ? 1 : 0;
     i.launch = &launch_cfg<C, MINB>;
     return i;
 }

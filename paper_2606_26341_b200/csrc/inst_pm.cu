@@ -1,7 +1,8 @@
-// inst_pm.cu -- slot kernel instantiation: PointmassDyn, 1 agent(s), 32 threads per problem slot, >= 16 CTA(s) per SM.
+// inst_pm.cu -- slot kernel instantiation: PointmassDyn, 1 agent(s), 32 threads per problem slot, >= 8 CTA(s) per SM,
+// hot layout group guaranteed shared-memory resident.
 #include "inst.cuh"
 namespace jipm {
-Inst inst_pm() { return make_inst<Cfg<PointmassDyn, 1, 32>, 16>(); }
+Inst inst_pm() { return make_inst<Cfg<PointmassDyn, 1, 32, true>, 8>(); }
 }  // namespace jipm
 
 namespace jipm {

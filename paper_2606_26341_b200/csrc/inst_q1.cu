@@ -1,5 +1,6 @@
-// inst_q1.cu -- slot kernel instantiation: QuadDyn, 1 agent(s), 128 threads per problem slot, >= 3 CTA(s) per SM.
+// inst_q1.cu -- slot kernel instantiation: QuadDyn, 1 agent(s), 256 threads per problem slot, >= 1 CTA(s) per SM,
+// hot layout group guaranteed shared-memory resident.
 #include "inst.cuh"
 namespace jipm {
-Inst inst_q1() { return make_inst<Cfg<QuadDyn, 1, 128>, 3>(); }
+Inst inst_q1() { return make_inst<Cfg<QuadDyn, 1, 256, true>, 1>(); }
 }  // namespace jipm

@@ -31,21 +31,37 @@ struct Solver {
     double theta_entry, zeta, f_pn, f_q, f_base, theta_base, cmax_base, dc_cur;
     long long pid;
     unsigned n_fact, n_solve, n_deriv, n_fc, n_iter, n_resto;
+    // SM-clock cycles this team spent in: 0 derivatives, 1 factorisations, 2 KKT solves, 3 residuals of (6),
+    // 4 trial-point evaluations, 5 whole iterations, 6 Step I, 7 (spare)
+    unsigned long long tph[8];
+    double* bl; double* bu;
 
     __device__ Solver(X& c_) : c(c_), lane(c_.lane) {
         n_fact = n_solve = n_deriv = n_fc = n_iter = n_resto = 0;
+        for (int q = 0; q < 8; ++q) tph[q] = 0;
+        // the shared bounds, copied next to the iterate once per kernel
+        bl = c.vh(L->bl); bu = c.vh(L->bu);
+        for (int q = lane; q < pb->n; q += NT) { bl[q] = pb->xL[q]; bu[q] = pb->xU[q]; }
+        c.tm.sync();
         mode = 0; nX = pb->n;
     }
     __device__ __forceinline__ double* V(int off) const { return c.v(off); }
+    __device__ __forceinline__ double* VH(int off) const { return c.vh(off); }
+    __device__ __forceinline__ Vec VX(int off) const {
+        Vec r;
+        r.a = c.v(off); r.n = pb->n;
+        r.t = c.v(L->tail0 + ((off - L->pv0) / L->npad) * L->tpad) - pb->n;
+        return r;
+    }
     // bounds of the extended primal vector: entries >= n are the restoration variables p, n >= 0
-    __device__ __forceinline__ double lo(int i) const { return i < pb->n ? pb->xL[i] : 0.0; }
-    __device__ __forceinline__ double hi(int i) const { return i < pb->n ? pb->xU[i] : INFINITY; }
+    __device__ __forceinline__ double lo(int i) const { return i < pb->n ? bl[i] : 0.0; }
+    __device__ __forceinline__ double hi(int i) const { return i < pb->n ? bu[i] : INFINITY; }
     __device__ __forceinline__ bool hasL(int i) const { return lo(i) > -INFINITY; }
     __device__ __forceinline__ bool hasU(int i) const { return hi(i) < INFINITY; }
     __device__ __forceinline__ double* filt_active() const { return V(mode ? L->filtR : L->filt); }
 
     // barrier objective (3) with the one-sided damping term; NaN outside the interior
-    __device__ double phi(const double* x, double fv, double mu_, int nvar) const {
+    __device__ double phi(const Vec x, double fv, double mu_, int nvar) const {
         double s = 0.0;
         int badpt = 0;
         for (int i = lane; i < nvar; i += NT) {
@@ -70,7 +86,7 @@ struct Solver {
     }
 
     // fraction to the boundary (PAPER.md:148 fn 2) on the primal step
-    __device__ double ftb_primal(const double* x, const double* dx, double tau_) const {
+    __device__ double ftb_primal(const Vec x, const Vec dx, double tau_) const {
         double a = 1.0;
         for (int i = lane; i < nX; i += NT) {
             const double l = lo(i), u = hi(i), d = dx[i];
@@ -79,7 +95,7 @@ struct Solver {
         }
         return c.tm.min(a);
     }
-    __device__ double ftb_dual(const double* zL, const double* zU, const double* dzL, const double* dzU,
+    __device__ double ftb_dual(const Vec zL, const Vec zU, const Vec dzL, const Vec dzU,
                                double tau_) const {
         double a = 1.0;
         for (int i = lane; i < nX; i += NT) {
@@ -91,7 +107,7 @@ struct Solver {
 
     // optimality error E_mu from the dual residual base in b1 (= grad f + A^T y - zL + zU)
     __device__ double opt_error(double mu_, double sd, double sc) const {
-        const double* x = V(L->x); const double* zL = V(L->zL); const double* zU = V(L->zU); const double* rdb = V(L->b1);
+        Vec x = VX(L->x); Vec zL = VX(L->zL); Vec zU = VX(L->zU); Vec rdb = VX(L->b1);
         double ed = 0.0, es = 0.0;
         for (int i = lane; i < nX; i += NT) {
             const double l = lo(i), u = hi(i);
@@ -152,8 +168,8 @@ struct Solver {
     // restoration mode the Schur complement 1/Sig_p + 1/Sig_n of the eliminated (p, n) pairs ([7] sec 3.3)
     __device__ void set_sigma(double dw, double dc) {
         dc_cur = dc;
-        const double* x = V(L->x); const double* zL = V(L->zL); const double* zU = V(L->zU);
-        double* Sig = V(L->Sig); double* Hd = V(L->Hd); double* Dc = V(L->Dc);
+        Vec x = VX(L->x); Vec zL = VX(L->zL); Vec zU = VX(L->zU);
+        Vec Sig = VX(L->Sig); Vec Hd = VX(L->Hd); double* Dc = VH(L->Dc);
         const double* DR2 = V(L->DR2);
         for (int i = lane; i < nX; i += NT) {
             const double l = lo(i), u = hi(i);
@@ -174,13 +190,13 @@ struct Solver {
         if (i < pb->n) return c.AT_entry(y, i);
         return (i < pb->n + pb->m) ? -y[i - pb->n] : y[i - pb->n - pb->m];
     }
-    __device__ __forceinline__ double Wx(const double* d, int i) const { return i < pb->n ? c.W_entry(d, i) : 0.0; }
+    __device__ __forceinline__ double Wx(const Vec d, int i) const { return i < pb->n ? c.W_entry(d.a, i) : 0.0; }
 
     // solve (6) through (7) + the Delta z recovery of PAPER.md:110 for rhs (b1,b2,b3,b4) -> (d1..d4)
-    __device__ void reduced_solve(const double* b1, const double* b2, const double* b3, const double* b4,
-                                  double* d1, double* d2, double* d3, double* d4) {
-        const double* x = V(L->x); const double* zL = V(L->zL); const double* zU = V(L->zU);
-        double* rr = V(L->rr);
+    __device__ void reduced_solve(const Vec b1, const double* b2, const Vec b3, const Vec b4,
+                                  Vec d1, double* d2, Vec d3, Vec d4) {
+        Vec x = VX(L->x); Vec zL = VX(L->zL); Vec zU = VX(L->zU);
+        Vec rr = VX(L->rr);
         for (int i = lane; i < nX; i += NT) {
             const double l = lo(i), u = hi(i);
             double r = b1[i];
@@ -190,7 +206,7 @@ struct Solver {
         }
         c.tm.sync();
         const double* rc = b2;
-        const double* Sig = V(L->Sig);
+        Vec Sig = VX(L->Sig);
         const int n = pb->n, m = pb->m;
         if (mode) {  // eliminate (dp, dn): dp = (r_p + dy)/Sig_p, dn = (r_n - dy)/Sig_n
             double* rc2 = V(L->rc2);
@@ -198,7 +214,9 @@ struct Solver {
             c.tm.sync();
             rc = rc2;
         }
-        K::solve(c, rr, rc, d1, d2, mode != 0 || dc_cur != 0.0);
+        const long long t0 = clock64();
+        K::solve(c, rr.a, rc, d1.a, d2, mode != 0 || dc_cur != 0.0);
+        tph[2] += clock64() - t0;
         n_solve++;
         if (mode) {
             for (int j = lane; j < m; j += NT) {
@@ -216,12 +234,12 @@ struct Solver {
     }
 
     // residual of the unreduced system (6): r = b - M d; returns ||r||_inf; dnorm = ||d||_inf
-    __device__ double full_residual(const double* b1, const double* b2, const double* b3, const double* b4,
-                                    const double* d1, const double* d2, const double* d3, const double* d4,
+    __device__ double full_residual(const Vec b1, const double* b2, const Vec b3, const Vec b4,
+                                    const Vec d1, const double* d2, const Vec d3, const Vec d4,
                                     double& dnorm) const {
-        const double* x = V(L->x); const double* zL = V(L->zL); const double* zU = V(L->zU);
-        const double* Hd = V(L->Hd);
-        double* r1 = V(L->r1); double* r2 = V(L->r2); double* r3 = V(L->r3); double* r4 = V(L->r4);
+        Vec x = VX(L->x); Vec zL = VX(L->zL); Vec zU = VX(L->zU);
+        Vec Hd = VX(L->Hd);
+        Vec r1 = VX(L->r1); double* r2 = VH(L->r2); Vec r3 = VX(L->r3); Vec r4 = VX(L->r4);
         double rn = 0.0, dn = 0.0;
         for (int i = lane; i < nX; i += NT) {
             const double l = lo(i), u = hi(i);
@@ -235,7 +253,7 @@ struct Solver {
             rn = fmax(rn, fmax(fabs(v3), fabs(v4)));
             dn = fmax(dn, fmax(fabs(d1[i]), fmax(fabs(d3[i]), fabs(d4[i]))));
         }
-        c.A_mul(d1, r2);
+        c.A_mul(d1.a, r2);
         for (int i = lane; i < pb->m; i += NT) {
             double ad = r2[i];
             if (mode) ad += d1[pb->n + pb->m + i] - d1[pb->n + i];
@@ -248,20 +266,22 @@ struct Solver {
     }
 
     // solve (6) with iterative refinement on the unreduced system (reading S-7); returns #refinements
-    __device__ int solve_full(const double* b1, const double* b2, const double* b3, const double* b4,
-                              double* d1, double* d2, double* d3, double* d4) {
+    __device__ int solve_full(const Vec b1, const double* b2, const Vec b3, const Vec b4,
+                              Vec d1, double* d2, Vec d3, Vec d4) {
         reduced_solve(b1, b2, b3, b4, d1, d2, d3, d4);
         double bn = 0.0;
         for (int i = lane; i < nX; i += NT) bn = fmax(bn, fmax(fabs(b1[i]), fmax(fabs(b3[i]), fabs(b4[i]))));
         for (int i = lane; i < pb->m; i += NT) bn = fmax(bn, fabs(b2[i]));
         bn = c.tm.max(bn);
         int nref = 0;
-        double* e1 = V(L->e1); double* e2 = V(L->e2); double* e3 = V(L->e3); double* e4 = V(L->e4);
+        Vec e1 = VX(L->e1); double* e2 = VH(L->e2); Vec e3 = VX(L->e3); Vec e4 = VX(L->e4);
         while (nref < o->refine_max) {
             double dn;
+            const long long t0 = clock64();
             const double rn = full_residual(b1, b2, b3, b4, d1, d2, d3, d4, dn);
+            tph[3] += clock64() - t0;
             if (nref >= o->refine_min && rn <= o->residual_ratio_max * (bn + dn)) break;
-            reduced_solve(V(L->r1), V(L->r2), V(L->r3), V(L->r4), e1, e2, e3, e4);
+            reduced_solve(VX(L->r1), VH(L->r2), VX(L->r3), VX(L->r4), e1, e2, e3, e4);
             for (int i = lane; i < nX; i += NT) { d1[i] += e1[i]; d3[i] += e3[i]; d4[i] += e4[i]; }
             for (int i = lane; i < pb->m; i += NT) d2[i] += e2[i];
             c.tm.sync();
@@ -280,7 +300,7 @@ struct Solver {
     __device__ void iterate();
     __device__ void enter_restoration(double* rec, int kind);
     __device__ void try_exit_restoration();
-    __device__ double eval_point(const double* xt, double* ct, double& th_t, double& cm_t, double& fb, double& thb,
+    __device__ double eval_point(const Vec xt, double* ct, double& th_t, double& cm_t, double& fb, double& thb,
                                  double& cmb, double& fpn, double& fq);
     __device__ void write_outputs();
     __device__ void dbg_load(const double* st);

@@ -12,7 +12,7 @@ __device__ void Solver<C>::init_problem(long long id) {
     c.th = A->th + id * pb->nth;
     const double* th = c.th;
     const int N = pb->N;
-    double* x = V(L->x); double* y = V(L->y); double* zL = V(L->zL); double* zU = V(L->zU);
+    Vec x = VX(L->x); double* y = VH(L->y); Vec zL = VX(L->zL); Vec zU = VX(L->zU);
     const double* x0 = A->x0 + id * pb->n;
     for (int i = lane; i < pb->n; i += NT) x[i] = x0[i];
     // cost targets per knot / agent
@@ -61,17 +61,17 @@ __device__ void Solver<C>::init_problem(long long id) {
     c.eval_derivs(x, y, 1.0);
     n_deriv++;
     {
-        double* Sig = V(L->Sig); double* Hd = V(L->Hd); double* Dc = V(L->Dc);
-        double* rr = V(L->rr); double* b2 = V(L->b2); const double* g = V(L->g);
+        Vec Sig = VX(L->Sig); Vec Hd = VX(L->Hd); double* Dc = VH(L->Dc);
+        Vec rr = VX(L->rr); double* b2 = VH(L->b2); Vec g = VX(L->g);
         for (int i = lane; i < pb->n; i += NT) { Sig[i] = 1.0; Hd[i] = 0.0; rr[i] = -(g[i] - zL[i] + zU[i]); }
         for (int i = lane; i < pb->m; i += NT) { Dc[i] = 0.0; b2[i] = 0.0; }
         c.tm.sync();
         int nz;
         const int bad = K::factor(c, nz, false, false);
         n_fact++;
-        K::solve(c, rr, b2, V(L->dx), V(L->dy), false);
+        K::solve(c, rr, b2, VX(L->dx), VH(L->dy), false);
         n_solve++;
-        const double* dy = V(L->dy);
+        const double* dy = VH(L->dy);
         double ym = 0.0, ys = 0.0;
         for (int i = lane; i < pb->m; i += NT) { ym = fmax(ym, fabs(dy[i])); ys += dy[i]; }
         ym = c.tm.max(ym); ys = c.tm.sum(ys);
@@ -83,7 +83,7 @@ __device__ void Solver<C>::init_problem(long long id) {
     tau = fmax(o->tau_min, 1.0 - mu);
     dw_last = 0.0;
     bool fin;
-    f = c.eval_fc(x, V(L->c), theta, cmax, fin);  // I-7
+    f = c.eval_fc(x, VH(L->c), theta, cmax, fin);  // I-7
     n_fc++;
     theta_max = o->theta_max_fact * fmax(1.0, theta);
     theta_min = o->theta_min_fact * fmax(1.0, theta);
@@ -95,10 +95,12 @@ __device__ void Solver<C>::init_problem(long long id) {
 // mode ([7] sec 3.3): X = [x; p; n], f_R = rho sum(p+n) + zeta/2 ||D_R (x - x_R)||^2, c_R = c(x) - p + n; the base
 // problem's f, theta, ||c||_inf come back too (the exit test of Step R needs them).
 template <class C>
-__device__ double Solver<C>::eval_point(const double* xt, double* ct, double& th_t, double& cm_t, double& fb,
+__device__ double Solver<C>::eval_point(const Vec xt, double* ct, double& th_t, double& cm_t, double& fb,
                                         double& thb, double& cmb, double& fpn, double& fq) {
     bool fin;
-    fb = c.eval_fc(xt, ct, thb, cmb, fin);
+    const long long t0 = clock64();
+    fb = c.eval_fc(xt.a, ct, thb, cmb, fin);
+    tph[4] += clock64() - t0;
     n_fc++;
     if (!mode) { th_t = thb; cm_t = cmb; fpn = 0.0; fq = 0.0; return fb; }
     const int n = pb->n, m = pb->m;
@@ -125,7 +127,7 @@ __device__ void Solver<C>::enter_restoration(double* rec, int kind) {
     if (!o->enable_restoration || mode == 1) { status = JIPM_ST_RESTORATION_FAILED; return; }  // no nesting (A20)
     if (theta < o->tol) { status = JIPM_ST_RESTO_AT_FEASIBLE_POINT; return; }
     const int n = pb->n, m = pb->m;
-    double* x = V(L->x); double* y = V(L->y); double* zL = V(L->zL); double* zU = V(L->zU); double* cv = V(L->c);
+    Vec x = VX(L->x); double* y = VH(L->y); Vec zL = VX(L->zL); Vec zU = VX(L->zU); double* cv = VH(L->c);
     const double theta_k = theta;
     const double phi_k = phi(x, f, mu, n);
     filter_add((1.0 - o->gamma_theta) * theta_k, phi_k - o->gamma_phi * theta_k);
@@ -175,7 +177,7 @@ __device__ void Solver<C>::enter_restoration(double* rec, int kind) {
 template <class C>
 __device__ void Solver<C>::try_exit_restoration() {
     const int n = pb->n;
-    double* x = V(L->x); double* y = V(L->y); double* zL = V(L->zL); double* zU = V(L->zU);
+    Vec x = VX(L->x); double* y = VH(L->y); Vec zL = VX(L->zL); Vec zU = VX(L->zU);
     const double phi_b = phi(x, f_base, mu_reg, n);
     if (!isfinite(phi_b) || !(theta_base <= o->kappa_resto * theta_entry)) return;
     if (in_filter_of(V(L->filt), nfilt_reg, theta_max_reg, theta_base, phi_b)) return;
@@ -190,17 +192,17 @@ __device__ void Solver<C>::try_exit_restoration() {
     mu = mu_reg; tau = tau_reg; dw_last = dw_last_reg; theta_min = theta_min_reg; theta_max = theta_max_reg;
     nfilt = nfilt_reg;
     bool fin;
-    f = c.eval_fc(x, V(L->c), theta, cmax, fin);  // base c back into the c vector (same point: same values)
+    f = c.eval_fc(x, VH(L->c), theta, cmax, fin);  // base c back into the c vector (same point: same values)
     n_fc++;
 }
 
 // ---- Step A: one iteration (either mode) ---------------------------------------------------------------------
 template <class C>
 __device__ void Solver<C>::iterate() {
-    double* x = V(L->x); double* y = V(L->y); double* zL = V(L->zL); double* zU = V(L->zU);
-    double* cv = V(L->c); double* g = V(L->g);
-    double* b1 = V(L->b1); double* b2 = V(L->b2); double* b3 = V(L->b3); double* b4 = V(L->b4);
-    double* dx = V(L->dx); double* dy = V(L->dy); double* dzL = V(L->dzL); double* dzU = V(L->dzU);
+    Vec x = VX(L->x); double* y = VH(L->y); Vec zL = VX(L->zL); Vec zU = VX(L->zU);
+    double* cv = VH(L->c); Vec g = VX(L->g);
+    Vec b1 = VX(L->b1); double* b2 = VH(L->b2); Vec b3 = VX(L->b3); Vec b4 = VX(L->b4);
+    Vec dx = VX(L->dx); double* dy = VH(L->dy); Vec dzL = VX(L->dzL); Vec dzU = VX(L->dzU);
     const int n = pb->n, m = pb->m;
     double rec[JIPM_TRACE_W];
 #pragma unroll
@@ -209,7 +211,9 @@ __device__ void Solver<C>::iterate() {
     n_iter++;
     if (mode) n_resto++;
     // A-1 derivatives at (x, y): sigma_f = 0 in restoration mode (its objective is rho e^T(p+n) + zeta/2 ||D_R(x-x_R)||^2)
+    const long long t_it = clock64();
     c.eval_derivs(x, y, mode ? 0.0 : 1.0);
+    tph[0] += clock64() - t_it;
     n_deriv++;
     if (mode) {
         const double* xR = V(L->xR); const double* DR2 = V(L->DR2);
@@ -269,6 +273,7 @@ __device__ void Solver<C>::iterate() {
     double dw = 0.0, dc = 0.0;
     bool ic_ok;
     set_sigma(0.0, 0.0);
+    long long t_f = clock64();
     int bad = K::factor(c, nzero, mode != 0, true); nfact++;  // IC-1
     ic_ok = (bad == 0);
     if (!ic_ok) {
@@ -283,6 +288,7 @@ __device__ void Solver<C>::iterate() {
         }
     }
     n_fact += nfact;
+    tph[1] += clock64() - t_f;
     rec[1] = nfact; rec[2] = dw; rec[3] = dc; rec[14] = theta;
     if (!ic_ok) { rec[1] = 0; rec[2] = 0; rec[3] = 0; enter_restoration(rec, KIND_IC_FAIL); trace_put(rec); return; }
     if (dw > 0.0) dw_last = dw;
@@ -324,7 +330,7 @@ __device__ void Solver<C>::iterate() {
                                      o->delta * pow(theta_k, o->s_theta) / pow(-gd, o->s_phi));
     else if (gd < 0.0) a_min = o->gamma_alpha * fmin(o->gamma_theta, o->gamma_phi * theta_k / (-gd));
     else a_min = o->gamma_alpha * o->gamma_theta;
-    double* xt = V(L->xt); double* ct = V(L->ct);
+    Vec xt = VX(L->xt); double* ct = VH(L->ct);
     double alpha = a_max, alpha_acc = 0.0, phi_acc = 0.0, f_acc = 0.0, th_acc = 0.0, cm_acc = 0.0;
     double fb_acc = 0.0, thb_acc = 0.0, cmb_acc = 0.0, fpn_acc = 0.0, fq_acc = 0.0;
     int ntrial = 0, nsoc = 0, acc = -1;  // acc: 0 newton, 1 soc
@@ -342,7 +348,7 @@ __device__ void Solver<C>::iterate() {
         if (ntrial == 0 && isfinite(th_t) && th_t >= theta_k && o->max_soc > 0) {
             // second-order correction (Table I row 2)
             double* csoc = V(L->csoc); double* bs2 = V(L->bs2);
-            double* sx = V(L->sx); double* sy = V(L->sy); double* szL = V(L->szL); double* szU = V(L->szU);
+            Vec sx = VX(L->sx); double* sy = V(L->sy); Vec szL = VX(L->szL); Vec szU = VX(L->szU);
             for (int i = lane; i < m; i += NT) csoc[i] = alpha * cv[i] + ct[i];
             c.tm.sync();
             double theta_old = theta_k;
@@ -376,10 +382,10 @@ __device__ void Solver<C>::iterate() {
     rec[6] = ntrial; rec[7] = nsoc;
     if (acc < 0) { enter_restoration(rec, KIND_LS_FAIL); trace_put(rec); return; }
     // A-6 accept, A-7 filter augmentation
-    const double* ax = (acc == 1) ? V(L->sx) : dx;
+    const Vec ax = (acc == 1) ? VX(L->sx) : dx;
     const double* ay = (acc == 1) ? V(L->sy) : dy;
-    const double* azL = (acc == 1) ? V(L->szL) : dzL;
-    const double* azU = (acc == 1) ? V(L->szU) : dzU;
+    const Vec azL = (acc == 1) ? VX(L->szL) : dzL;
+    const Vec azU = (acc == 1) ? VX(L->szU) : dzU;
     (void)ax;
     const double a_z = ftb_dual(zL, zU, azL, azU, tau);
     const bool ftype = switching(alpha, gd, theta_k) && armijo(phi_acc, phi_k, alpha, gd);
@@ -413,7 +419,7 @@ __device__ void Solver<C>::iterate() {
 
 template <class C>
 __device__ void Solver<C>::write_outputs() {
-    const double* x = V(L->x); const double* y = V(L->y); const double* zL = V(L->zL); const double* zU = V(L->zU);
+    Vec x = VX(L->x); const double* y = VH(L->y); Vec zL = VX(L->zL); Vec zU = VX(L->zU);
     if (A->x_out) for (int i = lane; i < pb->n; i += NT) A->x_out[pid * pb->n + i] = x[i];
     if (A->lam_out) for (int i = lane; i < pb->m; i += NT) A->lam_out[pid * pb->m + i] = y[i];
     if (A->zL_out) for (int i = lane; i < pb->n; i += NT) A->zL_out[pid * pb->n + i] = zL[i];

@@ -36,7 +36,7 @@ struct jipm_solver {
     unsigned long long* d_stats = nullptr;
     double* trace = nullptr;
     int trace_cap = 0;
-    long long stats[8] = {0};
+    long long stats[16] = {0};
     DbgLay dbg;
 };
 
@@ -89,42 +89,54 @@ extern "C" int jipm_family_sizes(int family, const jipm_family_dims* d, int64_t*
 
 // Workspace layout of one slot.  Arrays are laid out in PRIORITY order; the first L.nsm doubles (as many whole
 // arrays as the shared-memory budget holds) live in shared memory, the rest in the slot's global scratch.
-static void build_layout(jipm_solver* s, int sm_budget_doubles) {
+static int build_layout(jipm_solver* s, int sm_budget_doubles) {
     const Pb& pb = s->pb;
     const int n = pb.n, m = pb.m, N = pb.N, NX = s->NX, NU = s->NU, NZ = s->NZ;
     const int pd = (pb.family == JIPM_FAM_POINTMASS2D) ? 2 : 3;
-    const int nX = n + 2 * m;  // restoration mode iterates on X = [x; p; n]
     Lay& L = s->L;
     struct Ent { int Lay::*f; int cnt; };
     const int rkn = pb.family == JIPM_FAM_POINTMASS2D ? 0 : N * pb.na * 4 * RKW;
-    const Ent order[] = {
+    const int npad = (n + 1) & ~1, tpad = (2 * m + 1) & ~1;
+    const Ent hot[] = {
         // the factor and what every solve streams through
         {&Lay::Psi, N * NX * NX}, {&Lay::pv, (N + 1) * NX}, {&Lay::qv, N * NX}, {&Lay::wv, N * NX}, {&Lay::sv, N * NX}, {&Lay::tv, N * NU},
         {&Lay::T, (N + 1) * NX * NX}, {&Lay::Kf, N * NU * NX}, {&Lay::Gf, N * NU * NU},
-        {&Lay::J, N * NX * NZ}, {&Lay::Dc, m}, {&Lay::gv, N * pb.ng * pd}, {&Lay::tgt, (N + 1) * pb.na * pd},
-        {&Lay::filt, 2 * MAX_FILTER}, {&Lay::filtR, 2 * MAX_FILTER},
+        {&Lay::J, N * NX * NZ}, {&Lay::Dc, m}, {&Lay::gv, N * pb.ng * pd}, {&Lay::dgv, N * pb.ng}, {&Lay::tgt, (N + 1) * pb.na * pd},
+        {&Lay::bl, n}, {&Lay::bu, n},
+        {&Lay::filt, 2 * MAX_FILTER},
         // m-vectors
-        {&Lay::y, m}, {&Lay::c, m}, {&Lay::b2, m}, {&Lay::dy, m}, {&Lay::rc2, m}, {&Lay::ct, m}, {&Lay::r2, m}, {&Lay::e2, m},
+        {&Lay::y, m}, {&Lay::c, m}, {&Lay::b2, m}, {&Lay::dy, m}, {&Lay::ct, m}, {&Lay::r2, m}, {&Lay::e2, m},
         {&Lay::W, N * NZ * NZ + NX * NX},
-        // primal-sized vectors (n + 2m entries: the tail is only touched in restoration mode)
-        {&Lay::x, nX}, {&Lay::rr, nX}, {&Lay::dx, nX}, {&Lay::Sig, nX}, {&Lay::xt, nX}, {&Lay::zL, nX}, {&Lay::zU, nX},
-        {&Lay::b1, nX}, {&Lay::b3, nX}, {&Lay::b4, nX}, {&Lay::dzL, nX}, {&Lay::dzU, nX}, {&Lay::g, nX}, {&Lay::Hd, nX},
-        {&Lay::r1, nX}, {&Lay::r3, nX}, {&Lay::r4, nX}, {&Lay::e1, nX}, {&Lay::e3, nX}, {&Lay::e4, nX},
-        {&Lay::rk, rkn},
-        {&Lay::sx, nX}, {&Lay::sy, m}, {&Lay::szL, nX}, {&Lay::szU, nX}, {&Lay::csoc, m}, {&Lay::bs2, m},
-        {&Lay::xR, n}, {&Lay::DR2, n},
+    };
+    // primal-sized vectors: heads (n entries) contiguous with stride npad, in priority order; their restoration tails
+    // (2m entries: p and n of Step R) live apart, always in the global scratch
+    int Lay::*const primal[] = {
+        &Lay::x, &Lay::rr, &Lay::dx, &Lay::Sig, &Lay::xt, &Lay::zL, &Lay::zU, &Lay::b1, &Lay::dzL, &Lay::dzU, &Lay::b3, &Lay::b4,
+        &Lay::g, &Lay::Hd, &Lay::r1, &Lay::r3, &Lay::r4, &Lay::e1, &Lay::e3, &Lay::e4, &Lay::sx, &Lay::szL, &Lay::szU,
+    };
+    const Ent cold[] = {
+        {&Lay::rk, rkn}, {&Lay::sy, m}, {&Lay::csoc, m}, {&Lay::bs2, m}, {&Lay::rc2, m},
+        {&Lay::xR, n}, {&Lay::DR2, n}, {&Lay::filtR, 2 * MAX_FILTER},
     };
     int o = 0;
     L.nsm = 0;
     bool in_sm = true;
-    for (const Ent& e : order) {
-        const int cnt = (e.cnt + 1) & ~1;  // keep 16-byte alignment
+    auto place = [&](int Lay::*f, int cnt0) {
+        const int cnt = (cnt0 + 1) & ~1;  // keep 16-byte alignment
         if (in_sm && o + cnt > sm_budget_doubles) { in_sm = false; L.nsm = o; }
-        L.*(e.f) = o;
+        L.*f = o;
         o += cnt;
-    }
-    if (in_sm) L.nsm = o;
+    };
+    for (const Ent& e : hot) place(e.f, e.cnt);
+    const int hot_fits = in_sm ? 1 : 0;  // the whole hot group is shared-memory resident
+    L.pv0 = o; L.npad = npad; L.tpad = tpad;
+    for (auto f : primal) place(f, n);
+    for (const Ent& e : cold) place(e.f, e.cnt);
+    if (in_sm) { in_sm = false; L.nsm = o; }
+    L.tail0 = o;
+    o += tpad * (int)(sizeof(primal) / sizeof(primal[0]));
     L.total = o;
+    return hot_fits;
 }
 
 static cudaError_t dispatch(jipm_solver* s, const Args& a) { return s->inst.launch(a, s->stream); }
@@ -177,7 +189,17 @@ extern "C" int jipm_create(jipm_solver** out, int family, const jipm_family_dims
                                          (long)prop.sharedMemPerBlockOptin);
     const long budget = per_team / (long)sizeof(double) - s->inst.info.sm_fixed;
     if (budget < 0) { delete s; return fail(JIPM_ERR_NOMEM, "stage tiles do not fit shared memory"); }
-    build_layout(s, (int)budget);
+    int hot_fits = build_layout(s, (int)budget);
+    if (!hot_fits && s->inst.info.hot_sm) {
+        // the hot group does not fit: the general instantiation of the family (generic loads, arrays wherever they fit)
+        if (family == JIPM_FAM_POINTMASS2D) { delete s; return fail(JIPM_ERR_NOMEM, "problem too large for the point-mass kernel"); }
+        s->inst = inst_q1g();
+        s->teams_per_sm = std::max(1, std::min(s->inst.info.min_blocks, 2048 / s->inst.info.nt));
+        const long pt = std::min<long>((long)prop.sharedMemPerMultiprocessor / s->teams_per_sm - 1024, (long)prop.sharedMemPerBlockOptin);
+        const long b2 = pt / (long)sizeof(double) - s->inst.info.sm_fixed;
+        if (b2 < 0) { delete s; return fail(JIPM_ERR_NOMEM, "stage tiles do not fit shared memory"); }
+        hot_fits = build_layout(s, (int)b2);
+    }
     s->dbg = make_dbglay(pb.n, pb.m, pb.N, s->NX, s->NZ);
     if (resident_slots == 0) resident_slots = (int64_t)s->teams_per_sm * prop.multiProcessorCount;  // fill the GPU
     s->n_slots = (int)resident_slots;
@@ -186,7 +208,7 @@ extern "C" int jipm_create(jipm_solver** out, int family, const jipm_family_dims
         (e = cudaMalloc(&s->d_xU, n * sizeof(double))) != cudaSuccess ||
         (e = cudaMalloc(&s->d_ws, (size_t)s->n_slots * (s->L.total - s->L.nsm + 2) * sizeof(double))) != cudaSuccess ||
         (e = cudaMalloc(&s->d_queue, sizeof(int))) != cudaSuccess ||
-        (e = cudaMalloc(&s->d_stats, 8 * sizeof(unsigned long long))) != cudaSuccess) {
+        (e = cudaMalloc(&s->d_stats, 16 * sizeof(unsigned long long))) != cudaSuccess) {
         std::string msg = std::string("cudaMalloc: ") + cudaGetErrorString(e);
         jipm_destroy(s);
         return fail(JIPM_ERR_NOMEM, msg);
@@ -218,12 +240,12 @@ static int run(jipm_solver* s, Args& a) {
     a.trace = s->trace; a.trace_cap = s->trace_cap;
     a.dbg_len = s->dbg.len;
     CUDA_TRY(cudaMemsetAsync(s->d_queue, 0, sizeof(int), s->stream));
-    CUDA_TRY(cudaMemsetAsync(s->d_stats, 0, 8 * sizeof(unsigned long long), s->stream));
+    CUDA_TRY(cudaMemsetAsync(s->d_stats, 0, 16 * sizeof(unsigned long long), s->stream));
     CUDA_TRY(dispatch(s, a));
-    unsigned long long st[8];
+    unsigned long long st[16];
     CUDA_TRY(cudaMemcpyAsync(st, s->d_stats, sizeof(st), cudaMemcpyDeviceToHost, s->stream));
     CUDA_TRY(cudaStreamSynchronize(s->stream));
-    for (int i = 0; i < 8; ++i) s->stats[i] = (long long)st[i];
+    for (int i = 0; i < 16; ++i) s->stats[i] = (long long)st[i];
     s->stats[5] = a.n_slots; s->stats[6] = 1;
     return JIPM_OK;
 }
@@ -276,7 +298,7 @@ extern "C" int jipm_solve_batch_host(jipm_solver* s, int64_t P, const double* x0
 
 extern "C" int jipm_last_stats(jipm_solver* s, int64_t* stats, int64_t n_stats) {
     if (!s || !stats) return fail(JIPM_ERR_ARG, "NULL argument");
-    for (int64_t i = 0; i < n_stats && i < 8; ++i) stats[i] = s->stats[i];
+    for (int64_t i = 0; i < n_stats && i < 16; ++i) stats[i] = s->stats[i];
     return JIPM_OK;
 }
 

@@ -9,17 +9,17 @@ namespace jipm {
 template <class C>
 __device__ void Solver<C>::dbg_load(const double* st) {
     const DbgLay D = make_dbglay(pb->n, pb->m, pb->N, NX, NZ);
-    double* x = V(L->x); double* y = V(L->y); double* zL = V(L->zL); double* zU = V(L->zU);
+    double* x = V(L->x); double* y = VH(L->y); double* zL = V(L->zL); double* zU = V(L->zU);
     for (int i = lane; i < pb->n; i += NT) { x[i] = st[D.x + i]; zL[i] = st[D.zL + i]; zU[i] = st[D.zU + i]; }
     for (int i = lane; i < pb->m; i += NT) y[i] = st[D.y + i];
-    for (int i = lane; i < 2 * MAX_FILTER; i += NT) V(L->filt)[i] = st[D.filt + i];
+    for (int i = lane; i < 2 * MAX_FILTER; i += NT) VH(L->filt)[i] = st[D.filt + i];
     mode = 0; nX = pb->n;
     mu = st[D.sc + 0]; tau = st[D.sc + 1]; dw_last = st[D.sc + 2];
     theta_min = st[D.sc + 3]; theta_max = st[D.sc + 4];
     k = (int)st[D.sc + 5]; status = (int)st[D.sc + 6]; nfilt = (int)st[D.sc + 7];
     c.tm.sync();
     bool fin;
-    f = c.eval_fc(x, V(L->c), theta, cmax, fin);
+    f = c.eval_fc(x, VH(L->c), theta, cmax, fin);
 }
 
 template <class C>
@@ -32,11 +32,11 @@ __device__ void Solver<C>::dbg_store(double* st) {
         st[D.g + i] = V(L->g)[i];
     }
     for (int i = lane; i < pb->m; i += NT) {
-        st[D.y + i] = V(L->y)[i]; st[D.dy + i] = V(L->dy)[i]; st[D.c + i] = V(L->c)[i];
+        st[D.y + i] = VH(L->y)[i]; st[D.dy + i] = VH(L->dy)[i]; st[D.c + i] = VH(L->c)[i];
     }
-    for (int i = lane; i < 2 * MAX_FILTER; i += NT) st[D.filt + i] = V(L->filt)[i];
-    for (int i = lane; i < pb->N * NX * NZ; i += NT) st[D.J + i] = V(L->J)[i];
-    for (int i = lane; i < pb->N * NZ * NZ + NX * NX; i += NT) st[D.W + i] = V(L->W)[i];
+    for (int i = lane; i < 2 * MAX_FILTER; i += NT) st[D.filt + i] = VH(L->filt)[i];
+    for (int i = lane; i < pb->N * NX * NZ; i += NT) st[D.J + i] = VH(L->J)[i];
+    for (int i = lane; i < pb->N * NZ * NZ + NX * NX; i += NT) st[D.W + i] = VH(L->W)[i];
     if (lane == 0) {
         st[D.sc + 0] = mu; st[D.sc + 1] = tau; st[D.sc + 2] = dw_last; st[D.sc + 3] = theta_min;
         st[D.sc + 4] = theta_max; st[D.sc + 5] = k; st[D.sc + 6] = status; st[D.sc + 7] = nfilt;
@@ -45,13 +45,12 @@ __device__ void Solver<C>::dbg_store(double* st) {
 
 template <class C, int MINB>
 __global__ void __launch_bounds__(C::NT, MINB) jipm_slot_kernel() {
-    extern __shared__ double smem[];
     constexpr int NT = C::NT;
     const ArgsProxy A;
     const int lane = threadIdx.x;  // one team per CTA
     const int slot = blockIdx.x;
     double* ws = A->ws + (int64_t)slot * A->ws_stride;
-    Ctx<C> ctx(ws, smem, lane, 1);
+    Ctx<C> ctx(ws, jipm_smem, lane, 1);
     Solver<C> S(ctx);
     while (true) {
         int id = 0;
@@ -64,7 +63,7 @@ __global__ void __launch_bounds__(C::NT, MINB) jipm_slot_kernel() {
             // targets and J zeroing as in init
             {
                 const PbProxy pb;
-                double* tgt = ctx.v(A->L.tgt);
+                double* tgt = ctx.vh(A->L.tgt);
                 for (int it = lane; it < (pb->N + 1) * C::NA; it += NT) {
                     const int kk = it / C::NA, a = it % C::NA;
                     if (pb->family == JIPM_FAM_QUAD_TRACK) {
@@ -77,7 +76,7 @@ __global__ void __launch_bounds__(C::NT, MINB) jipm_slot_kernel() {
                     }
                 }
                 if (C::NA > 1)
-                    for (int it = lane; it < pb->N * C::NX * C::NZ; it += NT) ctx.v(A->L.J)[it] = 0.0;
+                    for (int it = lane; it < pb->N * C::NX * C::NZ; it += NT) ctx.vh(A->L.J)[it] = 0.0;
                 ctx.tm.sync();
             }
             ctx.tm.sync();
@@ -85,11 +84,15 @@ __global__ void __launch_bounds__(C::NT, MINB) jipm_slot_kernel() {
             for (int s = 0; s < A->dbg_steps && S.status == JIPM_ST_NOT_RUN; ++s) S.iterate();
             S.dbg_store(A->dbg_state + (int64_t)id * A->dbg_len);
         } else {
+            const long long t0i = clock64();
             S.init_problem(id);
             if (A->dbg_mode == 1) {
                 S.dbg_store(A->dbg_state + (int64_t)id * A->dbg_len);
             } else {
+                const long long t1 = clock64();
+                S.tph[6] += t1 - t0i;
                 while (S.status == JIPM_ST_NOT_RUN) S.iterate();
+                S.tph[5] += clock64() - t1;
                 S.write_outputs();
             }
         }
@@ -102,6 +105,7 @@ __global__ void __launch_bounds__(C::NT, MINB) jipm_slot_kernel() {
         atomicAdd(&A->stats[3], (unsigned long long)S.n_deriv);
         atomicAdd(&A->stats[4], (unsigned long long)S.n_fc);
         atomicAdd(&A->stats[7], (unsigned long long)S.n_resto);
+        for (int i = 0; i < 8; ++i) atomicAdd(&A->stats[8 + i], S.tph[i]);
     }
 }
 

@@ -30,55 +30,27 @@ struct Kkt {
     static constexpr int NX = C::NX, NU = C::NU, NZ = C::NZ, PD = C::PD, AX = C::AX, NA = C::NA, NT = C::NT;
     using X = Ctx<C>;
 
-    // dot product of length n with 4 independent partial sums (dependent-chain latency / 4)
-    __device__ static __forceinline__ double dot4(const double* a, int sa, const double* b, int sb, int n) {
+    // dot product with 4 independent partial sums (dependent-chain latency / 4), compile-time length and strides: fully unrolled, immediate offsets
+    template <int LEN, int SA, int SB>
+    __device__ static __forceinline__ double dotc(const double* a, const double* b) {
         double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
-        int l = 0;
-        for (; l + 3 < n; l += 4) {
-            s0 = fma(a[l * sa], b[l * sb], s0);
-            s1 = fma(a[(l + 1) * sa], b[(l + 1) * sb], s1);
-            s2 = fma(a[(l + 2) * sa], b[(l + 2) * sb], s2);
-            s3 = fma(a[(l + 3) * sa], b[(l + 3) * sb], s3);
+#pragma unroll
+        for (int l = 0; l + 3 < LEN; l += 4) {
+            s0 = fma(a[l * SA], b[l * SB], s0);
+            s1 = fma(a[(l + 1) * SA], b[(l + 1) * SB], s1);
+            s2 = fma(a[(l + 2) * SA], b[(l + 2) * SB], s2);
+            s3 = fma(a[(l + 3) * SA], b[(l + 3) * SB], s3);
         }
-        for (; l < n; ++l) s0 = fma(a[l * sa], b[l * sb], s0);
+#pragma unroll
+        for (int l = LEN & ~3; l < LEN; ++l) s0 = fma(a[l * SA], b[l * SB], s0);
         return (s0 + s1) + (s2 + s3);
-    }
-
-    // Dg weight of the condensed (slack, multiplier) pair (k, j)
-    __device__ static __forceinline__ double Dg(const X& c, int k, int j) {
-        const double sig = c.v(c.L->Sig)[c.is(k) + j], dcg = c.v(c.L->Dc)[c.icg(k) + j];
-        return 1.0 / (1.0 / sig + dcg);
-    }
-
-    // add sum_j Dg_j G_j^T G_j of stage k (k>=1) to the position entries of the tile M (leading dim ld)
-    __device__ static void add_cond(const X& c, int k, double* M, int ld) {
-        const PbProxy pb;
-        const double* gv = c.v(c.L->gv) + (k - 1) * pb->ng * PD;
-        constexpr int NPOS = NA * PD;
-        for (int e = c.lane; e < NPOS * NPOS; e += NT) {
-            const int r = e / NPOS, q = e % NPOS;
-            const int a = r / PD, i = r % PD, b = q / PD, i2 = q % PD;
-            double s = 0.0;
-            if (pb->family == JIPM_FAM_MULTIQUAD) {
-                for (int j = 0; j < pb->ng; ++j) {
-                    int pa, pb2; c.pair_ab(j, pa, pb2);
-                    const double sa = (pa == a) ? 1.0 : (pb2 == a ? -1.0 : 0.0);
-                    const double sb = (pa == b) ? 1.0 : (pb2 == b ? -1.0 : 0.0);
-                    if (sa != 0.0 && sb != 0.0) s += sa * sb * Dg(c, k, j) * gv[j * PD + i] * gv[j * PD + i2];
-                }
-            } else {
-                for (int j = 0; j < pb->ng; ++j) s += Dg(c, k, j) * gv[j * PD + i] * gv[j * PD + i2];
-            }
-            M[(AX * a + i) * ld + AX * b + i2] += s;
-        }
-        c.tm.sync();
     }
 
     // T <- (I + P D)^{-1} P in place on the NX x NX tile sT (symmetric), D = Dc at rows [row0, row0+NX).
     // Returns the number of non-positive pivots of I + E P E (0 when D == 0).  Uses sM (>= 2 NX^2) as scratch.
     __device__ static int transform_T(const X& c, double* sT, double* sM, int row0, bool any_dc) {
         if (!any_dc) return 0;
-        const double* Dc = c.v(c.L->Dc) + row0;
+        const double* Dc = c.vh(c.L->Dc) + row0;
         // G = I + E P E (NX x NX), E = sqrt(D); solve G Z = E P by an unpivoted LDL^T of G, then T = P - (P E) Z
         double* G = sM;
         double* Z = sM + NX * NX;
@@ -119,7 +91,7 @@ struct Kkt {
         c.tm.sync();
         for (int e = c.lane; e < NX * NX; e += NT) {
             const int i = e / NX, q = e % NX;
-            G[e] = sT[e] - dot4(sT + i, NX, Z + q, NX, NX);  // sum_l P[l][i] (e_l Z[l][q])   (P symmetric)
+            G[e] = sT[e] - dotc<NX, NX, NX>(sT + i, Z + q);  // sum_l P[l][i] (e_l Z[l][q])   (P symmetric)
         }
         c.tm.sync();
         for (int e = c.lane; e < NX * NX; e += NT) {
@@ -130,153 +102,171 @@ struct Kkt {
         return bad;
     }
 
-    // Factor.  Reads W, J, Sig, Dc, gv from the workspace; writes T, Kf, Gf, Psi.  Returns the number of pivots with
-    // the wrong sign (0 <=> inertia (n, m, 0)); nzero counts exactly-zero pivots.  any_dc: some Dc entry is non-zero.
+    // Factor.  Reads W, J, Sig, Dc, gv from the workspace; writes T, Kf, Gf, Psi, dgv.  Returns the number of pivots
+    // with the wrong sign (0 <=> inertia (n, m, 0)); nzero counts exactly-zero pivots.  any_dc: some Dc entry != 0.
+    // Per stage (regular mode): T J | M = Q + J^T (T J) + condensed slacks | nu Gauss-Jordan pivots on the control
+    // block, ping-pong between two tiles (afterwards the tile holds P_k, Kf_k, G_k at once) | Phi, stores.
     __device__ static __noinline__ int factor(const X& c, int& nzero, bool any_dc, bool useW) {
         const PbProxy pb;
-        const int N = pb->N, lane = c.lane;
-        double* sT = c.sm + C::SM_T;     // NX x NX   current T_{k+1} / P_k
-        double* sJ = c.sm + C::SM_J;     // NX x NZ   J_k = [A B]
-        double* sM = c.sm + C::SM_M;     // NZ x NZ   stage tile (>= 2 NX^2: scratch of transform_T)
-        double* sTJ = c.sm + C::SM_TJ;   // NX x NZ   T J, later Phi (NX x NX)
-        double* sK = c.sm + C::SM_K;     // NU x NX   Kf ; then NU x NU Linv
-        double* sLi = sK + NU * NX;
+        const int N = pb->N, lane = c.lane, ng = pb->ng;
+        double* sT = c.smt(C::SM_T);     // NX x NX   current T_{k+1} / P_k
+        double* sJc = c.smt(C::SM_J);    // NX x NZ   copy of J_k when J is not shared-memory resident
+        double* tA = c.smt(C::SM_M);     // NZ x NZ   stage tile (>= 2 NX^2: scratch of transform_T)
+        double* tB = c.smt(C::SM_M2);    // NZ x NZ   second tile of the Gauss-Jordan ping-pong
+        double* sTJ = c.smt(C::SM_TJ);   // NX x NZ   T J, later Phi (NX x NX)
         const double* Sig = c.v(c.L->Sig);
-        const double* Dc = c.v(c.L->Dc);
+        const double* Dc = c.vh(c.L->Dc);
+        const double* gvv = c.vh(c.L->gv);
+        double* dgv = c.vh(c.L->dgv);
+        const bool j_in_sm = c.L->J < c.L->nsm;
         int bad = 0;
         nzero = 0;
+        // weights of the condensed (slack, multiplier) pairs, once per factorisation (the solves reuse them)
+        for (int it = lane; it < N * ng; it += NT) {
+            const int k = it / ng + 1, j = it % ng;
+            dgv[it] = 1.0 / (1.0 / Sig[c.is(k) + j] + Dc[c.icg(k) + j]);
+        }
+        c.tm.sync();
         // terminal block
         {
             const double* WN = c.Wk(N);
+            double* TN = c.vh(c.L->T) + N * NX * NX;
             for (int e = lane; e < NX * NX; e += NT) {
                 const int r = e / NX, q = e % NX;
-                sT[e] = (useW ? WN[e] : 0.0) + (r == q ? Sig[c.ix(N) + r] : 0.0);
+                double v = (useW ? WN[e] : 0.0) + (r == q ? Sig[c.ix(N) + r] : 0.0);
+                if (ng > 0) v += cond_entry(c, gvv, dgv, N, r, q);
+                sT[e] = v;
+                if (!any_dc) TN[e] = v;
             }
             c.tm.sync();
-            if (pb->ng > 0) add_cond(c, N, sT, NX);
-            bad += transform_T(c, sT, sM, c.icd(N), any_dc);
-            double* TN = c.v(c.L->T) + N * NX * NX;
-            for (int e = lane; e < NX * NX; e += NT) TN[e] = sT[e];
-            c.tm.sync();
+            if (any_dc) {
+                bad += transform_T(c, sT, tA, c.icd(N), true);
+                for (int e = lane; e < NX * NX; e += NT) TN[e] = sT[e];
+                c.tm.sync();
+            }
         }
         for (int k = N - 1; k >= 0; --k) {
-            const double* Jg = c.Jk(k);
-            for (int e = lane; e < NX * NZ; e += NT) sJ[e] = Jg[e];
-            c.tm.sync();
+            const double* sJ = c.Jk(k);
+            if (!j_in_sm) {
+                for (int e = lane; e < NX * NZ; e += NT) sJc[e] = sJ[e];
+                sJ = sJc;
+                c.tm.sync();
+            }
             // TJ = T_{k+1} J_k
             for (int e = lane; e < NX * NZ; e += NT) {
                 const int l = e / NZ, j = e % NZ;
-                sTJ[e] = dot4(sT + l * NX, 1, sJ + j, NZ, NX);
+                sTJ[e] = dotc<NX, 1, NZ>(sT + l * NX, sJ + j);
             }
             c.tm.sync();
-            // M = Q_k + J^T (T J)
+            // M = Q_k + J^T (T J) + condensed slacks
             const double* Wg = c.Wk(k);
             for (int e = lane; e < NZ * NZ; e += NT) {
                 const int a = e / NZ, j = e % NZ;
-                double m = dot4(sJ + a, NZ, sTJ + j, NZ, NX);
+                double m = dotc<NX, NZ, NZ>(sJ + a, sTJ + j);
                 if (useW) m += Wg[e];
                 if (a == j) m += Sig[c.zidx(k, j)];
-                sM[e] = m;
+                if (k >= 1 && ng > 0 && a < NX && j < NX) m += cond_entry(c, gvv, dgv, k, a, j);
+                tA[e] = m;
             }
             c.tm.sync();
-            if (k >= 1 && pb->ng > 0) add_cond(c, k, sM, NZ);
-            // eliminate the controls: pivots NX .. NZ-1 (element-parallel rank-1 updates)
+            // Gauss-Jordan pivots on the controls NX .. NZ-1: every element from the previous tile, no races
+            double* src = tA; double* dst = tB;
             for (int p = 0; p < NU; ++p) {
                 const int pp = NX + p;
-                double d = sM[pp * NZ + pp];
+                double d = src[pp * NZ + pp];
                 if (!(d > 0.0)) { bad++; if (d == 0.0) { nzero++; d = 1.0; } }
                 const double id = 1.0 / d;
                 for (int e = lane; e < NZ * NZ; e += NT) {
                     const int a = e / NZ, b = e % NZ;
-                    if ((a < NX || a > pp) && (b < NX || b > pp)) sM[e] -= sM[a * NZ + pp] * (sM[pp * NZ + b] * id);
+                    const double rb = src[pp * NZ + b] * id, ca = src[a * NZ + pp];
+                    double v;
+                    if (a == pp) v = (b == pp) ? id : rb;
+                    else if (b == pp) v = -ca * id;
+                    else v = src[e] - ca * rb;
+                    dst[e] = v;
                 }
                 c.tm.sync();
+                double* t = src; src = dst; dst = t;
             }
-            // Linv = L_uu^{-1} (unit lower; thread <-> column), pivots d_p on the diagonal of the tile
-            for (int q = lane; q < NU; q += NT) {
-                for (int r = 0; r < NU; ++r) {
-                    double v = (r == q) ? 1.0 : 0.0;
-                    if (r > q) {
-                        for (int t = q; t < r; ++t) {
-                            double dt = sM[(NX + t) * NZ + NX + t];
-                            if (dt == 0.0) dt = 1.0;
-                            v -= (sM[(NX + r) * NZ + NX + t] / dt) * sLi[t * NU + q];
-                        }
-                    }
-                    sLi[r * NU + q] = (r >= q) ? v : 0.0;
-                }
-            }
-            c.tm.sync();
-            // Kf = L^{-T} X^T, X[i][p] = M[i][NX+p]/d_p ;  Gf = L^{-T} D^{-1} L^{-1}
-            double* Kg = c.v(c.L->Kf) + k * NU * NX;
-            double* Gg = c.v(c.L->Gf) + k * NU * NU;
-            for (int e = lane; e < NU * NX + NU * NU; e += NT) {
-                if (e < NU * NX) {
-                    const int p = e / NX, i = e % NX;
-                    double s = 0.0;
-                    for (int q = p; q < NU; ++q) {
-                        double dq = sM[(NX + q) * NZ + NX + q];
-                        if (dq == 0.0) dq = 1.0;
-                        s += sLi[q * NU + p] * (sM[i * NZ + NX + q] / dq);
-                    }
-                    sK[e] = s; Kg[e] = s;
-                } else {
-                    const int e2 = e - NU * NX, p = e2 / NU, q = e2 % NU;
-                    double s = 0.0;
-                    for (int r = (p > q ? p : q); r < NU; ++r) {
-                        double dr = sM[(NX + r) * NZ + NX + r];
-                        if (dr == 0.0) dr = 1.0;
-                        s += sLi[r * NU + p] * sLi[r * NU + q] / dr;
-                    }
-                    Gg[e2] = s;
-                }
-            }
-            c.tm.sync();
-            // Phi = A - B Kf  (into sTJ, NX x NX)
+            // src: [[P_k, -Kf^T], [Kf, G]].  Phi = A - B Kf; stores
+            double* Kg = c.vh(c.L->Kf) + k * NU * NX;
+            double* Gg = c.vh(c.L->Gf) + k * NU * NU;
+            double* Pg = c.vh(c.L->Psi) + k * NX * NX;
+            double* Tg = c.vh(c.L->T) + k * NX * NX;
             for (int e = lane; e < NX * NX; e += NT) {
                 const int i = e / NX, a = e % NX;
-                sTJ[e] = sJ[i * NZ + a] - dot4(sJ + i * NZ + NX, 1, sK + a, NX, NU);
+                const double phi = sJ[i * NZ + a] - dotc<NU, 1, NZ>(sJ + i * NZ + NX, src + NX * NZ + a);
+                if (any_dc) sTJ[e] = phi;
+                else {
+                    Pg[e] = phi;
+                    const double tn = 0.5 * (src[i * NZ + a] + src[a * NZ + i]);
+                    sT[e] = tn; Tg[e] = tn;
+                }
             }
+            for (int e = lane; e < NU * NX; e += NT) Kg[e] = src[(NX + e / NX) * NZ + e % NX];
+            for (int e = lane; e < NU * NU; e += NT) Gg[e] = src[(NX + e / NU) * NZ + NX + e % NU];
             c.tm.sync();
-            // Psi = (I - D_{k+1} T_{k+1}) Phi
-            double* Pg = c.v(c.L->Psi) + k * NX * NX;
-            const int r0 = c.icd(k + 1);
-            for (int e = lane; e < NX * NX; e += NT) {
-                const int i = e / NX, a = e % NX;
-                double v = sTJ[e];
-                if (any_dc) v -= Dc[r0 + i] * dot4(sT + i * NX, 1, sTJ + a, NX, NX);
-                Pg[e] = v;
+            if (any_dc) {
+                // Psi = (I - D_{k+1} T_{k+1}) Phi, then P_k -> T_k = (I + P_k D_k)^{-1} P_k
+                const int r0 = c.icd(k + 1);
+                for (int e = lane; e < NX * NX; e += NT) {
+                    const int i = e / NX, a = e % NX;
+                    Pg[e] = sTJ[e] - Dc[r0 + i] * dotc<NX, 1, NX>(sT + i * NX, sTJ + a);
+                }
+                c.tm.sync();
+                for (int e = lane; e < NX * NX; e += NT) {
+                    const int r = e / NX, q = e % NX;
+                    sT[e] = 0.5 * (src[r * NZ + q] + src[q * NZ + r]);
+                }
+                c.tm.sync();
+                bad += transform_T(c, sT, dst, c.icd(k), true);
+                for (int e = lane; e < NX * NX; e += NT) Tg[e] = sT[e];
+                c.tm.sync();
             }
-            // P_k = symmetrised x-block of the tile (sT is still read by the Psi loop above: barrier first)
-            c.tm.sync();
-            for (int e = lane; e < NX * NX; e += NT) {
-                const int r = e / NX, q = e % NX;
-                sT[e] = 0.5 * (sM[r * NZ + q] + sM[q * NZ + r]);
-            }
-            c.tm.sync();
-            bad += transform_T(c, sT, sM, c.icd(k), any_dc);
-            double* Tg = c.v(c.L->T) + k * NX * NX;
-            for (int e = lane; e < NX * NX; e += NT) Tg[e] = sT[e];
-            c.tm.sync();
         }
         return bad;
+    }
+
+    // entry (r, q) of sum_j Dg_j G_j^T G_j of stage k (k >= 1) in the x-block (0 outside the position entries)
+    __device__ static __forceinline__ double cond_entry(const X& c, const double* gvv, const double* dgv, int k, int r, int q) {
+        const int a = r / AX, i = r % AX, b = q / AX, i2 = q % AX;
+        if (i >= PD || i2 >= PD) return 0.0;
+        const PbProxy pb;
+        const int ng = pb->ng;
+        const double* gv = gvv + (k - 1) * ng * PD;
+        const double* dg = dgv + (k - 1) * ng;
+        double s = 0.0;
+        if (pb->family == JIPM_FAM_MULTIQUAD) {
+            for (int j = 0; j < ng; ++j) {
+                int pa, pb2; c.pair_ab(j, pa, pb2);
+                const double sa = (pa == a) ? 1.0 : (pb2 == a ? -1.0 : 0.0);
+                const double sb = (pa == b) ? 1.0 : (pb2 == b ? -1.0 : 0.0);
+                if (sa != 0.0 && sb != 0.0) s += sa * sb * dg[j] * gv[j * PD + i] * gv[j * PD + i2];
+            }
+        } else {
+            if (a != 0 || b != 0) return 0.0;
+            for (int j = 0; j < ng; ++j) s += dg[j] * gv[j * PD + i] * gv[j * PD + i2];
+        }
+        return s;
     }
 
     // condensed right-hand side contribution to x_k position entry (agent a, coordinate i), k >= 1:
     //   sum_j G_j^T Dg_j (rc_g,j + rp_s,j / sig_j)
     __device__ static double cond_rhs(const X& c, const double* rp, const double* rc, int k, int a, int i) {
         const PbProxy pb;
-        const double* gv = c.v(c.L->gv) + (k - 1) * pb->ng * PD;
+        const int ng = pb->ng;
+        const double* gv = c.vh(c.L->gv) + (k - 1) * ng * PD;
+        const double* dg = c.vh(c.L->dgv) + (k - 1) * ng;
+        const double* Sig = c.v(c.L->Sig) + c.is(k);
         double s = 0.0;
-        for (int j = 0; j < pb->ng; ++j) {
+        for (int j = 0; j < ng; ++j) {
             double sgn = 1.0;
             if (pb->family == JIPM_FAM_MULTIQUAD) {
                 int pa, pb2; c.pair_ab(j, pa, pb2);
                 sgn = (pa == a) ? 1.0 : (pb2 == a ? -1.0 : 0.0);
                 if (sgn == 0.0) continue;
             }
-            const double sig = c.v(c.L->Sig)[c.is(k) + j];
-            s += sgn * gv[j * PD + i] * Dg(c, k, j) * (rc[c.icg(k) + j] + rp[c.is(k) + j] / sig);
+            s += sgn * gv[j * PD + i] * dg[j] * (rc[c.icg(k) + j] + rp[c.is(k) + j] / Sig[j]);
         }
         return s;
     }
@@ -293,16 +283,16 @@ struct Kkt {
                                               bool any_dc) {
         const PbProxy pb;
         const int N = pb->N, lane = c.lane;
-        const double* Dc = c.v(c.L->Dc);
-        const double* Tf = c.v(c.L->T);
-        const double* Kf = c.v(c.L->Kf);
-        const double* Gf = c.v(c.L->Gf);
-        const double* Psi = c.v(c.L->Psi);
-        double* pv = c.v(c.L->pv);    // (N+1) x NX : cr_k, then p_k, then x_k
-        double* wv = c.v(c.L->wv);    // N x NX     : w_k, then sw_k
-        double* qv = c.v(c.L->qv);    // N x NX     : q_k, then e_k
-        double* hv = c.v(c.L->tv);    // N x NU     : h_k, then uo_k, then u_k
-        double* sv = c.v(c.L->sv);    // N x NX     : scratch (st_k, B uo_k, A x_k + B u_k)
+        const double* Dc = c.vh(c.L->Dc);
+        const double* Tf = c.vh(c.L->T);
+        const double* Kf = c.vh(c.L->Kf);
+        const double* Gf = c.vh(c.L->Gf);
+        const double* Psi = c.vh(c.L->Psi);
+        double* pv = c.vh(c.L->pv);    // (N+1) x NX : cr_k, then p_k, then x_k
+        double* wv = c.vh(c.L->wv);    // N x NX     : w_k, then sw_k
+        double* qv = c.vh(c.L->qv);    // N x NX     : q_k, then e_k
+        double* hv = c.vh(c.L->tv);    // N x NU     : h_k, then uo_k, then u_k
+        double* sv = c.vh(c.L->sv);    // N x NX     : scratch (st_k, B uo_k, A x_k + B u_k)
         // ---- phase 0a ----
         for (int e = lane; e < (N + 1) * NX; e += NT) {
             const int k = e / NX, i = e % NX;
@@ -313,24 +303,24 @@ struct Kkt {
         }
         for (int e = lane; e < N * NX; e += NT) {
             const int k = e / NX, i = e % NX;
-            wv[e] = dot4(Tf + (k + 1) * NX * NX + i, NX, rc + c.icd(k + 1), 1, NX);  // T symmetric
+            wv[e] = dotc<NX, NX, 1>(Tf + (k + 1) * NX * NX + i, rc + c.icd(k + 1));  // T symmetric
         }
         c.tm.sync();
         // ---- phase 0b: h_k ----
         for (int e = lane; e < N * NU; e += NT) {
             const int k = e / NU, p = e % NU;
-            hv[e] = rp[c.iu(k) + p] - dot4(c.Jk(k) + NX + p, NZ, wv + k * NX, 1, NX);
+            hv[e] = rp[c.iu(k) + p] - dotc<NX, NZ, 1>(c.Jk(k) + NX + p, wv + k * NX);
         }
         c.tm.sync();
         // ---- phase 0c: q_k ----
         for (int e = lane; e < N * NX; e += NT) {
             const int k = e / NX, i = e % NX;
-            qv[e] = pv[e] - dot4(c.Jk(k) + i, NZ, wv + k * NX, 1, NX) - dot4(Kf + k * NU * NX + i, NX, hv + k * NU, 1, NU);
+            qv[e] = pv[e] - dotc<NX, NZ, 1>(c.Jk(k) + i, wv + k * NX) - dotc<NU, NX, 1>(Kf + k * NU * NX + i, hv + k * NU);
         }
         c.tm.sync();
         // ---- phase 1: backward sweep (threads i < NX; whole-team barrier only if NX spans several warps) ----
         for (int k = N - 1; k >= 0; --k) {
-            if (lane < NX) pv[k * NX + lane] = qv[k * NX + lane] + dot4(Psi + k * NX * NX + lane, NX, pv + (k + 1) * NX, 1, NX);
+            if (lane < NX) pv[k * NX + lane] = qv[k * NX + lane] + dotc<NX, NX, 1>(Psi + k * NX * NX + lane, pv + (k + 1) * NX);
             if (NX <= 32) __syncwarp(); else c.tm.sync();
         }
         c.tm.sync();
@@ -349,23 +339,23 @@ struct Kkt {
         c.tm.sync();
         for (int e = lane; e < N * NU; e += NT) {
             const int k = e / NU, p = e % NU;
-            sv[e] = rp[c.iu(k) + p] - dot4(c.Jk(k) + NX + p, NZ, wv + k * NX, 1, NX);  // st_k (N x NU fits in sv)
+            sv[e] = rp[c.iu(k) + p] - dotc<NX, NZ, 1>(c.Jk(k) + NX + p, wv + k * NX);  // st_k (N x NU fits in sv)
         }
         c.tm.sync();
         for (int e = lane; e < N * NU; e += NT) {
             const int k = e / NU, p = e % NU;
-            hv[e] = dot4(Gf + k * NU * NU + p * NU, 1, sv + k * NU, 1, NU);  // uo_k = G st_k
+            hv[e] = dotc<NU, 1, 1>(Gf + k * NU * NU + p * NU, sv + k * NU);  // uo_k = G st_k
         }
         c.tm.sync();
         for (int e = lane; e < N * NX; e += NT) {
             const int k = e / NX, i = e % NX;
-            sv[e] = dot4(c.Jk(k) + i * NZ + NX, 1, hv + k * NU, 1, NU);  // B uo_k   (st_k is dead)
+            sv[e] = dotc<NU, 1, 1>(c.Jk(k) + i * NZ + NX, hv + k * NU);  // B uo_k   (st_k is dead)
         }
         c.tm.sync();
         for (int e = lane; e < N * NX; e += NT) {
             const int k = e / NX, i = e % NX, r0 = c.icd(k + 1);
             double v = sv[e] + rc[r0 + i];
-            if (any_dc) v -= Dc[r0 + i] * (dot4(Tf + (k + 1) * NX * NX + i, NX, sv + k * NX, 1, NX) + wv[e]);
+            if (any_dc) v -= Dc[r0 + i] * (dotc<NX, NX, 1>(Tf + (k + 1) * NX * NX + i, sv + k * NX) + wv[e]);
             qv[e] = v;  // e_k
         }
         // stage 0: nu_0 = T_0 (rc_0 + D_0 p_0) - p_0, x_0 = rc_0 - D_0 nu_0
@@ -382,7 +372,7 @@ struct Kkt {
         if (NX <= 32) __syncwarp(); else c.tm.sync();
         for (int k = 0; k < N; ++k) {
             if (lane < NX) {
-                const double xn = qv[k * NX + lane] + dot4(Psi + k * NX * NX + lane * NX, 1, pv + k * NX, 1, NX);
+                const double xn = qv[k * NX + lane] + dotc<NX, 1, 1>(Psi + k * NX * NX + lane * NX, pv + k * NX);
                 pv[(k + 1) * NX + lane] = xn;
             }
             if (NX <= 32) __syncwarp(); else c.tm.sync();
@@ -392,27 +382,27 @@ struct Kkt {
         for (int e = lane; e < N * NX; e += NT) dx[c.ix(e / NX + 1) + e % NX] = pv[e + NX];
         for (int e = lane; e < N * NU; e += NT) {
             const int k = e / NU, p = e % NU;
-            const double u = hv[e] - dot4(Kf + k * NU * NX + p * NX, 1, pv + k * NX, 1, NX);
+            const double u = hv[e] - dotc<NX, 1, 1>(Kf + k * NU * NX + p * NX, pv + k * NX);
             hv[e] = u; dx[c.iu(k) + p] = u;
         }
         c.tm.sync();
         for (int e = lane; e < N * NX; e += NT) {
             const int k = e / NX, i = e % NX;
-            sv[e] = dot4(c.Jk(k) + i * NZ, 1, pv + k * NX, 1, NX) + dot4(c.Jk(k) + i * NZ + NX, 1, hv + k * NU, 1, NU);
+            sv[e] = dotc<NX, 1, 1>(c.Jk(k) + i * NZ, pv + k * NX) + dotc<NU, 1, 1>(c.Jk(k) + i * NZ + NX, hv + k * NU);
         }
         c.tm.sync();
         for (int e = lane; e < N * NX; e += NT) {
             const int k = e / NX, i = e % NX;
-            const double nu = wv[e] + dot4(Tf + (k + 1) * NX * NX + i, NX, sv + k * NX, 1, NX);
+            const double nu = wv[e] + dotc<NX, NX, 1>(Tf + (k + 1) * NX * NX + i, sv + k * NX);
             dy[c.icd(k + 1) + i] = -nu;
         }
         // ---- slack / inequality-multiplier recovery ----
-        const double* gv = c.v(c.L->gv);
+        const double* gv = c.vh(c.L->gv);
         for (int it = lane; it < N * pb->ng; it += NT) {
             const int k = it / pb->ng + 1, j = it % pb->ng;
             const double sig = c.v(c.L->Sig)[c.is(k) + j];
             const double rps = rp[c.is(k) + j];
-            const double dyg = Dg(c, k, j) * (c.G_dot(gv, dx, k, j) - rc[c.icg(k) + j] - rps / sig);
+            const double dyg = c.vh(c.L->dgv)[it] * (c.G_dot(gv, dx, k, j) - rc[c.icg(k) + j] - rps / sig);
             dy[c.icg(k) + j] = dyg;
             dx[c.is(k) + j] = (rps + dyg) / sig;
         }

@@ -174,10 +174,11 @@ class Solver:
         return out
 
     def stats(self):
-        a = (C.c_int64 * 8)()
-        _check(lib().jipm_last_stats(self._h, a, 8))
+        a = (C.c_int64 * 16)()
+        _check(lib().jipm_last_stats(self._h, a, 16))
         names = ["iterations", "factorisations", "kkt_solves", "deriv_evals", "fc_evals", "slots", "launches",
-                 "resto_iterations"]
+                 "resto_iterations", "cyc_derivs", "cyc_factor", "cyc_solve", "cyc_residual", "cyc_trial_eval",
+                 "cyc_iterations", "cyc_init", "cyc_spare"]
         return dict(zip(names, list(a)))
 
     # ---- debug / parity entries ------------------------------------------------------------------------
