@@ -166,6 +166,20 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def shard_first_id(rank: int, batch_per_gpu: int) -> int:
+    """Queue sharding over ranks: rank r owns problem ids [r*P, (r+1)*P) (disjoint; no data-path collective)."""
+    return rank * batch_per_gpu
+
+
+def reduce_over_ranks(times, counts, world: int):
+    """Step times: max over ranks; solved / iteration / problem counts: sum over ranks (whole-job aggregate)."""
+    import torch.distributed as dist
+    if world > 1:
+        dist.all_reduce(times, op=dist.ReduceOp.MAX)
+        dist.all_reduce(counts, op=dist.ReduceOp.SUM)
+    return times, counts
+
+
 def run_jipm(args):
     import torch
     import torch.distributed as dist
@@ -181,7 +195,7 @@ def run_jipm(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     cfg = args.config
     P = args.batch or wl.CONFIG_BATCH[cfg]
-    d, theta, x0 = wl.generate(cfg, P, first_id=rank * P)  # queue sharded by rank: disjoint problem ids
+    d, theta, x0 = wl.generate(cfg, P, first_id=shard_first_id(rank, P))  # queue sharded by rank
     xL, xU = wl.bounds(d)
     opts = None
     if args.max_iter > 0:
@@ -253,9 +267,7 @@ def run_jipm(args):
     # ---- reduce over ranks ---------------------------------------------------------------------------------
     red = torch.tensor([dev_ms, e2e_s, t_wall], dtype=torch.float64, device=dev)
     cnt = torch.tensor([solved, e2e_solved, int(iters.sum()), P], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(red, op=dist.ReduceOp.MAX)
-        dist.all_reduce(cnt, op=dist.ReduceOp.SUM)
+    reduce_over_ranks(red, cnt, world)
     dev_ms, e2e_s, t_wall = red.tolist()
     solved_all, e2e_solved_all, iters_all, P_all = cnt.tolist()
     if rank == 0:
@@ -266,6 +278,8 @@ def run_jipm(args):
         cyc_it = max(stats_sum.get("cyc_iterations", 0), 1)
         phase_share = {k[4:]: round(stats_sum[k] / cyc_it, 4) for k in
                        ("cyc_derivs", "cyc_factor", "cyc_solve", "cyc_residual", "cyc_trial_eval")}
+        phase_share.update({"factor/" + k[5:]: round(stats_sum[k] / cyc_it, 4) for k in stats_sum if k.startswith("cycf_")
+                            and stats_sum[k] > 0})
         us_per_iter = cyc_it / max(stats_sum["iterations"], 1) / (clocks["sm_mhz"] or 1965.0) if clocks else None
         my_secs = sum(a.elapsed_time(b) for a, b in ev) * 1e-3
         achieved = flops / my_secs / 1e12
@@ -295,7 +309,7 @@ def run_jipm(args):
                                         "(MEASURED_PEAKS.json has no FP64 entry); nominal 148 SM x 64 DFMA/clk x 2 x "
                                         "1.965 GHz = 37.2",
                          "algorithmic_flops_per_step": flops / K,
-                         "counts_per_step": {k: v / K for k, v in stats_sum.items() if not k.startswith("cyc_")},
+                         "counts_per_step": {k: v / K for k, v in stats_sum.items() if not k.startswith("cyc")},
                          "phase_share_of_iteration_cycles": phase_share,
                          "slot_us_per_iteration": us_per_iter},
             "clocks": clocks,
@@ -313,12 +327,61 @@ def run_jipm(args):
         dist.destroy_process_group()
 
 
+def run_c4(args):
+    """BASELINE.json configs[4]: iteration-level batching sweep.  A queue of seeded problems of the C1 family
+    (reading D-2: 1-based "config-2 problem family") is solved with R = 1024, 4096, 16384, 65536 problem slots.
+    A slot is a CTA: R CTAs are launched, the SMs hold as many as fit (one per SM for this family) and every CTA pops
+    problems until the queue is empty, so a finished problem is replaced at once whatever R is."""
+    import torch
+    from paper_2606_26341_b200 import jipm
+    torch.cuda.set_device(0)
+    P = args.queue
+    d, theta, x0 = wl.generate(1, P)
+    xL, xU = wl.bounds(d)
+    dev = torch.device("cuda", 0)
+    x0_d, th_d = torch.as_tensor(x0, device=dev), torch.as_tensor(theta, device=dev)
+    out = dict(x=torch.empty((P, d.n), dtype=torch.float64, device=dev),
+               lam=torch.empty((P, d.m), dtype=torch.float64, device=dev),
+               status=torch.empty((P,), dtype=torch.int32, device=dev),
+               iters=torch.empty((P,), dtype=torch.int32, device=dev))
+    peak = jipm.fp64_peak_tflops()
+    sm_count = torch.cuda.get_device_properties(0).multi_processor_count
+    sweep, ref_iters = [], None
+    for R in [int(r) for r in args.slots_list.split(",")]:
+        s = jipm.Solver(d.family, d.horizon_N, d.n_agents, d.n_obstacles, d.dt, xL, xU, resident_slots=R)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(); s.solve_batch_into(x0_d, th_d, out); b.record(); torch.cuda.synchronize()
+        ms = a.elapsed_time(b)
+        st = s.stats()
+        iters = out["iters"].cpu().numpy(); status = out["status"].cpu().numpy()
+        if ref_iters is None:
+            ref_iters = iters.copy()
+        busy = (st["cyc_iterations"] + st["cyc_init"]) / 1.965e9
+        pct = np.percentile(iters, [50, 90, 99, 99.9]).tolist()
+        sweep.append({"R": R, "ms": ms, "nlps_per_s": float((status == 0).sum()) / (ms * 1e-3),
+                      "iterations_per_s": float(iters.sum()) / (ms * 1e-3),
+                      "slot_occupancy": busy / (min(R, sm_count) * ms * 1e-3),
+                      "fp64_frac": flops_from_stats(d, st) / (ms * 1e-3) / 1e12 / peak,
+                      "iters_identical_to_first_R": bool(np.array_equal(iters, ref_iters)),
+                      "iters_p50_p90_p99_p999": pct, "iters_max": int(iters.max()),
+                      "status_hist": {int(k): int((status == k).sum()) for k in np.unique(status)}})
+        s.close()
+    best = max(sweep, key=lambda r: r["nlps_per_s"])
+    print(json.dumps({"metric": METRIC, "value": best["nlps_per_s"], "unit": UNIT, "n_gpus": 1, "steps": 1, "warmup": 0,
+                      "ms_per_step": best["ms"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                      "dtype": "f64", "data": "synthetic",
+                      "config": {"workload": f"C4 iteration-level batching sweep, queue {P} problems of the C1 family",
+                                 "co_resident_slots": sm_count}, "sweep": sweep}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 3])
+    ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 3, 4])
+    ap.add_argument("--queue", type=int, default=100000, help="config 4: problems in the queue")
+    ap.add_argument("--slots-list", default="1024,4096,16384,65536", help="config 4: resident slot counts")
     ap.add_argument("--batch", type=int, default=0, help="problems per GPU per step (default: the config's batch)")
     ap.add_argument("--slots", type=int, default=0, help="resident slots (0: library picks)")
     ap.add_argument("--impl", default="jipm", choices=["jipm", "reference"])
@@ -327,7 +390,9 @@ def main():
                     help="cap IPM iterations per problem (profiling runs only: keeps the kernel short under ncu; "
                          "a line produced with this flag says so in config and is not a bench value)")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.config == 4:
+        run_c4(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_jipm(args)

@@ -99,7 +99,8 @@ const char* jipm_last_error(void);
  * stats[0] total IPM iterations, [1] factorisations, [2] KKT solves, [3] derivative evaluations,
  * [4] f/c-only evaluations, [5] slots launched, [6] kernel launches, [7] restoration iterations,
  * [8..14] SM-clock cycles summed over slots spent in: derivative evaluation, factorisations, KKT solves,
- * residuals of (6), trial-point evaluations, whole iterations, Step I (clock64 of each slot's thread 0). */
+ * residuals of (6), trial-point evaluations, whole iterations, Step I (clock64 of each slot's thread 0);
+ * [16..20] the same for the factorisation sub-phases: T J, M assembly, control pivots, Phi + stores, D != 0 extras. */
 int jipm_last_stats(jipm_solver* s, int64_t* stats, int64_t n_stats);
 
 /* ---- debug / parity-test entries (load a state, step once, compare) ------------------

@@ -22,7 +22,8 @@ struct Cfg {
     static constexpr int SM_T = 0, SM_J = SM_T + NX * NX, SM_M = SM_J + NX * NZ, SM_M2 = SM_M + SM_MSZ, SM_TJ = SM_M2 + SM_MSZ;
     static constexpr int SM_K = SM_TJ + NX * NZ, SM_G = SM_K + NU * NX + NU * NU;
     static constexpr int SM_RED = SM_G + (Dyn::AX == 12 ? (NT / 16) * 7 * 16 : 0);
-    static constexpr int SM_TOTAL = SM_RED + 2 * (NT / 32) + 2;
+    static constexpr int SM_SPEC = SM_RED + 2 * (NT / 32) + 2;  // (theta, phi) of the speculative trials, one pair per warp
+    static constexpr int SM_TOTAL = SM_SPEC + 2 * (NT / 32);
 };
 
 template <class C>
@@ -38,9 +39,11 @@ struct Ctx {
     const double* th;  // theta of the current problem
     int lane;          // thread index inside the team, 0 .. NT-1
     mutable Team<NT> tm;
+    mutable unsigned long long pc[8];  // diagnostic cycle counters of the factorisation's sub-phases (stats[16..23])
 
     __device__ Ctx(double* ws_, double* sm_, int tid_, int bar_)
         : ws(ws_ - g_A.L.nsm), sm(sm_), smd(sm_ + C::SM_TOTAL), th(nullptr), lane(tid_) {
+        for (int q = 0; q < 8; ++q) pc[q] = 0;
         tm.tid = tid_; tm.bar = bar_; tm.flip = 0; tm.red = sm_ + C::SM_RED;
     }
 

@@ -130,6 +130,16 @@ struct Solver {
         for (int j = lane; j < nf; j += NT) hit |= (th_t >= F[2 * j] && ph_t >= F[2 * j + 1]);
         return c.tm.any(hit);
     }
+    __device__ bool acceptable_serial(double th_t, double ph_t, double th_k, double ph_k, double alpha, double g) const {
+        if (!(isfinite(th_t) && isfinite(ph_t))) return false;
+        if (th_t >= theta_max) return false;
+        const double* F = filt_active();
+        for (int j = 0; j < nfilt; ++j)
+            if (th_t >= F[2 * j] && ph_t >= F[2 * j + 1]) return false;
+        if (th_k <= theta_min && switching(alpha, g, th_k)) return armijo(ph_t, ph_k, alpha, g);
+        return th_t <= (1.0 - o->gamma_theta) * th_k ||
+               ph_t - ph_k - 10.0 * EPS_MACH * fabs(ph_k) <= -o->gamma_phi * th_k;
+    }
     __device__ bool in_filter(double th_t, double ph_t) const {
         return in_filter_of(filt_active(), nfilt, theta_max, th_t, ph_t);
     }
@@ -298,6 +308,7 @@ struct Solver {
 
     __device__ void init_problem(long long id);
     __device__ void iterate();
+    __device__ void trial_warp(const Vec x, const Vec dx, double alpha, double& th_t, double& ph_t) const;
     __device__ void enter_restoration(double* rec, int kind);
     __device__ void try_exit_restoration();
     __device__ double eval_point(const Vec xt, double* ct, double& th_t, double& cm_t, double& fb, double& thb,

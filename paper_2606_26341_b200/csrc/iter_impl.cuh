@@ -118,6 +118,99 @@ __device__ double Solver<C>::eval_point(const Vec xt, double* ct, double& th_t, 
     return o->rho_resto * fpn + 0.5 * zeta * fq;
 }
 
+// Speculative trial evaluation ("compute the branch-unique work for all, then select"): ONE WARP
+// computes theta = ||c||_1 and phi_mu of the active problem (either mode) at x + alpha dx, nothing is stored and only
+// warp shuffles synchronise, so the NT/32 warps of the team evaluate NT/32 backtracking candidates at once.
+template <class C>
+__device__ void Solver<C>::trial_warp(const Vec x, const Vec dx, double alpha, double& th_t, double& ph_t) const {
+    const int wl = lane & 31;
+    const int N = pb->N, n = pb->n, m = pb->m, ng = pb->ng;
+    const double* xa = x.a; const double* da = dx.a;
+    const double* xt_ = x.t; const double* dt_ = dx.t;
+    const double* th = c.th;
+    const double* tgt = c.vh(L->tgt);
+    auto X = [&](int i) { return xa[i] + alpha * da[i]; };
+    // restoration rows: c_R = (c - p) + n with p, n at the tail entries n + r, n + m + r
+    auto ROW = [&](int r, double v) {
+        if (mode) v = (v - (xt_[n + r] + alpha * dt_[n + r])) + (xt_[n + m + r] + alpha * dt_[n + m + r]);
+        return fabs(v);
+    };
+    double f = 0.0, th1 = 0.0, bar = 0.0;
+    int badpt = 0;
+    if (!mode) {
+        for (int it = wl; it < (N + 1) * NA; it += 32) {
+            const int k = it / NA, a = it % NA, p0 = c.ix(k) + AX * a;
+            double s = 0.0;
+#pragma unroll
+            for (int i = 0; i < PD; ++i) { const double d = X(p0 + i) - tgt[it * PD + i]; s += d * d; }
+            f += s;
+        }
+        for (int it = wl; it < N * NU; it += 32) { const double u = X(c.iu(it / NU) + it % NU); f += pb->ru * (u * u); }
+    } else {
+        const double* xR = V(L->xR); const double* DR2 = V(L->DR2);
+        double sq = 0.0, spn = 0.0;
+        for (int i = wl; i < n; i += 32) { const double d = X(i) - xR[i]; sq += DR2[i] * d * d; }
+        for (int r = wl; r < 2 * m; r += 32) spn += xt_[n + r] + alpha * dt_[n + r];
+        f = o->rho_resto * spn + 0.5 * zeta * sq;
+    }
+    for (int i = wl; i < NX; i += 32) th1 += ROW(i, X(i) - th[i]);
+    for (int it = wl; it < N * NA; it += 32) {
+        const int k = it / NA, a = it % NA;
+        double xs[AX], us[C::AU], Fv[AX];
+#pragma unroll
+        for (int i = 0; i < AX; ++i) xs[i] = X(c.ix(k) + AX * a + i);
+#pragma unroll
+        for (int i = 0; i < C::AU; ++i) us[i] = X(c.iu(k) + C::AU * a + i);
+        C::Dyn::F(xs, us, pb->dt, Fv);
+#pragma unroll
+        for (int i = 0; i < AX; ++i) th1 += ROW(c.icd(k + 1) + AX * a + i, X(c.ix(k + 1) + AX * a + i) - Fv[i]);
+    }
+    for (int it = wl; it < N * ng; it += 32) {
+        const int k = it / ng + 1, j = it % ng;
+        double s = 0.0;
+        if (pb->family == JIPM_FAM_MULTIQUAD) {
+            int a, b; c.pair_ab(j, a, b);
+#pragma unroll
+            for (int i = 0; i < PD; ++i) { const double d = X(c.ix(k) + AX * a + i) - X(c.ix(k) + AX * b + i); s += d * d; }
+            s -= 0.25;
+        } else {
+            const double* ob = th + pb->th_obs + (PD + 1) * j;
+#pragma unroll
+            for (int i = 0; i < PD; ++i) { const double d = X(c.ix(k) + i) - ob[i]; s += d * d; }
+            s -= ob[PD] * ob[PD];
+        }
+        th1 += ROW(c.icg(k) + j, s - X(c.is(k) + j));
+    }
+    // barrier terms of (3) with the one-sided damping, as in phi()
+    for (int i = wl; i < nX; i += 32) {
+        const double l = lo(i), u = hi(i);
+        const bool hl = l > -INFINITY, hu = u < INFINITY;
+        if (!hl && !hu) continue;
+        const double xi = (i < n) ? X(i) : xt_[i] + alpha * dt_[i];
+        if (hl) {
+            const double sl = xi - l;
+            if (!(sl > 0.0)) badpt = 1;
+            bar -= mu * log(sl);
+            if (!hu) bar += o->kappa_d * mu * sl;
+        }
+        if (hu) {
+            const double su = u - xi;
+            if (!(su > 0.0)) badpt = 1;
+            bar -= mu * log(su);
+            if (!hl) bar += o->kappa_d * mu * su;
+        }
+    }
+#pragma unroll
+    for (int s = 16; s; s >>= 1) {
+        f += __shfl_xor_sync(FULL, f, s);
+        th1 += __shfl_xor_sync(FULL, th1, s);
+        bar += __shfl_xor_sync(FULL, bar, s);
+        badpt |= __shfl_xor_sync(FULL, badpt, s);
+    }
+    th_t = th1;
+    ph_t = badpt ? NAN : f + bar;
+}
+
 // Restoration entry (Table I row 6; Step R of SURVEY.md 8(c), [7] sec 3.3).  The restoration
 // problem  min rho e^T(p+n) + zeta/2 ||D_R(x-x_R)||^2  s.t. c(x) - p + n = 0, p, n >= 0, x_L <= x <= x_U  is iterated
 // by the SAME iterate() with mode = 1 (same KKT sparsity after eliminating p, n: that is what lets it fuse).
@@ -213,7 +306,8 @@ __device__ void Solver<C>::iterate() {
     // A-1 derivatives at (x, y): sigma_f = 0 in restoration mode (its objective is rho e^T(p+n) + zeta/2 ||D_R(x-x_R)||^2)
     const long long t_it = clock64();
     c.eval_derivs(x, y, mode ? 0.0 : 1.0);
-    tph[0] += clock64() - t_it;
+    const long long t_hd = clock64();
+    tph[0] += t_hd - t_it;
     n_deriv++;
     if (mode) {
         const double* xR = V(L->xR); const double* DR2 = V(L->DR2);
@@ -274,6 +368,7 @@ __device__ void Solver<C>::iterate() {
     bool ic_ok;
     set_sigma(0.0, 0.0);
     long long t_f = clock64();
+    c.pc[7] += t_f - t_hd;
     int bad = K::factor(c, nzero, mode != 0, true); nfact++;  // IC-1
     ic_ok = (bad == 0);
     if (!ic_ok) {
@@ -305,7 +400,9 @@ __device__ void Solver<C>::iterate() {
     }
     for (int i = lane; i < m; i += NT) b2[i] = -cv[i];
     c.tm.sync();
+    const long long t_sf = clock64();
     const int nref = solve_full(b1, b2, b3, b4, dx, dy, dzL, dzU);
+    c.pc[5] += clock64() - t_sf;
     rec[4] = nref;
     // A-5 filter line search
     double gd_part = 0.0;
@@ -330,6 +427,7 @@ __device__ void Solver<C>::iterate() {
                                      o->delta * pow(theta_k, o->s_theta) / pow(-gd, o->s_phi));
     else if (gd < 0.0) a_min = o->gamma_alpha * fmin(o->gamma_theta, o->gamma_phi * theta_k / (-gd));
     else a_min = o->gamma_alpha * o->gamma_theta;
+    const long long t_ls = clock64();
     Vec xt = VX(L->xt); double* ct = VH(L->ct);
     double alpha = a_max, alpha_acc = 0.0, phi_acc = 0.0, f_acc = 0.0, th_acc = 0.0, cm_acc = 0.0;
     double fb_acc = 0.0, thb_acc = 0.0, cmb_acc = 0.0, fpn_acc = 0.0, fq_acc = 0.0;
@@ -378,8 +476,37 @@ __device__ void Solver<C>::iterate() {
         alpha *= o->alpha_red;
         ntrial++;
         if (alpha < a_min || ntrial > o->max_backtrack) break;
+        if constexpr (NT >= 64) {
+            // Speculative backtracking: warp w evaluates the candidate alpha * alpha_red^w; the candidates
+            // are then scanned in the sequential order with the sequential termination rule, so the decision is the one
+            // of Step A-5.  The first acceptable candidate is re-evaluated by the regular path at the top of the loop
+            // (it fills c, f and confirms the test); rejected ones only advance alpha and the trial counter.
+            constexpr int NWP = NT / 32;
+            double* spec = c.smt(C::SM_SPEC);
+            bool exhausted = false, found = false;
+            const long long t_sp = clock64();
+            while (!found && !exhausted) {
+                double aw = alpha;
+                for (int w = 0; w < (lane >> 5); ++w) aw *= o->alpha_red;
+                double th_w, ph_w;
+                trial_warp(x, dx, aw, th_w, ph_w);
+                if ((lane & 31) == 0) { spec[2 * (lane >> 5)] = th_w; spec[2 * (lane >> 5) + 1] = ph_w; }
+                c.tm.sync();
+                for (int w = 0; w < NWP; ++w) {
+                    if (acceptable_serial(spec[2 * w], spec[2 * w + 1], theta_k, phi_k, alpha, gd)) { found = true; break; }
+                    n_fc++;
+                    alpha *= o->alpha_red;
+                    ntrial++;
+                    if (alpha < a_min || ntrial > o->max_backtrack) { exhausted = true; break; }
+                }
+                c.tm.sync();
+            }
+            tph[7] += clock64() - t_sp;
+            if (exhausted) break;
+        }
     }
     rec[6] = ntrial; rec[7] = nsoc;
+    c.pc[6] += clock64() - t_ls;
     if (acc < 0) { enter_restoration(rec, KIND_LS_FAIL); trace_put(rec); return; }
     // A-6 accept, A-7 filter augmentation
     const Vec ax = (acc == 1) ? VX(L->sx) : dx;

@@ -36,7 +36,7 @@ struct jipm_solver {
     unsigned long long* d_stats = nullptr;
     double* trace = nullptr;
     int trace_cap = 0;
-    long long stats[16] = {0};
+    long long stats[24] = {0};
     DbgLay dbg;
 };
 
@@ -101,7 +101,7 @@ static int build_layout(jipm_solver* s, int sm_budget_doubles) {
         // the factor and what every solve streams through
         {&Lay::Psi, N * NX * NX}, {&Lay::pv, (N + 1) * NX}, {&Lay::qv, N * NX}, {&Lay::wv, N * NX}, {&Lay::sv, N * NX}, {&Lay::tv, N * NU},
         {&Lay::T, (N + 1) * NX * NX}, {&Lay::Kf, N * NU * NX}, {&Lay::Gf, N * NU * NU},
-        {&Lay::J, N * NX * NZ}, {&Lay::Dc, m}, {&Lay::gv, N * pb.ng * pd}, {&Lay::dgv, N * pb.ng}, {&Lay::tgt, (N + 1) * pb.na * pd},
+        {&Lay::J, N * NX * NZ}, {&Lay::Dc, m}, {&Lay::gv, N * pb.ng * pd}, {&Lay::dgv, N * pb.ng}, {&Lay::cnd, N * pb.na * pd * pb.na * pd}, {&Lay::tgt, (N + 1) * pb.na * pd},
         {&Lay::bl, n}, {&Lay::bu, n},
         {&Lay::filt, 2 * MAX_FILTER},
         // m-vectors
@@ -208,7 +208,7 @@ extern "C" int jipm_create(jipm_solver** out, int family, const jipm_family_dims
         (e = cudaMalloc(&s->d_xU, n * sizeof(double))) != cudaSuccess ||
         (e = cudaMalloc(&s->d_ws, (size_t)s->n_slots * (s->L.total - s->L.nsm + 2) * sizeof(double))) != cudaSuccess ||
         (e = cudaMalloc(&s->d_queue, sizeof(int))) != cudaSuccess ||
-        (e = cudaMalloc(&s->d_stats, 16 * sizeof(unsigned long long))) != cudaSuccess) {
+        (e = cudaMalloc(&s->d_stats, 24 * sizeof(unsigned long long))) != cudaSuccess) {
         std::string msg = std::string("cudaMalloc: ") + cudaGetErrorString(e);
         jipm_destroy(s);
         return fail(JIPM_ERR_NOMEM, msg);
@@ -240,12 +240,12 @@ static int run(jipm_solver* s, Args& a) {
     a.trace = s->trace; a.trace_cap = s->trace_cap;
     a.dbg_len = s->dbg.len;
     CUDA_TRY(cudaMemsetAsync(s->d_queue, 0, sizeof(int), s->stream));
-    CUDA_TRY(cudaMemsetAsync(s->d_stats, 0, 16 * sizeof(unsigned long long), s->stream));
+    CUDA_TRY(cudaMemsetAsync(s->d_stats, 0, 24 * sizeof(unsigned long long), s->stream));
     CUDA_TRY(dispatch(s, a));
-    unsigned long long st[16];
+    unsigned long long st[24];
     CUDA_TRY(cudaMemcpyAsync(st, s->d_stats, sizeof(st), cudaMemcpyDeviceToHost, s->stream));
     CUDA_TRY(cudaStreamSynchronize(s->stream));
-    for (int i = 0; i < 16; ++i) s->stats[i] = (long long)st[i];
+    for (int i = 0; i < 24; ++i) s->stats[i] = (long long)st[i];
     s->stats[5] = a.n_slots; s->stats[6] = 1;
     return JIPM_OK;
 }
@@ -298,7 +298,7 @@ extern "C" int jipm_solve_batch_host(jipm_solver* s, int64_t P, const double* x0
 
 extern "C" int jipm_last_stats(jipm_solver* s, int64_t* stats, int64_t n_stats) {
     if (!s || !stats) return fail(JIPM_ERR_ARG, "NULL argument");
-    for (int64_t i = 0; i < n_stats && i < 16; ++i) stats[i] = s->stats[i];
+    for (int64_t i = 0; i < n_stats && i < 24; ++i) stats[i] = s->stats[i];
     return JIPM_OK;
 }
 

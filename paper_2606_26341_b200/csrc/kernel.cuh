@@ -106,6 +106,7 @@ __global__ void __launch_bounds__(C::NT, MINB) jipm_slot_kernel() {
         atomicAdd(&A->stats[4], (unsigned long long)S.n_fc);
         atomicAdd(&A->stats[7], (unsigned long long)S.n_resto);
         for (int i = 0; i < 8; ++i) atomicAdd(&A->stats[8 + i], S.tph[i]);
+        for (int i = 0; i < 8; ++i) atomicAdd(&A->stats[16 + i], ctx.pc[i]);
     }
 }
 

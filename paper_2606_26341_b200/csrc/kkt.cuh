@@ -121,12 +121,22 @@ struct Kkt {
         const bool j_in_sm = c.L->J < c.L->nsm;
         int bad = 0;
         nzero = 0;
-        // weights of the condensed (slack, multiplier) pairs, once per factorisation (the solves reuse them)
+        // weights of the condensed (slack, multiplier) pairs and their position-block sums G^T Dg G for every stage,
+        // once per factorisation and stage-parallel (the solves reuse the weights)
+        constexpr int NPOS = NA * PD;
+        double* cnd = c.vh(c.L->cnd);
         for (int it = lane; it < N * ng; it += NT) {
             const int k = it / ng + 1, j = it % ng;
             dgv[it] = 1.0 / (1.0 / Sig[c.is(k) + j] + Dc[c.icg(k) + j]);
         }
         c.tm.sync();
+        if (ng > 0) {
+            for (int it = lane; it < N * NPOS * NPOS; it += NT) {
+                const int k = it / (NPOS * NPOS) + 1, e = it % (NPOS * NPOS), r = e / NPOS, q = e % NPOS;
+                cnd[it] = cond_entry(c, gvv, dgv, k, AX * (r / PD) + r % PD, AX * (q / PD) + q % PD);
+            }
+            c.tm.sync();
+        }
         // terminal block
         {
             const double* WN = c.Wk(N);
@@ -134,7 +144,7 @@ struct Kkt {
             for (int e = lane; e < NX * NX; e += NT) {
                 const int r = e / NX, q = e % NX;
                 double v = (useW ? WN[e] : 0.0) + (r == q ? Sig[c.ix(N) + r] : 0.0);
-                if (ng > 0) v += cond_entry(c, gvv, dgv, N, r, q);
+                if (ng > 0 && r % AX < PD && q % AX < PD) v += cnd[(N - 1) * NPOS * NPOS + (PD * (r / AX) + r % AX) * NPOS + PD * (q / AX) + q % AX];
                 sT[e] = v;
                 if (!any_dc) TN[e] = v;
             }
@@ -146,6 +156,7 @@ struct Kkt {
             }
         }
         for (int k = N - 1; k >= 0; --k) {
+            long long tq = clock64();
             const double* sJ = c.Jk(k);
             if (!j_in_sm) {
                 for (int e = lane; e < NX * NZ; e += NT) sJc[e] = sJ[e];
@@ -158,6 +169,7 @@ struct Kkt {
                 sTJ[e] = dotc<NX, 1, NZ>(sT + l * NX, sJ + j);
             }
             c.tm.sync();
+            { const long long t2 = clock64(); c.pc[0] += t2 - tq; tq = t2; }
             // M = Q_k + J^T (T J) + condensed slacks
             const double* Wg = c.Wk(k);
             for (int e = lane; e < NZ * NZ; e += NT) {
@@ -165,10 +177,12 @@ struct Kkt {
                 double m = dotc<NX, NZ, NZ>(sJ + a, sTJ + j);
                 if (useW) m += Wg[e];
                 if (a == j) m += Sig[c.zidx(k, j)];
-                if (k >= 1 && ng > 0 && a < NX && j < NX) m += cond_entry(c, gvv, dgv, k, a, j);
+                if (k >= 1 && ng > 0 && a < NX && j < NX && a % AX < PD && j % AX < PD)
+                    m += cnd[(k - 1) * NPOS * NPOS + (PD * (a / AX) + a % AX) * NPOS + PD * (j / AX) + j % AX];
                 tA[e] = m;
             }
             c.tm.sync();
+            { const long long t2 = clock64(); c.pc[1] += t2 - tq; tq = t2; }
             // Gauss-Jordan pivots on the controls NX .. NZ-1: every element from the previous tile, no races
             double* src = tA; double* dst = tB;
             for (int p = 0; p < NU; ++p) {
@@ -188,6 +202,7 @@ struct Kkt {
                 c.tm.sync();
                 double* t = src; src = dst; dst = t;
             }
+            { const long long t2 = clock64(); c.pc[2] += t2 - tq; tq = t2; }
             // src: [[P_k, -Kf^T], [Kf, G]].  Phi = A - B Kf; stores
             double* Kg = c.vh(c.L->Kf) + k * NU * NX;
             double* Gg = c.vh(c.L->Gf) + k * NU * NU;
@@ -206,6 +221,7 @@ struct Kkt {
             for (int e = lane; e < NU * NX; e += NT) Kg[e] = src[(NX + e / NX) * NZ + e % NX];
             for (int e = lane; e < NU * NU; e += NT) Gg[e] = src[(NX + e / NU) * NZ + NX + e % NU];
             c.tm.sync();
+            { const long long t2 = clock64(); c.pc[3] += t2 - tq; tq = t2; }
             if (any_dc) {
                 // Psi = (I - D_{k+1} T_{k+1}) Phi, then P_k -> T_k = (I + P_k D_k)^{-1} P_k
                 const int r0 = c.icd(k + 1);
@@ -222,6 +238,7 @@ struct Kkt {
                 bad += transform_T(c, sT, dst, c.icd(k), true);
                 for (int e = lane; e < NX * NX; e += NT) Tg[e] = sT[e];
                 c.tm.sync();
+                c.pc[4] += clock64() - tq;
             }
         }
         return bad;

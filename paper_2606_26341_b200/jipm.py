@@ -174,11 +174,12 @@ class Solver:
         return out
 
     def stats(self):
-        a = (C.c_int64 * 16)()
-        _check(lib().jipm_last_stats(self._h, a, 16))
+        a = (C.c_int64 * 24)()
+        _check(lib().jipm_last_stats(self._h, a, 24))
         names = ["iterations", "factorisations", "kkt_solves", "deriv_evals", "fc_evals", "slots", "launches",
                  "resto_iterations", "cyc_derivs", "cyc_factor", "cyc_solve", "cyc_residual", "cyc_trial_eval",
-                 "cyc_iterations", "cyc_init", "cyc_spare"]
+                 "cyc_iterations", "cyc_init", "cyc_speculative_trials",
+                 "cycf_TJ", "cycf_M", "cycf_pivots", "cycf_phi_store", "cycf_dc_extra", "cycx_solve_full_first", "cycx_line_search", "cycx_iteration_head"]
         return dict(zip(names, list(a)))
 
     # ---- debug / parity entries ------------------------------------------------------------------------

@@ -150,6 +150,50 @@ def test_init_and_first_steps_state_parity(cfg):
     print(f"cfg {cfg}: worst KKT step residual {worst_res:.2e}, worst e_v {worst_ev:.2e}")
 
 
+@pytest.mark.parametrize("cfg", [2, 3])
+def test_full_size_c2_c3_first_iterations(cfg):
+    """BASELINE.json configs[2] (4 quadrotors, n=1448, m=1128) and configs[3] (clutter, n=1452, m=1332) at their FULL
+    dimensions, in the instantiation bench.py would launch: Step I and the first iterations of two problems against the
+    oracle (dense 2576 / 2784-row KKT): KKT step residual <= 1e-10 from the oracle's W, A; next iterate e_v <= 1e-8."""
+    import torch
+    d = wl.config_dims(cfg)
+    P = 2
+    d, theta, x0 = wl.generate(cfg, P, d)
+    s, xL, xU = make_solver(d)
+    lay = s.state_layout()
+    prob, osol = par.oracle_for(d, xL, xU)
+    n, m = d.n, d.m
+    state = s.debug_init(x0, theta)
+    sts = [osol.initialise(x0[i], theta[i]) for i in range(P)]
+    h = state.cpu().numpy()
+    for i in range(P):
+        assert par.e_v(h[i, lay["x"]:lay["x"] + n], sts[i].x) <= 1e-12
+        assert par.e_v(h[i, lay["y"]:lay["y"] + m], sts[i].y) <= Y_PARITY_TOL
+    for it in range(3):
+        before = state.clone().cpu().numpy()
+        s.debug_step(theta, state, 1)
+        torch.cuda.synchronize()
+        after = state.cpu().numpy()
+        tr_g = None
+        for i in range(P):
+            if sts[i].status != -1 or sts[i].resto is not None:
+                continue
+            xb, yb = before[i, lay["x"]:lay["x"] + n], before[i, lay["y"]:lay["y"] + m]
+            zLb, zUb = before[i, lay["zL"]:lay["zL"] + n], before[i, lay["zU"]:lay["zU"] + n]
+            tr = osol.iterate(sts[i], theta[i])
+            if tr["kind"] not in ("newton", "soc"):
+                continue
+            step = (after[i, lay["dx"]:lay["dx"] + n], after[i, lay["dy"]:lay["dy"] + m],
+                    after[i, lay["dzL"]:lay["dzL"] + n], after[i, lay["dzU"]:lay["dzU"] + n])
+            res = par.full_system_residual(prob, osol, xb, yb, zLb, zUb, theta[i], after[i, lay["sc"]], tr["dw"], tr["dc"], step)
+            assert res <= STEP_RESIDUAL_TOL, (cfg, it, i, res)
+            for name, ref in (("x", sts[i].x), ("y", sts[i].y), ("zL", sts[i].zL), ("zU", sts[i].zU)):
+                ln = n if name != "y" else m
+                ev = par.e_v(after[i, lay[name]:lay[name] + ln], ref)
+                assert ev <= (STEP_PARITY_TOL if name != "y" else Y_PARITY_TOL), (cfg, it, i, name, ev)
+    s.close()
+
+
 def prune_filter(filt):
     """Drop entries dominated by a later one (decision-neutral, reading S-10) so that the oracle's unbounded list
     fits the GPU filter capacity (128)."""
