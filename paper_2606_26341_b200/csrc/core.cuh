@@ -125,7 +125,7 @@ struct Ctx {
 
     // ---- f, c at a point (line-search trial evaluation) --------------------------------
     // returns f; writes c[m]; theta = ||c||_1, cmax = ||c||_inf; fin = all finite
-    __device__ double eval_fc(const double* x, double* c, double& theta, double& cmax, bool& fin) const {
+    __device__ __noinline__ double eval_fc(const double* x, double* c, double& theta, double& cmax, bool& fin) const {
         const int N = pb->N;
         double f = 0.0;
         const double* tgt = vh(L->tgt);
@@ -246,7 +246,7 @@ struct Ctx {
         return s;
     }
 
-    __device__ void eval_derivs(const double* x, const double* y, double sigma_f);
+    __device__ __noinline__ void eval_derivs(const double* x, const double* y, double sigma_f);
     __device__ void dyn_derivs(const double* x, const double* y);
 };
 

@@ -61,7 +61,7 @@ struct Solver {
     __device__ __forceinline__ double* filt_active() const { return V(mode ? L->filtR : L->filt); }
 
     // barrier objective (3) with the one-sided damping term; NaN outside the interior
-    __device__ double phi(const Vec x, double fv, double mu_, int nvar) const {
+    __device__ __noinline__ double phi(const Vec x, double fv, double mu_, int nvar) const {
         double s = 0.0;
         int badpt = 0;
         for (int i = lane; i < nvar; i += NT) {
@@ -276,7 +276,7 @@ struct Solver {
     }
 
     // solve (6) with iterative refinement on the unreduced system (reading S-7); returns #refinements
-    __device__ int solve_full(const Vec b1, const double* b2, const Vec b3, const Vec b4,
+    __device__ __noinline__ int solve_full(const Vec b1, const double* b2, const Vec b3, const Vec b4,
                               Vec d1, double* d2, Vec d3, Vec d4) {
         reduced_solve(b1, b2, b3, b4, d1, d2, d3, d4);
         double bn = 0.0;
@@ -308,10 +308,10 @@ struct Solver {
 
     __device__ void init_problem(long long id);
     __device__ void iterate();
-    __device__ void trial_warp(const Vec x, const Vec dx, double alpha, double& th_t, double& ph_t) const;
+    __device__ __noinline__ void trial_warp(const Vec x, const Vec dx, double alpha, double& th_t, double& ph_t) const;
     __device__ void enter_restoration(double* rec, int kind);
     __device__ void try_exit_restoration();
-    __device__ double eval_point(const Vec xt, double* ct, double& th_t, double& cm_t, double& fb, double& thb,
+    __device__ __noinline__ double eval_point(const Vec xt, double* ct, double& th_t, double& cm_t, double& fb, double& thb,
                                  double& cmb, double& fpn, double& fq);
     __device__ void write_outputs();
     __device__ void dbg_load(const double* st);

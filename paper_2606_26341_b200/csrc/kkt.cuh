@@ -47,56 +47,44 @@ struct Kkt {
     }
 
     // T <- (I + P D)^{-1} P in place on the NX x NX tile sT (symmetric), D = Dc at rows [row0, row0+NX).
-    // Returns the number of non-positive pivots of I + E P E (0 when D == 0).  Uses sM (>= 2 NX^2) as scratch.
+    // I + P D = E^{-1} (I + E P E) E with E = sqrt(D): the same leading minors, hence the same unpivoted pivots as the
+    // symmetric I + E P E whose inertia the test needs.  Gauss-Jordan inversion, ping-pong between the two halves of
+    // sM (>= 2 NX^2): one barrier per pivot.  Returns the number of non-positive pivots.
     __device__ static int transform_T(const X& c, double* sT, double* sM, int row0, bool any_dc) {
         if (!any_dc) return 0;
         const double* Dc = c.vh(c.L->Dc) + row0;
-        // G = I + E P E (NX x NX), E = sqrt(D); solve G Z = E P by an unpivoted LDL^T of G, then T = P - (P E) Z
-        double* G = sM;
-        double* Z = sM + NX * NX;
+        double* src = sM;
+        double* dst = sM + NX * NX;
         for (int e = c.lane; e < NX * NX; e += NT) {
             const int r = e / NX, q = e % NX;
-            const double er = sqrt(Dc[r]), eq = sqrt(Dc[q]);
-            G[e] = er * sT[e] * eq + (r == q ? 1.0 : 0.0);
-            Z[e] = er * sT[e];
+            src[e] = sT[e] * Dc[q] + (r == q ? 1.0 : 0.0);
         }
         c.tm.sync();
         int bad = 0;
-        // elimination: thread <-> element (r, q) of [G | Z], rows r > p
         for (int p = 0; p < NX; ++p) {
-            double d = G[p * NX + p];
+            double d = src[p * NX + p];
             if (!(d > 0.0)) { bad++; if (d == 0.0) d = 1.0; }
             const double id = 1.0 / d;
-            for (int e = c.lane; e < (NX - 1 - p) * (2 * NX); e += NT) {
-                const int r = p + 1 + e / (2 * NX), q = e % (2 * NX);
-                if (q < NX) { if (q > p) G[r * NX + q] -= G[r * NX + p] * (G[p * NX + q] * id); }
-                else Z[r * NX + q - NX] -= G[r * NX + p] * (Z[p * NX + q - NX] * id);
+            for (int e = c.lane; e < NX * NX; e += NT) {
+                const int a = e / NX, b = e % NX;
+                const double rb = src[p * NX + b] * id, ca = src[a * NX + p];
+                double v;
+                if (a == p) v = (b == p) ? id : rb;
+                else if (b == p) v = -ca * id;
+                else v = src[e] - ca * rb;
+                dst[e] = v;
             }
             c.tm.sync();
+            double* t = src; src = dst; dst = t;
         }
-        // Z <- L^{-T} D^{-1} Z (rows from the bottom; thread <-> column q); L[r][p] = G[r][p] / d_p
-        for (int p = NX - 1; p >= 0; --p) {
-            double d = G[p * NX + p];
-            if (d == 0.0) d = 1.0;
-            const double id = 1.0 / d;
-            for (int q = c.lane; q < NX; q += NT) {
-                double v = Z[p * NX + q];
-                for (int r = p + 1; r < NX; ++r) v -= G[r * NX + p] * Z[r * NX + q];
-                Z[p * NX + q] = v * id;
-            }
-            c.tm.sync();
-        }
-        // T = P - (P E) Z, (P E)[i][l] = P[i][l] e_l ; into G first (P is still being read), then symmetrised
-        for (int e = c.lane; e < NX * NX; e += NT) Z[e] *= sqrt(Dc[e / NX]);
-        c.tm.sync();
         for (int e = c.lane; e < NX * NX; e += NT) {
             const int i = e / NX, q = e % NX;
-            G[e] = sT[e] - dotc<NX, NX, NX>(sT + i, Z + q);  // sum_l P[l][i] (e_l Z[l][q])   (P symmetric)
+            dst[e] = dotc<NX, 1, NX>(src + i * NX, sT + q);
         }
         c.tm.sync();
         for (int e = c.lane; e < NX * NX; e += NT) {
             const int r = e / NX, q = e % NX;
-            sT[e] = 0.5 * (G[e] + G[q * NX + r]);
+            sT[e] = 0.5 * (dst[e] + dst[q * NX + r]);
         }
         c.tm.sync();
         return bad;
