@@ -137,6 +137,10 @@ def time_oracle(cfg: int, first: int, count: int, cores: int):
     return dt, sum(1 for s, _ in res if s == 0), sum(k for _, k in res)
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE slot-kernel launch over the config's full batch, from the
+# `ncu --set full` capture summarised in profiles/r1_ncu_full_c1.md (25.3 MB + 406.1 MB)
+NCU_TRAFFIC_BYTES = {1: 431.4e6}
+
 ORACLE_SAMPLE = {0: 256, 1: 16, 2: 2, 3: 2}  # problems per timed sample (about 10-30 s of CPU work)
 
 
@@ -303,7 +307,11 @@ def run_jipm(args):
                     "d2h_bytes_per_step": d2h},
             "gpu_launches": int(stats_sum["launches"]),
             "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_fp64, "unit": "TFLOP/s",
-                         "frac": achieved / peak_fp64, "traffic": None,
+                         "frac": achieved / peak_fp64,
+                         "traffic": (NCU_TRAFFIC_BYTES.get(cfg) if P == wl.CONFIG_BATCH[cfg] and args.max_iter == 0
+                                     else None),
+                         "traffic_unit": "bytes of DRAM traffic per launch (ncu); algorithmic bytes per launch = "
+                                         + str(h2d + d2h),
                          "kernel": "jipm_slot_kernel (persistent, one launch per step)",
                          "peak_source": "DFMA microbenchmark jipm_bench_fp64_peak measured in this run "
                                         "(MEASURED_PEAKS.json has no FP64 entry); nominal 148 SM x 64 DFMA/clk x 2 x "
