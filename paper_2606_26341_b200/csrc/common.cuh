@@ -30,7 +30,7 @@ struct Pb {
 
 // offsets (in doubles) into the per-warp workspace
 struct Lay {
-    int x, y, zL, zU, g, c, gv, dgv, cnd, tgt, J, W, Sig, Hd, Dc, T, Kf, Gf, Psi, pv, qv, sv, wv, tv, bl, bu;
+    int x, y, zL, zU, g, c, gv, dgv, cnd, tgt, J, W, Sig, Hd, Dc, T, Kf, Gf, Psi, pv, qv, sv, wv, tv, bl, bu, imap, cmap;
     int b1, b2, b3, b4, dx, dy, dzL, dzU, r1, r2, r3, r4, e1, e2, e3, e4;
     int sx, sy, szL, szU, xt, ct, csoc, bs2, rr, rk, filt, total;
     int pv0, npad, tail0, tpad;  // primal-sized vectors: contiguous block of npad-strided heads, 2m-tails (restoration) apart

@@ -39,12 +39,43 @@ struct Ctx {
     const double* th;  // theta of the current problem
     int lane;          // thread index inside the team, 0 .. NT-1
     mutable Team<NT> tm;
+    // index maps built once per kernel (no runtime integer division in the hot loops):
+    //   imap[i] of primal entry i: (k << 16) | (j << 8) | a   a < NZ: entry a of z_k = (x_k, u_k); a = 255: slack j of knot k
+    //   cmap[r] of equality row r: (k << 16) | (j << 8) | rr  rr < NX: row rr of dyn_{k+1}; 255: inequality j of knot k; 254: x_0 row
+    const int* imap; const int* cmap;
     mutable unsigned long long pc[8];  // diagnostic cycle counters of the factorisation's sub-phases (stats[16..23])
 
     __device__ Ctx(double* ws_, double* sm_, int tid_, int bar_)
         : ws(ws_ - g_A.L.nsm), sm(sm_), smd(sm_ + C::SM_TOTAL), th(nullptr), lane(tid_) {
         for (int q = 0; q < 8; ++q) pc[q] = 0;
         tm.tid = tid_; tm.bar = bar_; tm.flip = 0; tm.red = sm_ + C::SM_RED;
+    }
+
+    __device__ void build_maps() {
+        int* im = reinterpret_cast<int*>(vh(L->imap));
+        int* cm = reinterpret_cast<int*>(vh(L->cmap));
+        for (int idx = lane; idx < pb->n; idx += NT) {
+            int v;
+            if (idx < NX) v = idx;
+            else {
+                const int q = idx - NX, kk = q / pb->blk, r = q % pb->blk;
+                if (r < NU) v = (kk << 16) | (NX + r);
+                else if (r < NU + NX) v = ((kk + 1) << 16) | (r - NU);
+                else v = ((kk + 1) << 16) | ((r - NU - NX) << 8) | 255;
+            }
+            im[idx] = v;
+        }
+        for (int r = lane; r < pb->m; r += NT) {
+            int v;
+            if (r < NX) v = 254;
+            else {
+                const int q = r - NX, k = q / pb->cblk, rr = q % pb->cblk;
+                v = (rr < NX) ? ((k << 16) | rr) : (((k + 1) << 16) | ((rr - NX) << 8) | 255);
+            }
+            cm[r] = v;
+        }
+        imap = im; cmap = cm;
+        tm.sync();
     }
 
     // ---- stage-order index helpers (same layout as include/jipm.h) -----------------------------------
@@ -178,21 +209,19 @@ struct Ctx {
         const double* gv = vh(L->gv);
         for (int r = lane; r < pb->m; r += NT) {
             double s;
-            if (r < NX) s = d[r];
-            else {
-                const int q = r - NX, k = q / pb->cblk, rr = q % pb->cblk;
-                if (rr < NX) {
-                    const double* Jr = Jk(k) + rr * NZ;
-                    s = d[ix(k + 1) + rr];
-                    const double* dxk = d + ix(k); const double* duk = d + iu(k);
+            const int cmv = cmap[r], rr = cmv & 255, k = cmv >> 16;
+            if (rr == 254) s = d[r];
+            else if (rr < NX) {
+                const double* Jr = Jk(k) + rr * NZ;
+                s = d[ix(k + 1) + rr];
+                const double* dxk = d + ix(k); const double* duk = d + iu(k);
 #pragma unroll 4
-                    for (int a = 0; a < NX; ++a) s -= Jr[a] * dxk[a];
+                for (int a = 0; a < NX; ++a) s -= Jr[a] * dxk[a];
 #pragma unroll 4
-                    for (int a = 0; a < NU; ++a) s -= Jr[NX + a] * duk[a];
-                } else {
-                    const int j = rr - NX;
-                    s = G_dot(gv, d, k + 1, j) - d[is(k + 1) + j];
-                }
+                for (int a = 0; a < NU; ++a) s -= Jr[NX + a] * duk[a];
+            } else {
+                const int j = (cmv >> 8) & 255;
+                s = G_dot(gv, d, k, j) - d[is(k) + j];
             }
             out[r] = s;
         }
@@ -200,14 +229,8 @@ struct Ctx {
     }
     __device__ double AT_entry(const double* y, int idx) const {
         const double* gv = vh(L->gv);
-        int k, a;  // x_k[a] or u_k[a-NX]
-        if (idx < NX) { k = 0; a = idx; }
-        else {
-            const int q = idx - NX, kk = q / pb->blk, r = q % pb->blk;
-            if (r < NU) { k = kk; a = NX + r; }
-            else if (r < NU + NX) { k = kk + 1; a = r - NU; }
-            else return -y[icg(kk + 1) + (r - NU - NX)];
-        }
+        const int imv = imap[idx], k = imv >> 16, a = imv & 255;  // x_k[a] or u_k[a-NX]
+        if (a == 255) return -y[icg(k) + ((imv >> 8) & 255)];
         double s = 0.0;
         if (k < pb->N) {
             const double* Jc = Jk(k) + a; const double* yn = y + icd(k + 1);
@@ -223,14 +246,8 @@ struct Ctx {
     }
     // (W d)_idx
     __device__ double W_entry(const double* d, int idx) const {
-        int k, a;
-        if (idx < NX) { k = 0; a = idx; }
-        else {
-            const int q = idx - NX, kk = q / pb->blk, r = q % pb->blk;
-            if (r < NU) { k = kk; a = NX + r; }
-            else if (r < NU + NX) { k = kk + 1; a = r - NU; }
-            else return 0.0;
-        }
+        const int imv = imap[idx], k = imv >> 16, a = imv & 255;
+        if (a == 255) return 0.0;
         double s = 0.0;
         if (k < pb->N) {
             const double* Wr = Wk(k) + a * NZ; const double* dxk = d + ix(k); const double* duk = d + iu(k);

@@ -43,6 +43,7 @@ struct Solver {
         bl = c.vh(L->bl); bu = c.vh(L->bu);
         for (int q = lane; q < pb->n; q += NT) { bl[q] = pb->xL[q]; bu[q] = pb->xU[q]; }
         c.tm.sync();
+        c.build_maps();
         mode = 0; nX = pb->n;
     }
     __device__ __forceinline__ double* V(int off) const { return c.v(off); }

@@ -102,7 +102,7 @@ static int build_layout(jipm_solver* s, int sm_budget_doubles) {
         {&Lay::Psi, N * NX * NX}, {&Lay::pv, (N + 1) * NX}, {&Lay::qv, N * NX}, {&Lay::wv, N * NX}, {&Lay::sv, N * NX}, {&Lay::tv, N * NU},
         {&Lay::T, (N + 1) * NX * NX}, {&Lay::Kf, N * NU * NX}, {&Lay::Gf, N * NU * NU},
         {&Lay::J, N * NX * NZ}, {&Lay::Dc, m}, {&Lay::gv, N * pb.ng * pd}, {&Lay::dgv, N * pb.ng}, {&Lay::cnd, N * pb.na * pd * pb.na * pd}, {&Lay::tgt, (N + 1) * pb.na * pd},
-        {&Lay::bl, n}, {&Lay::bu, n},
+        {&Lay::bl, n}, {&Lay::bu, n}, {&Lay::imap, (n + 1) / 2}, {&Lay::cmap, (m + 1) / 2},
         {&Lay::filt, 2 * MAX_FILTER},
         // m-vectors
         {&Lay::y, m}, {&Lay::c, m}, {&Lay::b2, m}, {&Lay::dy, m}, {&Lay::ct, m}, {&Lay::r2, m}, {&Lay::e2, m},
