@@ -21,7 +21,8 @@ struct Cfg {
     static constexpr int SM_MSZ = (NZ * NZ > 2 * NX * NX) ? NZ * NZ : 2 * NX * NX;
     static constexpr int SM_T = 0, SM_J = SM_T + NX * NX, SM_M = SM_J + NX * NZ, SM_M2 = SM_M + SM_MSZ, SM_TJ = SM_M2 + SM_MSZ;
     static constexpr int SM_K = SM_TJ + NX * NZ, SM_G = SM_K + NU * NX + NU * NU;
-    static constexpr int SM_RED = SM_G + (Dyn::AX == 12 ? (NT / 16) * 7 * 16 : 0);
+    static constexpr int NGRP = (NT / 16 < 16) ? NT / 16 : 16;  // 16-thread groups of the Hessian column propagation
+    static constexpr int SM_RED = SM_G + (Dyn::AX == 12 ? NGRP * 7 * 16 : 0);
     static constexpr int SM_SPEC = SM_RED + 2 * (NT / 32) + 2;  // (theta, phi) of the speculative trials, one pair per warp
     static constexpr int SM_TOTAL = SM_SPEC + 2 * (NT / 32);
 };

@@ -76,10 +76,10 @@ __device__ void Ctx<C>::dyn_derivs(const double* x, const double* y) {
         // ---- phase 2: 16-thread group <-> (stage, agent), thread <-> column j of z = (x(12), u(4)) ----------
         // (two groups share a warp and run the same instruction stream: __syncwarp orders the staging)
         const int grp = lane >> 4, j = lane & 15;
-        constexpr int NGRP = NT / 16;
+        constexpr int NGRP = C::NGRP;  // threads beyond 16 * NGRP idle through this phase
         double* sV = smt(C::SM_G) + grp * (7 * 16);
         const int nit = N * NA;
-        for (int it0 = 0; it0 < nit; it0 += NGRP) {
+        for (int it0 = 0; it0 < nit && grp < NGRP; it0 += NGRP) {
             const int it = it0 + grp;
             const bool valid = it < nit;
             const int itc = valid ? it : nit - 1;
