@@ -1,8 +1,8 @@
-// inst_pm.cu -- slot kernel instantiation: PointmassDyn, 1 agent(s), 32 threads per problem slot, >= 8 CTA(s) per SM,
+// inst_pm.cu -- slot kernel instantiation: PointmassDyn, 1 agent(s), 128 threads per problem slot, >= 4 CTA(s) per SM,
 // hot layout group guaranteed shared-memory resident.
 #include "inst.cuh"
 namespace jipm {
-Inst inst_pm() { return make_inst<Cfg<PointmassDyn, 1, 32, true>, 8>(); }
+Inst inst_pm() { return make_inst<Cfg<PointmassDyn, 1, 128, true>, 4>(); }
 }  // namespace jipm
 
 namespace jipm {
