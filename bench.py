@@ -284,6 +284,9 @@ def run_jipm(args):
                        ("cyc_derivs", "cyc_factor", "cyc_solve", "cyc_residual", "cyc_trial_eval")}
         phase_share.update({"factor/" + k[5:]: round(stats_sum[k] / cyc_it, 4) for k in stats_sum if k.startswith("cycf_")
                             and stats_sum[k] > 0})
+        # overlapping views: whole blocks of the iteration (they contain the solves / evaluations counted above)
+        phase_share.update({"block/" + k[5:]: round(stats_sum[k] / cyc_it, 4) for k in stats_sum if k.startswith("cycx_")})
+        phase_share["block/speculative_trials"] = round(stats_sum.get("cyc_speculative_trials", 0) / cyc_it, 4)
         us_per_iter = cyc_it / max(stats_sum["iterations"], 1) / (clocks["sm_mhz"] or 1965.0) if clocks else None
         my_secs = sum(a.elapsed_time(b) for a, b in ev) * 1e-3
         achieved = flops / my_secs / 1e12
