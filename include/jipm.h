@@ -115,8 +115,12 @@ int jipm_debug_set_trace(jipm_solver* s, double* trace, int64_t max_records);
 
 /* Layout of the debug state vector used by jipm_debug_step: HOST out, offsets in doubles:
  * lay[0]=len, [1]=x, [2]=y, [3]=zL, [4]=zU, [5]=scalars(mu,tau,delta_w_last,theta_min,theta_max,k,status,nfilt),
- * [6]=filter (128 pairs theta,phi), [7]=dx, [8]=dy, [9]=dzL, [10]=dzU (step of the last iteration),
- * [11]=grad f, [12]=c, [13]=J blocks [N][nx][nx+nu], [14]=W blocks [N][nz][nz] then [nx][nx] */
+ * [6]=filter (256 pairs theta,phi), [7]=dx, [8]=dy, [9]=dzL, [10]=dzU (step of the last iteration),
+ * [11]=grad f, [12]=c, [13]=J blocks [N][nx][nx+nu], [14]=W blocks [N][nz][nz] then [nx][nx],
+ * restoration mode (Step R): [15]=16 scalars (mode, then the parked regular mu, tau, delta_w_last, theta_min,
+ * theta_max, #filter entries, theta at entry, zeta), [16]=(p, n) [2m], [17]=(z_p, z_n) [2m], [18]=x_R [n],
+ * [19]=restoration filter (256 pairs).  With mode = 1 the fields [1]-[5] hold the restoration iterate and scalars
+ * and [6] still holds the REGULAR filter. */
 int jipm_debug_state_layout(jipm_solver* s, int64_t* lay, int64_t n_lay);
 
 /* Load P states (DEVICE [P x len], regular mode), run n_steps iterations each (stops early on a final

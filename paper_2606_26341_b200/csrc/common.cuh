@@ -13,7 +13,7 @@
 namespace jipm {
 
 constexpr unsigned FULL = 0xffffffffu;
-constexpr int MAX_FILTER = 128;
+constexpr int MAX_FILTER = 256;
 constexpr double EPS_MACH = 2.220446049250313e-16;
 
 // problem description, passed by value to the kernel
@@ -60,7 +60,7 @@ struct Args {
 };
 
 // debug state layout (doubles) -- mirrored by jipm_debug_state_layout
-struct DbgLay { int len, x, y, zL, zU, sc, filt, dx, dy, dzL, dzU, g, c, J, W; };
+struct DbgLay { int len, x, y, zL, zU, sc, filt, dx, dy, dzL, dzU, g, c, J, W, rs, pn, zpn, xR, filtR; };
 
 constexpr int RKW = 42;  // doubles of quadrotor phase-1 output per (stage, RK point); see dyn.cuh
 
@@ -72,6 +72,8 @@ __host__ __device__ inline DbgLay make_dbglay(int n, int m, int N, int NX, int N
     d.dx = o; o += n; d.dy = o; o += m; d.dzL = o; o += n; d.dzU = o; o += n;
     d.g = o; o += n; d.c = o; o += m;
     d.J = o; o += N * NX * NZ; d.W = o; o += N * NZ * NZ + NX * NX;
+    // restoration mode (Step R): scalars, (p, n), (z_p, z_n), reference point x_R, the restoration filter
+    d.rs = o; o += 16; d.pn = o; o += 2 * m; d.zpn = o; o += 2 * m; d.xR = o; o += n; d.filtR = o; o += 2 * MAX_FILTER;
     d.len = o;
     return d;
 }

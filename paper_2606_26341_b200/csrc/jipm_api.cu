@@ -311,8 +311,9 @@ extern "C" int jipm_debug_set_trace(jipm_solver* s, double* trace, int64_t max_r
 extern "C" int jipm_debug_state_layout(jipm_solver* s, int64_t* lay, int64_t n_lay) {
     if (!s || !lay) return fail(JIPM_ERR_ARG, "NULL argument");
     const DbgLay& d = s->dbg;
-    const int v[15] = {d.len, d.x, d.y, d.zL, d.zU, d.sc, d.filt, d.dx, d.dy, d.dzL, d.dzU, d.g, d.c, d.J, d.W};
-    for (int64_t i = 0; i < n_lay && i < 15; ++i) lay[i] = v[i];
+    const int v[20] = {d.len, d.x, d.y, d.zL, d.zU, d.sc, d.filt, d.dx, d.dy, d.dzL, d.dzU, d.g, d.c, d.J, d.W,
+                       d.rs, d.pn, d.zpn, d.xR, d.filtR};
+    for (int64_t i = 0; i < n_lay && i < 20; ++i) lay[i] = v[i];
     return JIPM_OK;
 }
 

@@ -13,13 +13,31 @@ __device__ void Solver<C>::dbg_load(const double* st) {
     for (int i = lane; i < pb->n; i += NT) { x[i] = st[D.x + i]; zL[i] = st[D.zL + i]; zU[i] = st[D.zU + i]; }
     for (int i = lane; i < pb->m; i += NT) y[i] = st[D.y + i];
     for (int i = lane; i < 2 * MAX_FILTER; i += NT) VH(L->filt)[i] = st[D.filt + i];
-    mode = 0; nX = pb->n;
+    mode = (int)st[D.rs + 0]; nX = mode ? pb->n + 2 * pb->m : pb->n;
     mu = st[D.sc + 0]; tau = st[D.sc + 1]; dw_last = st[D.sc + 2];
     theta_min = st[D.sc + 3]; theta_max = st[D.sc + 4];
     k = (int)st[D.sc + 5]; status = (int)st[D.sc + 6]; nfilt = (int)st[D.sc + 7];
+    if (mode) {  // restoration state: regular scalars parked, (p, n), (z_p, z_n), x_R, D_R, the restoration filter
+        mu_reg = st[D.rs + 1]; tau_reg = st[D.rs + 2]; dw_last_reg = st[D.rs + 3];
+        theta_min_reg = st[D.rs + 4]; theta_max_reg = st[D.rs + 5]; nfilt_reg = (int)st[D.rs + 6];
+        theta_entry = st[D.rs + 7]; zeta = st[D.rs + 8];
+        Vec xv = VX(L->x); Vec zLv = VX(L->zL); Vec zUv = VX(L->zU);
+        for (int j = lane; j < 2 * pb->m; j += NT) {
+            xv[pb->n + j] = st[D.pn + j]; zLv[pb->n + j] = st[D.zpn + j]; zUv[pb->n + j] = 0.0;
+        }
+        double* xR = V(L->xR); double* DR2 = V(L->DR2);
+        for (int i = lane; i < pb->n; i += NT) {
+            const double xi = st[D.xR + i];
+            xR[i] = xi;
+            const double dr = fmin(1.0, 1.0 / fmax(fabs(xi), 1e-300));
+            DR2[i] = dr * dr;
+        }
+        for (int i = lane; i < 2 * MAX_FILTER; i += NT) V(L->filtR)[i] = st[D.filtR + i];
+    }
     c.tm.sync();
-    bool fin;
-    f = c.eval_fc(x, VH(L->c), theta, cmax, fin);
+    double thb, cmb;
+    f = eval_point(VX(L->x), VH(L->c), theta, cmax, f_base, theta_base, cmax_base, f_pn, f_q);
+    (void)thb; (void)cmb;
 }
 
 template <class C>
@@ -40,6 +58,15 @@ __device__ void Solver<C>::dbg_store(double* st) {
     if (lane == 0) {
         st[D.sc + 0] = mu; st[D.sc + 1] = tau; st[D.sc + 2] = dw_last; st[D.sc + 3] = theta_min;
         st[D.sc + 4] = theta_max; st[D.sc + 5] = k; st[D.sc + 6] = status; st[D.sc + 7] = nfilt;
+        st[D.rs + 0] = mode; st[D.rs + 1] = mu_reg; st[D.rs + 2] = tau_reg; st[D.rs + 3] = dw_last_reg;
+        st[D.rs + 4] = theta_min_reg; st[D.rs + 5] = theta_max_reg; st[D.rs + 6] = nfilt_reg;
+        st[D.rs + 7] = theta_entry; st[D.rs + 8] = zeta;
+    }
+    if (mode) {
+        Vec xv = VX(L->x); Vec zLv = VX(L->zL);
+        for (int j = lane; j < 2 * pb->m; j += NT) { st[D.pn + j] = xv[pb->n + j]; st[D.zpn + j] = zLv[pb->n + j]; }
+        for (int i = lane; i < pb->n; i += NT) st[D.xR + i] = V(L->xR)[i];
+        for (int i = lane; i < 2 * MAX_FILTER; i += NT) st[D.filtR + i] = V(L->filtR)[i];
     }
 }
 

@@ -104,7 +104,8 @@ def fp64_peak_tflops() -> float:
 class Solver:
     """jipm_create / jipm_solve_batch / jipm_destroy with torch tensors for device memory."""
 
-    LAY_NAMES = ["len", "x", "y", "zL", "zU", "sc", "filt", "dx", "dy", "dzL", "dzU", "g", "c", "J", "W"]
+    LAY_NAMES = ["len", "x", "y", "zL", "zU", "sc", "filt", "dx", "dy", "dzL", "dzU", "g", "c", "J", "W",
+                 "rs", "pn", "zpn", "xR", "filtR"]
 
     def __init__(self, family, horizon_N, n_agents, n_obstacles, dt, xL, xU, opts: Options | None = None,
                  resident_slots: int = 0):
@@ -194,8 +195,8 @@ class Solver:
         return self._trace
 
     def state_layout(self):
-        a = (C.c_int64 * 15)()
-        _check(lib().jipm_debug_state_layout(self._h, a, 15))
+        a = (C.c_int64 * 20)()
+        _check(lib().jipm_debug_state_layout(self._h, a, 20))
         return dict(zip(self.LAY_NAMES, list(a)))
 
     def debug_init(self, x0, params):

@@ -115,3 +115,43 @@ def full_system_residual(prob, osol, x, y, zL, zU, theta, mu, dw, dc, step):
     bn = max(float(np.max(np.abs(v))) for v in b)
     sn = max(float(np.max(np.abs(v))) for v in (dx, dy, dzL, dzU))
     return rn / (bn + sn)
+
+
+def prune_filter(filt):
+    """Drop entries dominated by a later one (decision-neutral, reading S-10) so that the oracle's unbounded list
+    fits the GPU filter capacity (256)."""
+    out = []
+    for (t, p) in filt:
+        out = [(a, b) for (a, b) in out if not (a >= t and b >= p)]
+        out.append((t, p))
+    return out
+
+
+def snapshot_state(lay, st, n, m):
+    """Full state of the oracle before an iteration, in the layout of jipm_debug_state_layout (either mode)."""
+    snap = np.zeros(lay["len"])
+
+    def put_filter(key, filt):
+        f = prune_filter(filt)
+        assert len(f) <= 256, len(f)
+        for j, (t, p) in enumerate(f):
+            snap[lay[key] + 2 * j], snap[lay[key] + 2 * j + 1] = t, p
+        return len(f)
+
+    nreg = put_filter("filt", st.filt)
+    if st.resto is None:
+        cur = st
+        snap[lay["x"]:lay["x"] + n], snap[lay["zL"]:lay["zL"] + n], snap[lay["zU"]:lay["zU"] + n] = st.x, st.zL, st.zU
+        nf = nreg
+    else:  # Step R: the restoration iterate X = [x; p; n] with its own scalars and filter, the regular ones parked
+        cur, rp = st.resto.state, st.resto.sub.p
+        snap[lay["x"]:lay["x"] + n], snap[lay["pn"]:lay["pn"] + 2 * m] = cur.x[:n], cur.x[n:]
+        snap[lay["zL"]:lay["zL"] + n], snap[lay["zpn"]:lay["zpn"] + 2 * m] = cur.zL[:n], cur.zL[n:]
+        snap[lay["zU"]:lay["zU"] + n] = cur.zU[:n]
+        snap[lay["xR"]:lay["xR"] + n] = rp.xR
+        snap[lay["rs"]:lay["rs"] + 9] = [1, st.mu, st.tau, st.delta_w_last, st.theta_min, st.theta_max, nreg,
+                                         st.resto.theta_entry, rp.zeta]
+        nf = put_filter("filtR", cur.filt)
+    snap[lay["y"]:lay["y"] + m] = cur.y
+    snap[lay["sc"]:lay["sc"] + 8] = [cur.mu, cur.tau, cur.delta_w_last, cur.theta_min, cur.theta_max, st.k, -1, nf]
+    return snap
