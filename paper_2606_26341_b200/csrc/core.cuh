@@ -20,9 +20,13 @@ struct Cfg {
     // quadrotor Hessian columns (7 x 16 per 16-thread group), the reduction scratch
     static constexpr int SM_MSZ = (NZ * NZ > 2 * NX * NX) ? NZ * NZ : 2 * NX * NX;
     static constexpr int SM_T = 0, SM_J = SM_T + NX * NX, SM_M = SM_J + NX * NZ, SM_M2 = SM_M + SM_MSZ, SM_TJ = SM_M2 + SM_MSZ;
-    static constexpr int SM_K = SM_TJ + NX * NZ, SM_G = SM_K + NU * NX + NU * NU;
+    static constexpr int SM_K = SM_TJ + NX * NZ, SM_TILE_END = SM_K + NU * NX + NU * NU;
     static constexpr int NGRP = (NT / 16 < 16) ? NT / 16 : 16;  // 16-thread groups of the Hessian column propagation
-    static constexpr int SM_RED = SM_G + (Dyn::AX == 12 ? NGRP * 7 * 16 : 0);
+    // the staging of the Hessian columns aliases the factorisation tiles M, M2, TJ, K (derivative evaluation and
+    // factorisation are never live at the same time)
+    static constexpr int SM_G = SM_M;
+    static constexpr int SM_G_END = SM_G + (Dyn::AX == 12 ? NGRP * 7 * 16 : 0);
+    static constexpr int SM_RED = (SM_TILE_END > SM_G_END) ? SM_TILE_END : SM_G_END;
     static constexpr int SM_SPEC = SM_RED + 2 * (NT / 32) + 2;  // (theta, phi) of the speculative trials, one pair per warp
     static constexpr int SM_TOTAL = SM_SPEC + 2 * (NT / 32);
 };
@@ -215,11 +219,12 @@ struct Ctx {
             else if (rr < NX) {
                 const double* Jr = Jk(k) + rr * NZ;
                 s = d[ix(k + 1) + rr];
-                const double* dxk = d + ix(k); const double* duk = d + iu(k);
+                const int ar = (NA == 1) ? 0 : rr / AX;  // J_k is block diagonal over the agents
+                const double* dxk = d + ix(k) + AX * ar; const double* duk = d + iu(k) + AU * ar;
 #pragma unroll 4
-                for (int a = 0; a < NX; ++a) s -= Jr[a] * dxk[a];
+                for (int a = 0; a < AX; ++a) s -= Jr[AX * ar + a] * dxk[a];
 #pragma unroll 4
-                for (int a = 0; a < NU; ++a) s -= Jr[NX + a] * duk[a];
+                for (int a = 0; a < AU; ++a) s -= Jr[NX + AU * ar + a] * duk[a];
             } else {
                 const int j = (cmv >> 8) & 255;
                 s = G_dot(gv, d, k, j) - d[is(k) + j];
@@ -234,9 +239,10 @@ struct Ctx {
         if (a == 255) return -y[icg(k) + ((imv >> 8) & 255)];
         double s = 0.0;
         if (k < pb->N) {
-            const double* Jc = Jk(k) + a; const double* yn = y + icd(k + 1);
+            const int ac = (NA == 1) ? 0 : (a < NX ? a / AX : (a - NX) / AU);  // J_k is block diagonal over the agents
+            const double* Jc = Jk(k) + AX * ac * NZ + a; const double* yn = y + icd(k + 1) + AX * ac;
 #pragma unroll 4
-            for (int l = 0; l < NX; ++l) s -= Jc[l * NZ] * yn[l];
+            for (int l = 0; l < AX; ++l) s -= Jc[l * NZ] * yn[l];
         }
         if (a < NX) {
             s += y[icd(k) + a];

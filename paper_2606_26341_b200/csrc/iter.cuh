@@ -131,12 +131,14 @@ struct Solver {
         for (int j = lane; j < nf; j += NT) hit |= (th_t >= F[2 * j] && ph_t >= F[2 * j + 1]);
         return c.tm.any(hit);
     }
-    __device__ bool acceptable_serial(double th_t, double ph_t, double th_k, double ph_k, double alpha, double g) const {
+    // acceptance test of one speculative candidate by ONE WARP (the filter scanned 32 entries at a time)
+    __device__ bool acceptable_warp(double th_t, double ph_t, double th_k, double ph_k, double alpha, double g) const {
         if (!(isfinite(th_t) && isfinite(ph_t))) return false;
         if (th_t >= theta_max) return false;
         const double* F = filt_active();
-        for (int j = 0; j < nfilt; ++j)
-            if (th_t >= F[2 * j] && ph_t >= F[2 * j + 1]) return false;
+        int hit = 0;
+        for (int j = lane & 31; j < nfilt; j += 32) hit |= (th_t >= F[2 * j] && ph_t >= F[2 * j + 1]);
+        if (__any_sync(FULL, hit)) return false;
         if (th_k <= theta_min && switching(alpha, g, th_k)) return armijo(ph_t, ph_k, alpha, g);
         return th_t <= (1.0 - o->gamma_theta) * th_k ||
                ph_t - ph_k - 10.0 * EPS_MACH * fabs(ph_k) <= -o->gamma_phi * th_k;

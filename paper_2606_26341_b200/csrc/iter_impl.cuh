@@ -490,10 +490,11 @@ __device__ void Solver<C>::iterate() {
                 for (int w = 0; w < (lane >> 5); ++w) aw *= o->alpha_red;
                 double th_w, ph_w;
                 trial_warp(x, dx, aw, th_w, ph_w);
-                if ((lane & 31) == 0) { spec[2 * (lane >> 5)] = th_w; spec[2 * (lane >> 5) + 1] = ph_w; }
+                const bool ok_w = acceptable_warp(th_w, ph_w, theta_k, phi_k, aw, gd);
+                if ((lane & 31) == 0) spec[lane >> 5] = ok_w ? 1.0 : 0.0;
                 c.tm.sync();
                 for (int w = 0; w < NWP; ++w) {
-                    if (acceptable_serial(spec[2 * w], spec[2 * w + 1], theta_k, phi_k, alpha, gd)) { found = true; break; }
+                    if (spec[w] != 0.0) { found = true; break; }
                     n_fc++;
                     alpha *= o->alpha_red;
                     ntrial++;

@@ -27,8 +27,22 @@ namespace jipm {
 
 template <class C>
 struct Kkt {
-    static constexpr int NX = C::NX, NU = C::NU, NZ = C::NZ, PD = C::PD, AX = C::AX, NA = C::NA, NT = C::NT;
+    static constexpr int NX = C::NX, NU = C::NU, NZ = C::NZ, PD = C::PD, AX = C::AX, AU = C::AU, NA = C::NA, NT = C::NT;
     using X = Ctx<C>;
+    // J_k = [A B] is block diagonal over the agents (AX x (AX | AU) blocks): every product with J runs over one
+    // agent's rows / columns only.  agent of column j of z = (x, u):
+    __device__ static __forceinline__ int col_agent(int j) {
+        if constexpr (NA == 1) return 0;
+        else return j < NX ? j / AX : (j - NX) / AU;
+    }
+    __device__ static __forceinline__ int row_agent(int i) {
+        if constexpr (NA == 1) return 0;
+        else return i / AX;
+    }
+    __device__ static __forceinline__ int ctl_agent(int p) {
+        if constexpr (NA == 1) return 0;
+        else return p / AU;
+    }
 
     // dot product with 4 independent partial sums (dependent-chain latency / 4), compile-time length and strides: fully unrolled, immediate offsets
     template <int LEN, int SA, int SB>
@@ -154,7 +168,8 @@ struct Kkt {
             // TJ = T_{k+1} J_k
             for (int e = lane; e < NX * NZ; e += NT) {
                 const int l = e / NZ, j = e % NZ;
-                sTJ[e] = dotc<NX, 1, NZ>(sT + l * NX, sJ + j);
+                const int aj = col_agent(j);
+                sTJ[e] = dotc<AX, 1, NZ>(sT + l * NX + AX * aj, sJ + AX * aj * NZ + j);
             }
             c.tm.sync();
             { const long long t2 = clock64(); c.pc[0] += t2 - tq; tq = t2; }
@@ -162,7 +177,8 @@ struct Kkt {
             const double* Wg = c.Wk(k);
             for (int e = lane; e < NZ * NZ; e += NT) {
                 const int a = e / NZ, j = e % NZ;
-                double m = dotc<NX, NZ, NZ>(sJ + a, sTJ + j);
+                const int aa = col_agent(a);
+                double m = dotc<AX, NZ, NZ>(sJ + AX * aa * NZ + a, sTJ + AX * aa * NZ + j);
                 if (useW) m += Wg[e];
                 if (a == j) m += Sig[c.zidx(k, j)];
                 if (k >= 1 && ng > 0 && a < NX && j < NX && a % AX < PD && j % AX < PD)
@@ -198,7 +214,8 @@ struct Kkt {
             double* Tg = c.vh(c.L->T) + k * NX * NX;
             for (int e = lane; e < NX * NX; e += NT) {
                 const int i = e / NX, a = e % NX;
-                const double phi = sJ[i * NZ + a] - dotc<NU, 1, NZ>(sJ + i * NZ + NX, src + NX * NZ + a);
+                const int ai = row_agent(i);
+                const double phi = sJ[i * NZ + a] - dotc<AU, 1, NZ>(sJ + i * NZ + NX + AU * ai, src + (NX + AU * ai) * NZ + a);
                 if (any_dc) sTJ[e] = phi;
                 else {
                     Pg[e] = phi;
@@ -314,13 +331,15 @@ struct Kkt {
         // ---- phase 0b: h_k ----
         for (int e = lane; e < N * NU; e += NT) {
             const int k = e / NU, p = e % NU;
-            hv[e] = rp[c.iu(k) + p] - dotc<NX, NZ, 1>(c.Jk(k) + NX + p, wv + k * NX);
+            const int ap = ctl_agent(p);
+            hv[e] = rp[c.iu(k) + p] - dotc<AX, NZ, 1>(c.Jk(k) + AX * ap * NZ + NX + p, wv + k * NX + AX * ap);
         }
         c.tm.sync();
         // ---- phase 0c: q_k ----
         for (int e = lane; e < N * NX; e += NT) {
             const int k = e / NX, i = e % NX;
-            qv[e] = pv[e] - dotc<NX, NZ, 1>(c.Jk(k) + i, wv + k * NX) - dotc<NU, NX, 1>(Kf + k * NU * NX + i, hv + k * NU);
+            const int ai = row_agent(i);
+            qv[e] = pv[e] - dotc<AX, NZ, 1>(c.Jk(k) + AX * ai * NZ + i, wv + k * NX + AX * ai) - dotc<NU, NX, 1>(Kf + k * NU * NX + i, hv + k * NU);
         }
         c.tm.sync();
         // ---- phase 1: backward sweep (threads i < NX; whole-team barrier only if NX spans several warps) ----
@@ -344,7 +363,8 @@ struct Kkt {
         c.tm.sync();
         for (int e = lane; e < N * NU; e += NT) {
             const int k = e / NU, p = e % NU;
-            sv[e] = rp[c.iu(k) + p] - dotc<NX, NZ, 1>(c.Jk(k) + NX + p, wv + k * NX);  // st_k (N x NU fits in sv)
+            const int ap = ctl_agent(p);
+            sv[e] = rp[c.iu(k) + p] - dotc<AX, NZ, 1>(c.Jk(k) + AX * ap * NZ + NX + p, wv + k * NX + AX * ap);  // st_k
         }
         c.tm.sync();
         for (int e = lane; e < N * NU; e += NT) {
@@ -354,7 +374,8 @@ struct Kkt {
         c.tm.sync();
         for (int e = lane; e < N * NX; e += NT) {
             const int k = e / NX, i = e % NX;
-            sv[e] = dotc<NU, 1, 1>(c.Jk(k) + i * NZ + NX, hv + k * NU);  // B uo_k   (st_k is dead)
+            const int ai = row_agent(i);
+            sv[e] = dotc<AU, 1, 1>(c.Jk(k) + i * NZ + NX + AU * ai, hv + k * NU + AU * ai);  // B uo_k   (st_k is dead)
         }
         c.tm.sync();
         for (int e = lane; e < N * NX; e += NT) {
@@ -393,7 +414,9 @@ struct Kkt {
         c.tm.sync();
         for (int e = lane; e < N * NX; e += NT) {
             const int k = e / NX, i = e % NX;
-            sv[e] = dotc<NX, 1, 1>(c.Jk(k) + i * NZ, pv + k * NX) + dotc<NU, 1, 1>(c.Jk(k) + i * NZ + NX, hv + k * NU);
+            const int ai = row_agent(i);
+            sv[e] = dotc<AX, 1, 1>(c.Jk(k) + i * NZ + AX * ai, pv + k * NX + AX * ai) +
+                    dotc<AU, 1, 1>(c.Jk(k) + i * NZ + NX + AU * ai, hv + k * NU + AU * ai);
         }
         c.tm.sync();
         for (int e = lane; e < N * NX; e += NT) {
