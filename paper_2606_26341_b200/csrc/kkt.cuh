@@ -60,48 +60,102 @@ struct Kkt {
         return (s0 + s1) + (s2 + s3);
     }
 
-    // T <- (I + P D)^{-1} P in place on the NX x NX tile sT (symmetric), D = Dc at rows [row0, row0+NX).
-    // I + P D = E^{-1} (I + E P E) E with E = sqrt(D): the same leading minors, hence the same unpivoted pivots as the
-    // symmetric I + E P E whose inertia the test needs.  Gauss-Jordan inversion, ping-pong between the two halves of
-    // sM (>= 2 NX^2): one barrier per pivot.  Returns the number of non-positive pivots.
-    __device__ static int transform_T(const X& c, double* sT, double* sM, int row0, bool any_dc) {
-        if (!any_dc) return 0;
-        const double* Dc = c.vh(c.L->Dc) + row0;
-        double* src = sM;
-        double* dst = sM + NX * NX;
-        for (int e = c.lane; e < NX * NX; e += NT) {
-            const int r = e / NX, q = e % NX;
-            src[e] = sT[e] * Dc[q] + (r == q ? 1.0 : 0.0);
+    // G consecutive Gauss-Jordan pivots p0 .. p0+G-1 on the n x n tile src (row stride LD, NE = n * LD elements) in ONE
+    // phase: every element of dst is computed from src alone (no races, one barrier per G pivots), by the thread that
+    // owns it, with exactly the operations the G sequential pivot steps would apply to it -- bit-identical to the
+    // one-pivot-per-barrier form, in particular as stable (forming the inverse of the G x G pivot block explicitly
+    // is not: its determinant cancels when the block is dominated by a rank-one term, e.g. Sigma of one active
+    // obstacle constraint seen through B).  Per element (a, b) this is Gaussian elimination of the bordered matrix
+    //      [ A    B_b  ]      A = src[Pi, Pi],  B_b = src[Pi, b],  C_a = src[a, Pi],  D = src[a, b]
+    //      [ C_a  D    ]
+    // down to its Schur complement D - C_a A^{-1} B_b; the rows / columns inside Pi use C_a = -e_a^T, B_b = e_b,
+    // D = 0, which reproduces the Gauss-Jordan entries (scaled pivot row, negated scaled pivot column, reciprocal
+    // pivot) with exact operations.  The elimination of A (pivots, scaled rows, multipliers) is the same for every
+    // element and done once per thread; the pivot signs carry the inertia test.  An exactly-zero pivot is counted in
+    // nzero and replaced by 1 (the factorisation is rejected anyway).
+    template <int G, int LD, int NE>
+    __device__ static __forceinline__ void gjk(const X& c, const double* src, double* dst, int p0, int& bad, int& nzero) {
+        double A[G][G], id[G];
+#pragma unroll
+        for (int i = 0; i < G; ++i)
+#pragma unroll
+            for (int l = 0; l < G; ++l) A[i][l] = src[(p0 + i) * LD + p0 + l];
+        // after step i: id[i] = 1 / pivot, A[i][l] (l > i) = scaled pivot row, A[j][i] (j > i) = multiplier
+#pragma unroll
+        for (int i = 0; i < G; ++i) {
+            double d = A[i][i];
+            if (!(d > 0.0)) { bad++; if (d == 0.0) { nzero++; d = 1.0; } }
+            id[i] = 1.0 / d;
+#pragma unroll
+            for (int l = i + 1; l < G; ++l) A[i][l] *= id[i];
+#pragma unroll
+            for (int j = i + 1; j < G; ++j)
+#pragma unroll
+                for (int l = i + 1; l < G; ++l) A[j][l] -= A[j][i] * A[i][l];
         }
-        c.tm.sync();
-        int bad = 0;
-        for (int p = 0; p < NX; ++p) {
-            double d = src[p * NX + p];
-            if (!(d > 0.0)) { bad++; if (d == 0.0) d = 1.0; }
-            const double id = 1.0 / d;
-            for (int e = c.lane; e < NX * NX; e += NT) {
-                const int a = e / NX, b = e % NX;
-                const double rb = src[p * NX + b] * id, ca = src[a * NX + p];
-                double v;
-                if (a == p) v = (b == p) ? id : rb;
-                else if (b == p) v = -ca * id;
-                else v = src[e] - ca * rb;
-                dst[e] = v;
+        for (int e = c.lane; e < NE; e += NT) {
+            const int a = e / LD, b = e % LD;
+            const int ia = a - p0, ib = b - p0;
+            const bool ain = ia >= 0 && ia < G, bin = ib >= 0 && ib < G;
+            double B[G], C[G];
+#pragma unroll
+            for (int i = 0; i < G; ++i) {
+                B[i] = bin ? (ib == i ? 1.0 : 0.0) : src[(p0 + i) * LD + b];
+                C[i] = ain ? (ia == i ? -1.0 : 0.0) : src[a * LD + p0 + i];
             }
+            double D = (ain || bin) ? 0.0 : src[e];
+#pragma unroll
+            for (int i = 0; i < G; ++i) {
+                const double rb = B[i] * id[i];
+#pragma unroll
+                for (int j = i + 1; j < G; ++j) B[j] -= A[j][i] * rb;
+#pragma unroll
+                for (int l = i + 1; l < G; ++l) C[l] -= C[i] * A[i][l];
+                D -= C[i] * rb;
+            }
+            dst[e] = D;
+        }
+    }
+    // pivots p0 .. p0+n-1 in groups of four (then two, then one); src / dst are swapped after every phase
+    template <int LD, int NE, int NP>
+    __device__ static __forceinline__ void gj_range(const X& c, double*& src, double*& dst, int p0, int& bad, int& nzero) {
+#pragma unroll 1
+        for (int p = 0; p + 4 <= NP; p += 4) {
+            gjk<4, LD, NE>(c, src, dst, p0 + p, bad, nzero);
             c.tm.sync();
             double* t = src; src = dst; dst = t;
         }
+        if constexpr ((NP & 3) >= 2) {
+            gjk<2, LD, NE>(c, src, dst, p0 + (NP & ~3), bad, nzero);
+            c.tm.sync();
+            double* t = src; src = dst; dst = t;
+        }
+        if constexpr (NP & 1) {
+            gjk<1, LD, NE>(c, src, dst, p0 + NP - 1, bad, nzero);
+            c.tm.sync();
+            double* t = src; src = dst; dst = t;
+        }
+    }
+
+    // T = (I + P D)^{-1} P (D != 0): the tile wk (2 NX^2) holds I + P D in its first half
+    // (written by the caller, barrier passed).  I + P D = E^{-1} (I + E P E) E with E = sqrt(D): the same leading
+    // minors, hence the same unpivoted pivots as the symmetric I + E P E whose inertia the test needs.  Gauss-Jordan
+    // inversion ping-pong between the halves of wk, four pivots per barrier (gjk); `first` runs inside the first phase (work
+    // of the caller that only needs the same barrier).  Then T = sym(inv P) with both (i,q) and (q,i) products in
+    // the same thread (no separate symmetrisation phase); P symmetric at Pm with row stride LDP.  Writes sT and Tg.
+    template <int LDP, class F>
+    __device__ static __forceinline__ void transform_T(const X& c, double* wk, const double* Pm, double* sT, double* Tg,
+                                                       int& bad, int& nzero, F first) {
+        double* src = wk;
+        double* dst = wk + NX * NX;
+        first();
+        gj_range<NX, NX * NX, NX>(c, src, dst, 0, bad, nzero);
         for (int e = c.lane; e < NX * NX; e += NT) {
             const int i = e / NX, q = e % NX;
-            dst[e] = dotc<NX, 1, NX>(src + i * NX, sT + q);
+            const double v = 0.5 * (dotc<NX, 1, LDP>(src + i * NX, Pm + q) + dotc<NX, 1, LDP>(src + q * NX, Pm + i));
+            sT[e] = v; Tg[e] = v;
         }
         c.tm.sync();
-        for (int e = c.lane; e < NX * NX; e += NT) {
-            const int r = e / NX, q = e % NX;
-            sT[e] = 0.5 * (dst[e] + dst[q * NX + r]);
-        }
-        c.tm.sync();
-        return bad;
     }
 
     // Factor.  Reads W, J, Sig, Dc, gv from the workspace; writes T, Kf, Gf, Psi, dgv.  Returns the number of pivots
@@ -139,23 +193,21 @@ struct Kkt {
             }
             c.tm.sync();
         }
-        // terminal block
+        // terminal block: P_N = W_N + Sigma + condensed slacks
         {
             const double* WN = c.Wk(N);
             double* TN = c.vh(c.L->T) + N * NX * NX;
+            double* Pn = any_dc ? tB : sT;
             for (int e = lane; e < NX * NX; e += NT) {
                 const int r = e / NX, q = e % NX;
                 double v = (useW ? WN[e] : 0.0) + (r == q ? Sig[c.ix(N) + r] : 0.0);
                 if (ng > 0 && r % AX < PD && q % AX < PD) v += cnd[(N - 1) * NPOS * NPOS + (PD * (r / AX) + r % AX) * NPOS + PD * (q / AX) + q % AX];
-                sT[e] = v;
-                if (!any_dc) TN[e] = v;
+                Pn[e] = v;
+                if (any_dc) tA[e] = v * Dc[c.icd(N) + q] + (r == q ? 1.0 : 0.0);
+                else TN[e] = v;
             }
             c.tm.sync();
-            if (any_dc) {
-                bad += transform_T(c, sT, tA, c.icd(N), true);
-                for (int e = lane; e < NX * NX; e += NT) TN[e] = sT[e];
-                c.tm.sync();
-            }
+            if (any_dc) transform_T<NX>(c, tA, tB, sT, TN, bad, nzero, [] {});
         }
         for (int k = N - 1; k >= 0; --k) {
             long long tq = clock64();
@@ -187,37 +239,30 @@ struct Kkt {
             }
             c.tm.sync();
             { const long long t2 = clock64(); c.pc[1] += t2 - tq; tq = t2; }
-            // Gauss-Jordan pivots on the controls NX .. NZ-1: every element from the previous tile, no races
+            // Gauss-Jordan pivots on the controls NX .. NZ-1, four per barrier: every element from the previous tile
             double* src = tA; double* dst = tB;
-            for (int p = 0; p < NU; ++p) {
-                const int pp = NX + p;
-                double d = src[pp * NZ + pp];
-                if (!(d > 0.0)) { bad++; if (d == 0.0) { nzero++; d = 1.0; } }
-                const double id = 1.0 / d;
-                for (int e = lane; e < NZ * NZ; e += NT) {
-                    const int a = e / NZ, b = e % NZ;
-                    const double rb = src[pp * NZ + b] * id, ca = src[a * NZ + pp];
-                    double v;
-                    if (a == pp) v = (b == pp) ? id : rb;
-                    else if (b == pp) v = -ca * id;
-                    else v = src[e] - ca * rb;
-                    dst[e] = v;
-                }
-                c.tm.sync();
-                double* t = src; src = dst; dst = t;
-            }
+            gj_range<NZ, NZ * NZ, NU>(c, src, dst, NX, bad, nzero);
             { const long long t2 = clock64(); c.pc[2] += t2 - tq; tq = t2; }
             // src: [[P_k, -Kf^T], [Kf, G]].  Phi = A - B Kf; stores
             double* Kg = c.vh(c.L->Kf) + k * NU * NX;
             double* Gg = c.vh(c.L->Gf) + k * NU * NU;
             double* Pg = c.vh(c.L->Psi) + k * NX * NX;
             double* Tg = c.vh(c.L->T) + k * NX * NX;
+            const int r1 = c.icd(k);
             for (int e = lane; e < NX * NX; e += NT) {
                 const int i = e / NX, a = e % NX;
                 const int ai = row_agent(i);
                 const double phi = sJ[i * NZ + a] - dotc<AU, 1, NZ>(sJ + i * NZ + NX + AU * ai, src + (NX + AU * ai) * NZ + a);
-                if (any_dc) sTJ[e] = phi;
-                else {
+                if (any_dc) {
+                    sTJ[e] = phi;
+                    // P_k symmetrised in place (the thread of (i, a), i <= a, owns both entries) and I + P_k D_k
+                    if (i <= a) {
+                        const double tn = 0.5 * (src[i * NZ + a] + src[a * NZ + i]);
+                        src[i * NZ + a] = tn; src[a * NZ + i] = tn;
+                        dst[i * NX + a] = tn * Dc[r1 + a] + (i == a ? 1.0 : 0.0);
+                        dst[a * NX + i] = tn * Dc[r1 + i] + (i == a ? 1.0 : 0.0);
+                    }
+                } else {
                     Pg[e] = phi;
                     const double tn = 0.5 * (src[i * NZ + a] + src[a * NZ + i]);
                     sT[e] = tn; Tg[e] = tn;
@@ -228,21 +273,14 @@ struct Kkt {
             c.tm.sync();
             { const long long t2 = clock64(); c.pc[3] += t2 - tq; tq = t2; }
             if (any_dc) {
-                // Psi = (I - D_{k+1} T_{k+1}) Phi, then P_k -> T_k = (I + P_k D_k)^{-1} P_k
+                // Psi = (I - D_{k+1} T_{k+1}) Phi inside the first pivot phase, then P_k -> T_k = (I + P_k D_k)^{-1} P_k
                 const int r0 = c.icd(k + 1);
-                for (int e = lane; e < NX * NX; e += NT) {
-                    const int i = e / NX, a = e % NX;
-                    Pg[e] = sTJ[e] - Dc[r0 + i] * dotc<NX, 1, NX>(sT + i * NX, sTJ + a);
-                }
-                c.tm.sync();
-                for (int e = lane; e < NX * NX; e += NT) {
-                    const int r = e / NX, q = e % NX;
-                    sT[e] = 0.5 * (src[r * NZ + q] + src[q * NZ + r]);
-                }
-                c.tm.sync();
-                bad += transform_T(c, sT, dst, c.icd(k), true);
-                for (int e = lane; e < NX * NX; e += NT) Tg[e] = sT[e];
-                c.tm.sync();
+                transform_T<NZ>(c, dst, src, sT, Tg, bad, nzero, [&] {
+                    for (int e = lane; e < NX * NX; e += NT) {
+                        const int i = e / NX, a = e % NX;
+                        Pg[e] = sTJ[e] - Dc[r0 + i] * dotc<NX, 1, NX>(sT + i * NX, sTJ + a);
+                    }
+                });
                 c.pc[4] += clock64() - tq;
             }
         }
