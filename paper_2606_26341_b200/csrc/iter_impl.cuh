@@ -182,6 +182,17 @@ __device__ void Solver<C>::trial_warp(const Vec x, const Vec dx, double alpha, d
         th1 += ROW(c.icg(k) + j, s - X(c.is(k) + j));
     }
     // barrier terms of (3) with the one-sided damping, as in phi()
+    // sum of log(slack) as ONE log per lane: slack = mant * 2^ex with mant in [1, 2); the mantissas are multiplied (a
+    // lane sees nX / 32 + 1 < 1000 of them, far from overflow) and the exponents added as integers.  A slack that is
+    // not a positive normal number marks the point as bad (phi_mu = inf), as log would.
+    double mprod = 1.0;
+    int esum = 0;
+    auto LOGACC = [&](double sl) {
+        if (!(sl >= 2.2250738585072014e-308) || !(sl < INFINITY)) { badpt = 1; return; }
+        const int hi32 = __double2hiint(sl);
+        esum += (hi32 >> 20) - 1023;
+        mprod *= __hiloint2double((hi32 & 0x000fffff) | 0x3ff00000, __double2loint(sl));
+    };
     for (int i = wl; i < nX; i += 32) {
         const double l = lo(i), u = hi(i);
         const bool hl = l > -INFINITY, hu = u < INFINITY;
@@ -189,17 +200,16 @@ __device__ void Solver<C>::trial_warp(const Vec x, const Vec dx, double alpha, d
         const double xi = (i < n) ? X(i) : xt_[i] + alpha * dt_[i];
         if (hl) {
             const double sl = xi - l;
-            if (!(sl > 0.0)) badpt = 1;
-            bar -= mu * log(sl);
+            LOGACC(sl);
             if (!hu) bar += o->kappa_d * mu * sl;
         }
         if (hu) {
             const double su = u - xi;
-            if (!(su > 0.0)) badpt = 1;
-            bar -= mu * log(su);
+            LOGACC(su);
             if (!hl) bar += o->kappa_d * mu * su;
         }
     }
+    bar -= mu * (log(mprod) + 0.6931471805599453 * (double)esum);
 #pragma unroll
     for (int s = 16; s; s >>= 1) {
         f += __shfl_xor_sync(FULL, f, s);

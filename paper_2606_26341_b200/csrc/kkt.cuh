@@ -108,21 +108,21 @@ struct Kkt {
             const int a = e / LD, b = e % LD;
             const int ia = a - p0, ib = b - p0;
             const bool ain = ia >= 0 && ia < G, bin = ib >= 0 && ib < G;
-            double B[G], C[G];
+            double Bv[G], Cv[G];
 #pragma unroll
             for (int i = 0; i < G; ++i) {
-                B[i] = bin ? (ib == i ? 1.0 : 0.0) : src[(p0 + i) * LD + b];
-                C[i] = ain ? (ia == i ? -1.0 : 0.0) : src[a * LD + p0 + i];
+                Bv[i] = bin ? (ib == i ? 1.0 : 0.0) : src[(p0 + i) * LD + b];
+                Cv[i] = ain ? (ia == i ? -1.0 : 0.0) : src[a * LD + p0 + i];
             }
             double D = (ain || bin) ? 0.0 : src[e];
 #pragma unroll
             for (int i = 0; i < G; ++i) {
-                const double rb = B[i] * id[i];
+                const double rb = Bv[i] * id[i];
 #pragma unroll
-                for (int j = i + 1; j < G; ++j) B[j] -= A[j][i] * rb;
+                for (int j = i + 1; j < G; ++j) Bv[j] -= A[j][i] * rb;
 #pragma unroll
-                for (int l = i + 1; l < G; ++l) C[l] -= C[i] * A[i][l];
-                D -= C[i] * rb;
+                for (int l = i + 1; l < G; ++l) Cv[l] -= Cv[i] * A[i][l];
+                D -= Cv[i] * rb;
             }
             dst[e] = D;
         }
