@@ -18,8 +18,12 @@ struct Cfg {
     static constexpr int NX = AX * NA, NU = AU * NA, NZ = NX + NU;
     // fixed shared memory per team (doubles): T, J, M, TJ/Phi, Kf/Linv tiles of the stage sweep, the staging of the
     // quadrotor Hessian columns (7 x 16 per 16-thread group), the reduction scratch
+    // row stride of the stage Jacobians J_k = [A B] (NX x NZ): odd in doubles, so that row-wise AND column-wise
+    // accesses by consecutive threads fall on distinct shared-memory banks (stride NZ = 16 made every row-wise
+    // product a 16-way bank conflict)
+    static constexpr int LDJ = NZ + 1;
     static constexpr int SM_MSZ = (NZ * NZ > 2 * NX * NX) ? NZ * NZ : 2 * NX * NX;
-    static constexpr int SM_T = 0, SM_J = SM_T + NX * NX, SM_M = SM_J + NX * NZ, SM_M2 = SM_M + SM_MSZ, SM_TJ = SM_M2 + SM_MSZ;
+    static constexpr int SM_T = 0, SM_J = SM_T + NX * NX, SM_M = SM_J + ((NX * LDJ + 1) & ~1), SM_M2 = SM_M + SM_MSZ, SM_TJ = SM_M2 + SM_MSZ;
     static constexpr int SM_K = SM_TJ + NX * NZ, SM_TILE_END = SM_K + NU * NX + NU * NU;
     static constexpr int NGRP = (NT / 16 < 16) ? NT / 16 : 16;  // 16-thread groups of the Hessian column propagation
     // the staging of the Hessian columns aliases the factorisation tiles M, M2, TJ, K (derivative evaluation and
@@ -33,7 +37,7 @@ struct Cfg {
 
 template <class C>
 struct Ctx {
-    static constexpr int NX = C::NX, NU = C::NU, NZ = C::NZ, PD = C::PD, AX = C::AX, AU = C::AU, NA = C::NA;
+    static constexpr int NX = C::NX, NU = C::NU, NZ = C::NZ, PD = C::PD, AX = C::AX, AU = C::AU, NA = C::NA, LDJ = C::LDJ;
     static constexpr int NT = C::NT;
     PbProxy pb;        // launch arguments: constant memory (common.cuh)
     LayProxy L;
@@ -90,7 +94,7 @@ struct Ctx {
     __device__ __forceinline__ int icd(int k) const { return k == 0 ? 0 : NX + (k - 1) * pb->cblk; }
     __device__ __forceinline__ int icg(int k) const { return NX + (k - 1) * pb->cblk + NX; }
     __device__ __forceinline__ int zidx(int k, int a) const { return a < NX ? ix(k) + a : iu(k) + a - NX; }
-    __device__ __forceinline__ double* Jk(int k) const { return vh(L->J) + k * (NX * NZ); }
+    __device__ __forceinline__ double* Jk(int k) const { return vh(L->J) + k * (NX * LDJ); }
     __device__ __forceinline__ double* Wk(int k) const { return vh(L->W) + k * (NZ * NZ); }  // k == N: NX x NX
     // workspace array at layout offset off: the first L->nsm doubles of the layout live in shared memory (the
     // hot vectors and factor blocks), the rest in this slot's global workspace (L2-resident scratch)
@@ -217,7 +221,7 @@ struct Ctx {
             const int cmv = cmap[r], rr = cmv & 255, k = cmv >> 16;
             if (rr == 254) s = d[r];
             else if (rr < NX) {
-                const double* Jr = Jk(k) + rr * NZ;
+                const double* Jr = Jk(k) + rr * LDJ;
                 s = d[ix(k + 1) + rr];
                 const int ar = (NA == 1) ? 0 : rr / AX;  // J_k is block diagonal over the agents
                 const double* dxk = d + ix(k) + AX * ar; const double* duk = d + iu(k) + AU * ar;
@@ -240,9 +244,9 @@ struct Ctx {
         double s = 0.0;
         if (k < pb->N) {
             const int ac = (NA == 1) ? 0 : (a < NX ? a / AX : (a - NX) / AU);  // J_k is block diagonal over the agents
-            const double* Jc = Jk(k) + AX * ac * NZ + a; const double* yn = y + icd(k + 1) + AX * ac;
+            const double* Jc = Jk(k) + AX * ac * LDJ + a; const double* yn = y + icd(k + 1) + AX * ac;
 #pragma unroll 4
-            for (int l = 0; l < AX; ++l) s -= Jc[l * NZ] * yn[l];
+            for (int l = 0; l < AX; ++l) s -= Jc[l * LDJ] * yn[l];
         }
         if (a < NX) {
             s += y[icd(k) + a];
@@ -251,23 +255,24 @@ struct Ctx {
         }
         return s;
     }
-    // (W d)_idx
+    // (W d)_idx.  W is symmetric: column idx is read instead of row idx, so that consecutive threads read consecutive
+    // addresses (row access with stride NZ is a 16-way shared-memory bank conflict)
     __device__ double W_entry(const double* d, int idx) const {
         const int imv = imap[idx], k = imv >> 16, a = imv & 255;
         if (a == 255) return 0.0;
-        double s = 0.0;
+        double s0 = 0.0, s1 = 0.0;
         if (k < pb->N) {
-            const double* Wr = Wk(k) + a * NZ; const double* dxk = d + ix(k); const double* duk = d + iu(k);
+            const double* Wc = Wk(k) + a; const double* dxk = d + ix(k); const double* duk = d + iu(k);
 #pragma unroll 4
-            for (int b = 0; b < NX; ++b) s += Wr[b] * dxk[b];
+            for (int b = 0; b < NX; b += 2) { s0 += Wc[b * NZ] * dxk[b]; s1 += Wc[(b + 1) * NZ] * dxk[b + 1]; }
 #pragma unroll 4
-            for (int b = 0; b < NU; ++b) s += Wr[NX + b] * duk[b];
+            for (int b = 0; b < NU; b += 2) { s0 += Wc[(NX + b) * NZ] * duk[b]; s1 += Wc[(NX + b + 1) * NZ] * duk[b + 1]; }
         } else {
-            const double* Wr = Wk(k) + a * NX; const double* dxk = d + ix(k);
+            const double* Wc = Wk(k) + a; const double* dxk = d + ix(k);
 #pragma unroll 4
-            for (int b = 0; b < NX; ++b) s += Wr[b] * dxk[b];
+            for (int b = 0; b < NX; b += 2) { s0 += Wc[b * NX] * dxk[b]; s1 += Wc[(b + 1) * NX] * dxk[b + 1]; }
         }
-        return s;
+        return s0 + s1;
     }
 
     __device__ __noinline__ void eval_derivs(const double* x, const double* y, double sigma_f);

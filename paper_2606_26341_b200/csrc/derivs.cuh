@@ -20,7 +20,7 @@ __device__ void Ctx<C>::dyn_derivs(const double* x, const double* y) {
             else if (r < 2 && cidx == r + 2) v = h;
             else if (r < 2 && cidx == r + 4) v = 0.5 * h * h;
             else if (r >= 2 && cidx == r + 2) v = h;
-            Jk(k)[e] = v;
+            Jk(k)[r * LDJ + cidx] = v;
         }
         for (int it = lane; it < N * NZ * NZ + NX * NX; it += NT) vh(L->W)[it] = 0.0;
         tm.sync();
@@ -126,7 +126,7 @@ __device__ void Ctx<C>::dyn_derivs(const double* x, const double* y) {
                 const int col = (j < 12) ? 12 * a + j : NX + 4 * a + (j - 12);
                 double* Jb = Jk(k);
 #pragma unroll
-                for (int i = 0; i < 12; ++i) Jb[(12 * a + i) * NZ + col] = Jc[i];
+                for (int i = 0; i < 12; ++i) Jb[(12 * a + i) * LDJ + col] = Jc[i];
                 double* Wb = Wk(k);
 #pragma unroll
                 for (int c2 = 0; c2 < 16; ++c2) {

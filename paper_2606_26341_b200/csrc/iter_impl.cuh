@@ -31,7 +31,7 @@ __device__ void Solver<C>::init_problem(long long id) {
         }
     }
     if (NA > 1) {
-        for (int it = lane; it < N * NX * NZ; it += NT) V(L->J)[it] = 0.0;
+        for (int it = lane; it < N * NX * C::LDJ; it += NT) V(L->J)[it] = 0.0;
     }
     c.tm.sync();
     if (o->init_slacks) {  // I-2

@@ -101,7 +101,8 @@ static int build_layout(jipm_solver* s, int sm_budget_doubles) {
         // the factor and what every solve streams through
         {&Lay::Psi, N * NX * NX}, {&Lay::pv, (N + 1) * NX}, {&Lay::qv, N * NX}, {&Lay::wv, N * NX}, {&Lay::sv, N * NX}, {&Lay::tv, N * NU},
         {&Lay::T, (N + 1) * NX * NX}, {&Lay::Kf, N * NU * NX}, {&Lay::Gf, N * NU * NU},
-        {&Lay::J, N * NX * NZ}, {&Lay::Dc, m}, {&Lay::gv, N * pb.ng * pd}, {&Lay::dgv, N * pb.ng}, {&Lay::cnd, N * pb.na * pd * pb.na * pd}, {&Lay::tgt, (N + 1) * pb.na * pd},
+        {&Lay::J, N * NX * (NZ + 1)},  // row stride LDJ = NZ + 1 (core.cuh)
+        {&Lay::Dc, m}, {&Lay::gv, N * pb.ng * pd}, {&Lay::dgv, N * pb.ng}, {&Lay::cnd, N * pb.na * pd * pb.na * pd}, {&Lay::tgt, (N + 1) * pb.na * pd},
         {&Lay::bl, n}, {&Lay::bu, n}, {&Lay::imap, (n + 1) / 2}, {&Lay::cmap, (m + 1) / 2},
         {&Lay::filt, 2 * MAX_FILTER},
         // m-vectors

@@ -53,7 +53,7 @@ __device__ void Solver<C>::dbg_store(double* st) {
         st[D.y + i] = VH(L->y)[i]; st[D.dy + i] = VH(L->dy)[i]; st[D.c + i] = VH(L->c)[i];
     }
     for (int i = lane; i < 2 * MAX_FILTER; i += NT) st[D.filt + i] = VH(L->filt)[i];
-    for (int i = lane; i < pb->N * NX * NZ; i += NT) st[D.J + i] = VH(L->J)[i];
+    for (int i = lane; i < pb->N * NX * NZ; i += NT) st[D.J + i] = VH(L->J)[(i / NZ) * C::LDJ + i % NZ];  // dense in the debug state
     for (int i = lane; i < pb->N * NZ * NZ + NX * NX; i += NT) st[D.W + i] = VH(L->W)[i];
     if (lane == 0) {
         st[D.sc + 0] = mu; st[D.sc + 1] = tau; st[D.sc + 2] = dw_last; st[D.sc + 3] = theta_min;
@@ -103,7 +103,7 @@ __global__ void __launch_bounds__(C::NT, MINB) jipm_slot_kernel() {
                     }
                 }
                 if (C::NA > 1)
-                    for (int it = lane; it < pb->N * C::NX * C::NZ; it += NT) ctx.vh(A->L.J)[it] = 0.0;
+                    for (int it = lane; it < pb->N * C::NX * C::LDJ; it += NT) ctx.vh(A->L.J)[it] = 0.0;
                 ctx.tm.sync();
             }
             ctx.tm.sync();

@@ -27,7 +27,7 @@ namespace jipm {
 
 template <class C>
 struct Kkt {
-    static constexpr int NX = C::NX, NU = C::NU, NZ = C::NZ, PD = C::PD, AX = C::AX, AU = C::AU, NA = C::NA, NT = C::NT;
+    static constexpr int NX = C::NX, NU = C::NU, NZ = C::NZ, PD = C::PD, AX = C::AX, AU = C::AU, NA = C::NA, NT = C::NT, LDJ = C::LDJ;
     using X = Ctx<C>;
     // J_k = [A B] is block diagonal over the agents (AX x (AX | AU) blocks): every product with J runs over one
     // agent's rows / columns only.  agent of column j of z = (x, u):
@@ -177,7 +177,7 @@ struct Kkt {
         const PbProxy pb;
         const int N = pb->N, lane = c.lane, ng = pb->ng;
         double* sT = c.smt(C::SM_T);     // NX x NX   current T_{k+1} / P_k
-        double* sJc = c.smt(C::SM_J);    // NX x NZ   copy of J_k when J is not shared-memory resident
+        double* sJc = c.smt(C::SM_J);    // NX x LDJ  copy of J_k when J is not shared-memory resident
         double* tA = c.smt(C::SM_M);     // NZ x NZ   stage tile (>= 2 NX^2: scratch of transform_T)
         double* tB = c.smt(C::SM_M2);    // NZ x NZ   second tile of the Gauss-Jordan ping-pong
         double* sTJ = c.smt(C::SM_TJ);   // NX x NZ   T J, later Phi (NX x NX)
@@ -224,7 +224,7 @@ struct Kkt {
             long long tq = clock64();
             const double* sJ = c.Jk(k);
             if (!j_in_sm) {
-                for (int e = lane; e < NX * NZ; e += NT) sJc[e] = sJ[e];
+                for (int e = lane; e < NX * LDJ; e += NT) sJc[e] = sJ[e];
                 sJ = sJc;
                 c.tm.sync();
             }
@@ -232,7 +232,7 @@ struct Kkt {
             for (int e = lane; e < NX * NZ; e += NT) {
                 const int l = e / NZ, j = e % NZ;
                 const int aj = col_agent(j);
-                sTJ[e] = dotc<AX, 1, NZ>(sT + l * NX + AX * aj, sJ + AX * aj * NZ + j);
+                sTJ[e] = dotc<AX, 1, LDJ>(sT + l * NX + AX * aj, sJ + AX * aj * LDJ + j);
             }
             c.tm.sync();
             { const long long t2 = clock64(); c.pc[0] += t2 - tq; tq = t2; }
@@ -241,7 +241,7 @@ struct Kkt {
             for (int e = lane; e < NZ * NZ; e += NT) {
                 const int a = e / NZ, j = e % NZ;
                 const int aa = col_agent(a);
-                double m = dotc<AX, NZ, NZ>(sJ + AX * aa * NZ + a, sTJ + AX * aa * NZ + j);
+                double m = dotc<AX, LDJ, NZ>(sJ + AX * aa * LDJ + a, sTJ + AX * aa * NZ + j);
                 if (useW) m += Wg[e];
                 if (a == j) m += Sig[c.zidx(k, j)];
                 if (k >= 1 && ng > 0 && a < NX && j < NX && a % AX < PD && j % AX < PD)
@@ -263,7 +263,7 @@ struct Kkt {
             for (int e = lane; e < NX * NX; e += NT) {
                 const int i = e / NX, a = e % NX;
                 const int ai = row_agent(i);
-                const double phi = sJ[i * NZ + a] - dotc<AU, 1, NZ>(sJ + i * NZ + NX + AU * ai, src + (NX + AU * ai) * NZ + a);
+                const double phi = sJ[i * LDJ + a] - dotc<AU, 1, NZ>(sJ + i * LDJ + NX + AU * ai, src + (NX + AU * ai) * NZ + a);
                 if (any_dc) {
                     sTJ[e] = phi;
                     // P_k symmetrised in place (the thread of (i, a), i <= a, owns both entries) and I + P_k D_k
@@ -381,14 +381,14 @@ struct Kkt {
         for (int e = lane; e < N * NU; e += NT) {
             const int k = e / NU, p = e % NU;
             const int ap = ctl_agent(p);
-            hv[e] = rp[c.iu(k) + p] - dotc<AX, NZ, 1>(c.Jk(k) + AX * ap * NZ + NX + p, wv + k * NX + AX * ap);
+            hv[e] = rp[c.iu(k) + p] - dotc<AX, LDJ, 1>(c.Jk(k) + AX * ap * LDJ + NX + p, wv + k * NX + AX * ap);
         }
         c.tm.sync();
         // ---- phase 0c: q_k ----
         for (int e = lane; e < N * NX; e += NT) {
             const int k = e / NX, i = e % NX;
             const int ai = row_agent(i);
-            qv[e] = pv[e] - dotc<AX, NZ, 1>(c.Jk(k) + AX * ai * NZ + i, wv + k * NX + AX * ai) - dotc<NU, NX, 1>(Kf + k * NU * NX + i, hv + k * NU);
+            qv[e] = pv[e] - dotc<AX, LDJ, 1>(c.Jk(k) + AX * ai * LDJ + i, wv + k * NX + AX * ai) - dotc<NU, NX, 1>(Kf + k * NU * NX + i, hv + k * NU);
         }
         c.tm.sync();
         // ---- phase 1: backward sweep (threads i < NX; whole-team barrier only if NX spans several warps) ----
@@ -413,7 +413,7 @@ struct Kkt {
         for (int e = lane; e < N * NU; e += NT) {
             const int k = e / NU, p = e % NU;
             const int ap = ctl_agent(p);
-            sv[e] = rp[c.iu(k) + p] - dotc<AX, NZ, 1>(c.Jk(k) + AX * ap * NZ + NX + p, wv + k * NX + AX * ap);  // st_k
+            sv[e] = rp[c.iu(k) + p] - dotc<AX, LDJ, 1>(c.Jk(k) + AX * ap * LDJ + NX + p, wv + k * NX + AX * ap);  // st_k
         }
         c.tm.sync();
         for (int e = lane; e < N * NU; e += NT) {
@@ -424,7 +424,7 @@ struct Kkt {
         for (int e = lane; e < N * NX; e += NT) {
             const int k = e / NX, i = e % NX;
             const int ai = row_agent(i);
-            sv[e] = dotc<AU, 1, 1>(c.Jk(k) + i * NZ + NX + AU * ai, hv + k * NU + AU * ai);  // B uo_k   (st_k is dead)
+            sv[e] = dotc<AU, 1, 1>(c.Jk(k) + i * LDJ + NX + AU * ai, hv + k * NU + AU * ai);  // B uo_k   (st_k is dead)
         }
         c.tm.sync();
         for (int e = lane; e < N * NX; e += NT) {
@@ -464,8 +464,8 @@ struct Kkt {
         for (int e = lane; e < N * NX; e += NT) {
             const int k = e / NX, i = e % NX;
             const int ai = row_agent(i);
-            sv[e] = dotc<AX, 1, 1>(c.Jk(k) + i * NZ + AX * ai, pv + k * NX + AX * ai) +
-                    dotc<AU, 1, 1>(c.Jk(k) + i * NZ + NX + AU * ai, hv + k * NU + AU * ai);
+            sv[e] = dotc<AX, 1, 1>(c.Jk(k) + i * LDJ + AX * ai, pv + k * NX + AX * ai) +
+                    dotc<AU, 1, 1>(c.Jk(k) + i * LDJ + NX + AU * ai, hv + k * NU + AU * ai);
         }
         c.tm.sync();
         for (int e = lane; e < N * NX; e += NT) {
