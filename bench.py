@@ -138,9 +138,9 @@ def time_oracle(cfg: int, first: int, count: int, cores: int):
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE slot-kernel launch over the config's full batch, from the
-# `ncu --set full` capture summarised in profiles/r1_ncu_full_c1.md (37.8 MB read + 2131.1 MB
+# `ncu --set full` capture summarised in profiles/r1_ncu_full_c1.md (40.1 MB read + 2191.2 MB
 # written: write-back of the L2-resident per-slot scratch)
-NCU_TRAFFIC_BYTES = {1: 2168.9e6}
+NCU_TRAFFIC_BYTES = {1: 2231.3e6}
 
 ORACLE_SAMPLE = {0: 256, 1: 16, 2: 2, 3: 2}  # problems per timed sample (about 10-30 s of CPU work)
 
