@@ -171,8 +171,10 @@ struct Kkt {
 
     // Factor.  Reads W, J, Sig, Dc, gv from the workspace; writes T, Kf, Gf, Psi, dgv.  Returns the number of pivots
     // with the wrong sign (0 <=> inertia (n, m, 0)); nzero counts exactly-zero pivots.  any_dc: some Dc entry != 0.
-    // Per stage (regular mode): T J | M = Q + J^T (T J) + condensed slacks | nu Gauss-Jordan pivots on the control
-    // block, ping-pong between two tiles (afterwards the tile holds P_k, Kf_k, G_k at once) | Phi, stores.
+    // Per stage (regular mode, one barrier per item): T J | M = Q + J^T (T J) + condensed slacks | the nu Gauss-Jordan
+    // pivots on the control block, four per barrier (gjk), ping-pong between two tiles (afterwards the tile holds P_k,
+    // Kf_k, G_k at once) | Phi, stores.  With D != 0: the Phi phase also symmetrises P_k and writes I + P_k D_k, Psi runs
+    // inside the first pivot phase of transform_T.
     __device__ static __noinline__ int factor(const X& c, int& nzero, bool any_dc, bool useW) {
         const PbProxy pb;
         const int N = pb->N, lane = c.lane, ng = pb->ng;
