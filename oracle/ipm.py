@@ -2,10 +2,11 @@
 interior-point iteration of arxiv 2606.26341 section IV: barrier problem (3), iterate
 (x, y_c, z_L, z_U) and Lagrangian (4), Newton system (6), augmented system (7) with inertia-correcting
 perturbations (delta_w, delta_c), and the Table I fallbacks the hot path covers
-(PAPER.md:118-142): backtracking line search, second-order correction, hard feasibility restoration,
-monotone barrier update.  The paper defers every constant and the filter/restoration details to its
-reference [7] (Waechter & Biegler 2006); the readings taken are listed in DESIGN.md "Readings" and all
-constants live in ``Options``.
+(PAPER.md:118-142): backtracking line search (row 1), second-order correction (row 2), watchdog (row 3),
+tiny-step rule (row 4), soft feasibility restoration (row 5), hard feasibility restoration (row 6),
+monotone barrier update (row 7).  The paper defers every constant and the filter/restoration details to
+its reference [7] (Waechter & Biegler 2006); the readings taken are listed in DESIGN.md "Readings" and
+all constants live in ``Options``.
 
 The oracle follows the algorithm step by step (Step I = initialise, Step A = one iteration, Step R =
 restoration) on DENSE matrices: the Newton step is the solution of the dense
@@ -13,9 +14,11 @@ system (7) by Bunch-Kaufman LDL^T (oracle/linsolve.py), Delta z from PAPER.md:11
 unreduced system (6).  Restoration is the same iteration applied, recursively, to the restoration NLP
 written out as an NLP (no elimination of p, n).  Nothing here is shared with the CUDA path.
 
-Parity status: every function below is pinned by tests/test_oracle_*.py EXCEPT the items DESIGN.md lists
-as "parity unpinned" (exact restoration trajectory and multiplier reset after restoration; the IPOPT
-release values of gamma_phi, eta_phi, kappa_d).
+Parity status: every function below is pinned by tests/test_oracle_*.py (closed forms, hand-computed cases,
+independent library routines).  What stays "parity unpinned": the VALUES of the constants
+recalled from IPOPT's release (gamma_phi, eta_phi, kappa_d, the watchdog / soft-restoration / tiny-step
+thresholds) and the choice of readings R-1, R-2, S-15 of Step R -- the mechanics of each reading are pinned,
+that IPOPT takes the same reading cannot be checked here ([7] and IPOPT are not available).
 """
 from __future__ import annotations
 
@@ -27,7 +30,7 @@ import numpy as np
 from .linsolve import DenseLDL
 
 ST_NOT_RUN, ST_SOLVED, ST_MAXITER, ST_LOCALLY_INFEASIBLE = -1, 0, 1, 2
-ST_RESTORATION_FAILED, ST_RESTO_AT_FEASIBLE_POINT, ST_NONFINITE = 3, 4, 5
+ST_RESTORATION_FAILED, ST_RESTO_AT_FEASIBLE_POINT, ST_NONFINITE, ST_TINY_STEP = 3, 4, 5, 6
 EPS = 2.220446049250313e-16
 
 
@@ -79,6 +82,17 @@ class Options:
     zero_pivot_tol: float = 0.0
     init_slacks: int = 1
     enable_restoration: int = 1
+    # iterative refinement / "pretend singular" (reading S-7)
+    residual_ratio_singular: float = 1e-5
+    residual_improvement_factor: float = 0.999999999
+    # Table I rows 3-5 (readings W, T, SR of DESIGN.md section 3)
+    watchdog_trigger: int = 10        # consecutive shortened steps that wake the watchdog (0 = off)
+    watchdog_trial_max: int = 3       # trial steps accepted unconditionally before reverting
+    tiny_step_tol: float = 10.0 * 2.220446049250313e-16
+    tiny_step_y_tol: float = 1e-2
+    tiny_step_cviol: float = 1e-4
+    soft_resto_factor: float = 1.0 - 1e-4   # required reduction of the primal-dual error (0 = off)
+    max_soft_resto_iters: int = 10
 
     @property
     def mu_min(self) -> float:
@@ -100,6 +114,27 @@ class State:
     k: int = 0
     status: int = ST_NOT_RUN
     resto: "RestoContext | None" = None
+    n_short: int = 0                  # consecutive iterations whose accepted step needed backtracking
+    wd: "Watchdog | None" = None      # watchdog in progress (Table I row 3)
+    soft: bool = False                # in the soft restoration phase (Table I row 5)
+    soft_count: int = 0
+    tiny_last: bool = False           # the previous iteration took a tiny step (Table I row 4)
+    tiny_flag: bool = False           # two tiny steps in a row: force a barrier decrease at the next A-3
+
+
+@dataclass
+class Watchdog:
+    """Entry iterate of the watchdog, its search direction and the reference values of the acceptance test."""
+    x: np.ndarray
+    y: np.ndarray
+    zL: np.ndarray
+    zU: np.ndarray
+    d: tuple
+    theta: float
+    phi: float
+    gd: float
+    alpha: float
+    trials: int = 0
 
 
 def relax_bounds(xL, xU, o: Options):
@@ -248,15 +283,31 @@ class Solver:
         K[n:, n:] = -dc * np.eye(m)
         return K
 
-    def inertia_correction(self, W, Sigma, A, mu, dw_last):
-        """Algorithm IC ([7] sec 3.1, recalled).  Returns (factor, dw, dc, nfact) or None."""
+    def inertia_correction(self, W, Sigma, A, mu, dw_last, resume=None):
+        """Algorithm IC ([7] sec 3.1, recalled).  Returns (factor, dw, dc, nfact) or None.
+
+        ``resume=(dw, dc)``: the factorisation with these perturbations had the right inertia but the solve with it
+        failed the refinement test ("pretend singular", reading S-7): the matrix is treated like one with a zero
+        eigenvalue -- delta_c takes its IC-2 value, delta_w moves to the next rung of the ladder (IC-3 from 0,
+        else IC-5) -- and the loop IC-4..IC-6 continues from there."""
         o, n, m = self.o, self.n, self.m
-        fac = DenseLDL(self.kkt_matrix(W, Sigma, A, 0.0, 0.0), o.zero_pivot_tol)  # IC-1
-        nfact = 1
-        if fac.inertia == (n, m, 0):
-            return fac, 0.0, 0.0, nfact
-        dc = o.delta_c_bar * mu ** o.kappa_c if fac.inertia[2] > 0 else 0.0  # IC-2
-        dw = o.delta_w_0 if dw_last == 0.0 else max(o.delta_w_min, o.kappa_w_minus * dw_last)  # IC-3
+        nfact = 0
+        if resume is None:
+            fac = DenseLDL(self.kkt_matrix(W, Sigma, A, 0.0, 0.0), o.zero_pivot_tol)  # IC-1
+            nfact = 1
+            if fac.inertia == (n, m, 0):
+                return fac, 0.0, 0.0, nfact
+            dc = o.delta_c_bar * mu ** o.kappa_c if fac.inertia[2] > 0 else 0.0  # IC-2
+            dw = o.delta_w_0 if dw_last == 0.0 else max(o.delta_w_min, o.kappa_w_minus * dw_last)  # IC-3
+        else:
+            dw, dc = resume
+            dc = o.delta_c_bar * mu ** o.kappa_c
+            if dw == 0.0:
+                dw = o.delta_w_0 if dw_last == 0.0 else max(o.delta_w_min, o.kappa_w_minus * dw_last)
+            else:
+                dw = (o.kappa_w_plus_first if dw_last == 0.0 else o.kappa_w_plus) * dw
+                if dw > o.delta_w_max:
+                    return None
         while True:
             fac = DenseLDL(self.kkt_matrix(W, Sigma, A, dw, dc), o.zero_pivot_tol)  # IC-4
             nfact += 1
@@ -291,20 +342,35 @@ class Solver:
             dzU = np.where(self.hasU, (b4 + zU * dx) / sU, 0.0)
             return [dx, dy, dzL, dzU]
 
-        d = reduced_solve(*b)
-        bnorm = max(float(np.max(np.abs(v))) if v.size else 0.0 for v in b)
-        nref = 0
-        while nref < o.refine_max:
+        def ratio(d):
             lhs = self.full_matvec(W, A, x, zL, zU, dw, dc, d)
             res = [bi - li for bi, li in zip(b, lhs)]
             rnorm = max(float(np.max(np.abs(v))) if v.size else 0.0 for v in res)
             dnorm = max(float(np.max(np.abs(v))) if v.size else 0.0 for v in d)
-            if nref >= o.refine_min and rnorm <= o.residual_ratio_max * (bnorm + dnorm):
+            den = bnorm + dnorm
+            return res, (rnorm / den if den > 0.0 else rnorm)
+
+        d = reduced_solve(*b)
+        bnorm = max(float(np.max(np.abs(v))) if v.size else 0.0 for v in b)
+        res, rat = ratio(d)
+        nref, failed = 0, False
+        # at least refine_min steps; stop at ratio <= residual_ratio_max; give up when refine_max is exceeded or
+        # a step no longer improves the ratio -- then the solution is kept if the ratio is below
+        # residual_ratio_singular, else the solve is reported as FAILED (the caller pretends the matrix is singular)
+        while rat > o.residual_ratio_max or nref < o.refine_min:
+            if not math.isfinite(rat):
+                failed = True
                 break
             corr = reduced_solve(*res)
             d = [di + ci for di, ci in zip(d, corr)]
             nref += 1
-        return d, nref
+            rat_old = rat
+            res, rat = ratio(d)
+            if rat > o.residual_ratio_max and nref > o.refine_min and (
+                    nref >= o.refine_max or rat > o.residual_improvement_factor * rat_old):
+                failed = not (rat < o.residual_ratio_singular)
+                break
+        return d, nref, failed
 
     # ---- filter acceptance ([7] sec 2.3) -----------------------------------------
     def switching(self, alpha, g, theta_k):
@@ -336,6 +402,29 @@ class Solver:
         theta = float(np.sum(np.abs(cv))) if cv.size else 0.0
         return fv, cv, theta, self.phi(x, fv, mu)
 
+    def alpha_min(self, gd, theta_k, theta_min):
+        """Smallest step length the backtracking line search tries before it gives up (A-5; [7] eq 23, recalled)."""
+        o = self.o
+        if gd < 0.0 and theta_k <= theta_min:
+            return o.gamma_alpha * min(o.gamma_theta, o.gamma_phi * theta_k / (-gd),
+                                       o.delta * theta_k ** o.s_theta / (-gd) ** o.s_phi)
+        if gd < 0.0:
+            return o.gamma_alpha * min(o.gamma_theta, o.gamma_phi * theta_k / (-gd))
+        return o.gamma_alpha * o.gamma_theta
+
+    def pd_error(self, x, y, zL, zU, g, cval, A, mu):
+        """Error of the primal-dual system (5a-d) as the soft restoration phase measures it:
+        the 1-norm of each block divided by its length, summed (reading SR)."""
+        sL, sU = self.slacks(x)
+        rd = g + A.T @ y - zL + zU + self.damping(mu)
+        comp = np.concatenate([(sL * zL - mu)[self.hasL], (sU * zU - mu)[self.hasU]])
+        e = float(np.sum(np.abs(rd))) / self.n
+        if self.m:
+            e += float(np.sum(np.abs(cval))) / self.m
+        if comp.size:
+            e += float(np.sum(np.abs(comp))) / comp.size
+        return e
+
     # ---- Step A: one iteration ------------------------------------------------------------------------
     def iterate(self, st: State, th) -> dict:
         """Advance ``st`` by one iteration (regular or restoration mode); returns the decision trace."""
@@ -343,7 +432,7 @@ class Solver:
             return self.iterate_resto(st, th)
         o, p, n, m = self.o, self.p, self.n, self.m
         tr = dict(mode=0, nfact=0, dw=0.0, dc=0.0, nref=0, kind="", ls=0, soc=0, alpha=0.0, alpha_z=0.0,
-                  ftype=False, augment=False, nmu=0, status=ST_NOT_RUN)
+                  ftype=False, augment=False, nmu=0, status=ST_NOT_RUN, npsing=0, wd=0, soft=0, tiny=0)
         x, y = st.x, st.y
         # A-1 evaluate
         fv, g, cv, A = p.f(x, th), p.grad_f(x, th), p.c(x, th), p.jac(x, th)
@@ -359,12 +448,24 @@ class Solver:
         if st.k >= o.max_iter:
             st.status = tr["status"] = ST_MAXITER
             return tr
-        # A-3 monotone barrier update (Table I row 7: the monotone schedule)
-        while (tr["nmu"] < o.max_mu_updates and st.mu > o.mu_min
-               and self.opt_error(x, y, st.zL, st.zU, g, cv, A, st.mu) <= o.kappa_eps * st.mu):
+        # A-3 monotone barrier update (Table I row 7: the monotone schedule).  Two tiny steps in a
+        # row (Table I row 4) force one decrease; if mu cannot decrease any more the search direction has become
+        # too small to make progress: TINY_STEP.
+        force = st.tiny_flag
+        st.tiny_flag = False
+        while tr["nmu"] < o.max_mu_updates and (
+                force or self.opt_error(x, y, st.zL, st.zU, g, cv, A, st.mu) <= o.kappa_eps * st.mu):
+            if not st.mu > o.mu_min:
+                if force:
+                    st.status = tr["status"] = ST_TINY_STEP
+                    return tr
+                break
+            force = False
             st.mu = max(o.mu_min, min(o.kappa_mu * st.mu, st.mu ** o.theta_mu))
             st.tau = max(o.tau_min, 1.0 - st.mu)
             st.filt = []
+            # a new barrier problem: the watchdog, its counter and the soft restoration phase start afresh
+            st.wd, st.n_short, st.soft, st.soft_count = None, 0, False, 0
             tr["nmu"] += 1
             if hasattr(p, "set_mu"):
                 p.set_mu(st.mu)
@@ -374,49 +475,149 @@ class Solver:
         # A-4 search direction
         sL, sU = self.slacks(x)
         Sigma = np.where(self.hasL, st.zL / sL, 0.0) + np.where(self.hasU, st.zU / sU, 0.0)
-        ic = self.inertia_correction(W, Sigma, A, mu, st.delta_w_last)
-        if ic is None:
-            tr["kind"] = "ic_fail"
-            return self.enter_restoration(st, th, tr, fv, cv)
-        fac, dw, dc, tr["nfact"] = ic
-        tr["dw"], tr["dc"] = dw, dc
-        if dw > 0.0:
-            st.delta_w_last = dw
         gphi = self.grad_phi(x, g, mu)
         b = [-(g + A.T @ y - st.zL + st.zU + self.damping(mu)), -cv,
              np.where(self.hasL, mu - sL * st.zL, 0.0), np.where(self.hasU, mu - sU * st.zU, 0.0)]
-        (dx, dy, dzL, dzU), tr["nref"] = self.solve_full(fac, W, A, x, st.zL, st.zU, dw, dc, b)
+        resume = None
+        while True:
+            ic = self.inertia_correction(W, Sigma, A, mu, st.delta_w_last, resume)
+            if ic is None:
+                tr["kind"] = "ic_fail"
+                tr["nfact"] = tr["nref"] = 0
+                tr["dw"] = tr["dc"] = 0.0
+                return self.enter_restoration(st, th, tr, fv, cv)
+            fac, dw, dc, nf = ic
+            tr["nfact"] += nf
+            (dx, dy, dzL, dzU), tr["nref"], failed = self.solve_full(fac, W, A, x, st.zL, st.zU, dw, dc, b)
+            if not failed:
+                break
+            tr["npsing"] += 1          # refinement failed: pretend the matrix is singular (reading S-7)
+            resume = (dw, dc)
+        tr["dw"], tr["dc"] = dw, dc
+        if dw > 0.0:
+            st.delta_w_last = dw
         tr["step"] = (dx, dy, dzL, dzU)
-        # A-5 filter line search
+        d = (dx, dy, dzL, dzU)
+        # A-5 line search
         theta_k = float(np.sum(np.abs(cv))) if m else 0.0
         phi_k = self.phi(x, fv, mu)
         gd = float(gphi @ dx)
         a_max = self.ftb_primal(x, dx, tau)
-        if gd < 0.0 and theta_k <= st.theta_min:
-            a_min = o.gamma_alpha * min(o.gamma_theta, o.gamma_phi * theta_k / (-gd),
-                                        o.delta * theta_k ** o.s_theta / (-gd) ** o.s_phi)
-        elif gd < 0.0:
-            a_min = o.gamma_alpha * min(o.gamma_theta, o.gamma_phi * theta_k / (-gd))
+        tr["theta"], tr["phi"], tr["gd"], tr["a_max"] = theta_k, phi_k, gd, a_max
+
+        # Table I row 4: a step too small for backtracking to refine is accepted as it is
+        xmax = float(np.max(np.abs(dx) / (1.0 + np.abs(x)))) if n else 0.0
+        cmax = float(np.max(np.abs(cv))) if m else 0.0
+        if xmax <= o.tiny_step_tol and cmax <= o.tiny_step_cviol:
+            tr["tiny"] = 1
+            if st.tiny_last and (float(np.max(np.abs(dy))) if m else 0.0) < o.tiny_step_y_tol:
+                st.tiny_flag = True
+            st.tiny_last = True
+            xt = x + a_max * dx
+            return self.accept(st, tr, dict(x=xt, d=d, alpha=a_max, kind="tiny"), mu, tau, ftype=True)
+        st.tiny_last = False
+
+        # Table I row 5: in the soft restoration phase the acceptance criterion is a
+        # reduction of the primal-dual error, until the original criterion holds again or the limit is reached
+        if st.soft:
+            st.soft_count += 1
+            if st.soft_count > o.max_soft_resto_iters:
+                st.soft = False
+                tr["kind"] = "ls_fail"
+                return self.enter_restoration(st, th, tr, fv, cv)
+            return self.soft_step(st, th, tr, d, mu, tau, fv, g, cv, A, theta_k, phi_k, gd)
+
+        # Table I row 3: after watchdog_trigger shortened steps in a row the watchdog wakes up
+        if st.wd is None and o.watchdog_trigger > 0 and st.n_short >= o.watchdog_trigger:
+            st.wd = Watchdog(x=x.copy(), y=y.copy(), zL=st.zL.copy(), zU=st.zU.copy(), d=d,
+                             theta=theta_k, phi=phi_k, gd=gd, alpha=a_max)
+            tr["wd"] = 1
+        if st.wd is not None:
+            wd = st.wd
+            xt = x + a_max * dx
+            ft, ct, theta_t, phi_t = self.trial_point(xt, th, mu)
+            if self.acceptable(st, theta_t, phi_t, wd.theta, wd.phi, wd.alpha, wd.gd):
+                # the watchdog succeeded: the point is acceptable to the entry iterate's criterion
+                ftype = self.switching(wd.alpha, wd.gd, wd.theta) and self.armijo(phi_t, wd.phi, wd.alpha, wd.gd)
+                if not ftype:
+                    st.filt.append(((1.0 - o.gamma_theta) * wd.theta, wd.phi - o.gamma_phi * wd.theta))
+                st.wd, st.n_short = None, 0
+                tr["wd"] = 3
+                tr["augment"] = not ftype
+                return self.accept(st, tr, dict(x=xt, d=d, alpha=a_max, kind="newton"), mu, tau, ftype=ftype)
+            wd.trials += 1
+            if wd.trials <= o.watchdog_trial_max and math.isfinite(theta_t) and math.isfinite(phi_t):
+                if tr["wd"] == 0:
+                    tr["wd"] = 2       # accepted unconditionally
+                return self.accept(st, tr, dict(x=xt, d=d, alpha=a_max, kind="newton"), mu, tau, ftype=True)
+            # the watchdog gives up: back to its entry iterate and direction, ordinary backtracking from there
+            # (the full step of the entry iterate was tried when the watchdog started: skip it; no correction)
+            st.x, st.y, st.zL, st.zU = wd.x, wd.y, wd.zL, wd.zU
+            x, y, d = st.x, st.y, wd.d
+            dx, dy, dzL, dzU = d
+            theta_k, phi_k, gd, a_max = wd.theta, wd.phi, wd.gd, wd.alpha
+            st.wd, st.n_short = None, 0
+            tr["wd"] = 4
+            tr["step"] = d
+            fv, g, cv, A = p.f(x, th), p.grad_f(x, th), p.c(x, th), p.jac(x, th)
+            acc = self.backtrack(st, th, tr, x, d, cv, None, mu, tau, theta_k, phi_k, gd, a_max, skip_first=True)
         else:
-            a_min = o.gamma_alpha * o.gamma_theta
-        alpha, ntrial, acc = a_max, 0, None
+            acc = self.backtrack(st, th, tr, x, d, cv, (fac, W, A, dw, dc, b), mu, tau, theta_k, phi_k, gd, a_max,
+                                 skip_first=False)
+        if acc is None:
+            # the line search failed: first the soft restoration phase (row 5), then the hard one (row 6)
+            if o.soft_resto_factor > 0.0:
+                st.soft, st.soft_count = True, 0
+                st.filt.append(((1.0 - o.gamma_theta) * theta_k, phi_k - o.gamma_phi * theta_k))
+                return self.soft_step(st, th, tr, d, mu, tau, fv, g, cv, A, theta_k, phi_k, gd)
+            tr["kind"] = "ls_fail"
+            return self.enter_restoration(st, th, tr, fv, cv)
+        # A-6 accept, A-7 filter
+        ftype = self.switching(acc["alpha_test"], gd, theta_k) and self.armijo(acc["phi"], phi_k, acc["alpha_test"], gd)
+        if not ftype:
+            st.filt.append(((1.0 - o.gamma_theta) * theta_k, phi_k - o.gamma_phi * theta_k))
+        st.n_short = st.n_short + 1 if tr["ls"] > 0 else 0
+        tr["augment"] = not ftype
+        return self.accept(st, tr, acc, mu, tau, ftype=ftype)
+
+    def backtrack(self, st, th, tr, x, d, cv, lin, mu, tau, theta_k, phi_k, gd, a_max, skip_first):
+        """Backtracking line search with the second-order correction (Table I rows 1-2; A-5).
+        ``lin`` = (factor, W, A, dw, dc, b) for the correction solves, or None (no correction).  Returns the
+        accepted trial (dict) or None when alpha falls below alpha_min."""
+        o = self.o
+        dx = d[0]
+        a_min = self.alpha_min(gd, theta_k, st.theta_min)
+        tr["a_min"] = a_min
+        alpha, ntrial = a_max, 0
+        if skip_first:
+            alpha *= o.alpha_red
+            ntrial = 1
+            if alpha < a_min:
+                tr["ls"] = ntrial
+                return None
+        acc = None
         while True:
             xt = x + alpha * dx
             ft, ct, theta_t, phi_t = self.trial_point(xt, th, mu)
             if self.acceptable(st, theta_t, phi_t, theta_k, phi_k, alpha, gd):
-                acc = dict(x=xt, d=(dx, dy, dzL, dzU), alpha=alpha, alpha_test=alpha, phi=phi_t, kind="newton")
+                acc = dict(x=xt, d=d, alpha=alpha, alpha_test=alpha, phi=phi_t, kind="newton")
                 break
-            if ntrial == 0 and math.isfinite(theta_t) and theta_t >= theta_k and o.max_soc > 0:
+            if (ntrial == 0 and lin is not None and math.isfinite(theta_t) and theta_t >= theta_k
+                    and o.max_soc > 0):
                 # second-order correction (Table I row 2, PAPER.md:130; [7] sec 2.4)
+                fac, W, A, dw, dc, b = lin
                 c_soc = alpha * cv + ct
                 theta_old = theta_k
+                tr["soc_rhs"], tr["soc_steps"] = [], []
                 for psoc in range(1, o.max_soc + 1):
                     bs = [b[0], -c_soc, b[2], b[3]]
-                    ds, _ = self.solve_full(fac, W, A, x, st.zL, st.zU, dw, dc, bs)
+                    ds, _, _ = self.solve_full(fac, W, A, x, st.zL, st.zU, dw, dc, bs)
                     a_soc = self.ftb_primal(x, ds[0], tau)
                     xs = x + a_soc * ds[0]
                     fs, cs, theta_s, phi_s = self.trial_point(xs, th, mu)
                     tr["soc"] = psoc
+                    tr["soc_rhs"].append(c_soc.copy())
+                    tr["soc_steps"].append(tuple(ds))
                     if self.acceptable(st, theta_s, phi_s, theta_k, phi_k, alpha, gd):
                         acc = dict(x=xs, d=tuple(ds), alpha=a_soc, alpha_test=alpha, phi=phi_s, kind="soc")
                         break
@@ -431,22 +632,47 @@ class Solver:
             if alpha < a_min or ntrial > o.max_backtrack:
                 break
         tr["ls"] = ntrial
-        if acc is None:
+        return acc
+
+    def soft_step(self, st, th, tr, d, mu, tau, fv, g, cv, A, theta_k, phi_k, gd):
+        """One step of the soft restoration phase (Table I row 5; reading SR): the same step
+        length for primal and dual variables; accepted if the original criterion holds (then the phase ends) or
+        if the primal-dual error drops by the factor soft_resto_factor; otherwise hard restoration."""
+        o, p = self.o, self.p
+        x, y = st.x, st.y
+        dx, dy, dzL, dzU = d
+        alpha = min(self.ftb_primal(x, dx, tau), self.ftb_dual(st.zL, st.zU, dzL, dzU, tau))
+        xt = x + alpha * dx
+        ft, ct, theta_t, phi_t = self.trial_point(xt, th, mu)
+        ok = math.isfinite(theta_t) and math.isfinite(phi_t)
+        orig = ok and self.acceptable(st, theta_t, phi_t, theta_k, phi_k, 0.0, gd)
+        if ok and not orig:
+            yt, zLt, zUt = y + alpha * dy, st.zL + alpha * dzL, st.zU + alpha * dzU
+            gt, At = p.grad_f(xt, th), p.jac(xt, th)
+            e_t = self.pd_error(xt, yt, zLt, zUt, gt, ct, At, mu)
+            e_k = self.pd_error(x, y, st.zL, st.zU, g, cv, A, mu)
+            ok = math.isfinite(e_t) and e_t <= o.soft_resto_factor * e_k
+        if not ok:
+            st.soft = False
             tr["kind"] = "ls_fail"
             return self.enter_restoration(st, th, tr, fv, cv)
-        # A-6 accept, A-7 filter
+        tr["soft"] = 2 if orig else 1
+        if orig:
+            st.soft, st.soft_count = False, 0
+        st.n_short = 0
+        return self.accept(st, tr, dict(x=xt, d=d, alpha=alpha, kind="soft"), mu, tau, ftype=True, alpha_z=alpha)
+
+    def accept(self, st, tr, acc, mu, tau, ftype, alpha_z=None):
+        """A-6 / A-8: move to the accepted trial point, step the multipliers, safeguard z, count the iteration."""
         dxa, dya, dzLa, dzUa = acc["d"]
-        a_z = self.ftb_dual(st.zL, st.zU, dzLa, dzUa, tau)
-        ftype = self.switching(acc["alpha_test"], gd, theta_k) and self.armijo(acc["phi"], phi_k, acc["alpha_test"], gd)
-        if not ftype:
-            st.filt.append(((1.0 - o.gamma_theta) * theta_k, phi_k - o.gamma_phi * theta_k))
+        a_z = self.ftb_dual(st.zL, st.zU, dzLa, dzUa, tau) if alpha_z is None else alpha_z
         st.x = acc["x"]
-        st.y = y + acc["alpha"] * dya
+        st.y = st.y + acc["alpha"] * dya
         st.zL = st.zL + a_z * dzLa
         st.zU = st.zU + a_z * dzUa
         self.safeguard_z(st, mu)
         st.k += 1  # A-8
-        tr.update(kind=acc["kind"], alpha=acc["alpha"], alpha_z=a_z, ftype=ftype, augment=not ftype)
+        tr.update(kind=acc["kind"], alpha=acc["alpha"], alpha_z=a_z, ftype=ftype)
         return tr
 
     def safeguard_z(self, st: State, mu):
@@ -477,6 +703,8 @@ class Solver:
             return tr
         phi_k = self.phi(st.x, fv, st.mu)
         st.filt.append(((1.0 - o.gamma_theta) * theta_k, phi_k - o.gamma_phi * theta_k))
+        # the regular problem's line-search memory does not survive a restoration phase
+        st.wd, st.n_short, st.soft, st.soft_count, st.tiny_last, st.tiny_flag = None, 0, False, 0, False, False
         mu_bar = max(st.mu, float(np.max(np.abs(cv))))
         rp = RestoNLP(self.p, st.x, o.rho_resto, mu_bar)
         n, m, rho = self.n, self.m, o.rho_resto
