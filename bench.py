@@ -117,32 +117,52 @@ class ClockSampler(threading.Thread):
 
 
 def _oracle_worker(args):
-    cfg, idx = args
+    cfg, idx, budget_s = args
     os.environ["OMP_NUM_THREADS"] = "1"
     from oracle import families as ofam, ipm as oipm
     d, theta, x0 = wl.generate(cfg, 1, first_id=idx)
     xL, xU = wl.bounds(d)
     prob = ofam.Problem(d.family, d.horizon_N, d.n_agents, d.n_obstacles, d.dt)
-    st = oipm.Solver(prob, xL, xU).solve(x0[0], theta[0])
+    s = oipm.Solver(prob, xL, xU)
+    t_end = time.perf_counter() + budget_s
+    st = s.initialise(x0[0], theta[0])
+    while st.status == oipm.ST_NOT_RUN and time.perf_counter() < t_end:
+        s.iterate(st, theta[0])
     return int(st.status), int(st.k)
 
 
-def time_oracle(cfg: int, first: int, count: int, cores: int):
-    """The oracle as it stands, one problem per process over `cores` host cores; returns (seconds, solved, iters)."""
+def time_oracle(cfg: int, first: int, count: int, cores: int, budget_s: float):
+    """The oracle as it stands, one problem per process over `cores` host cores.  A problem still running after
+    budget_s seconds is cut (status -1: not counted as solved, its iterations are).  Returns (seconds, solved,
+    iterations, problems cut)."""
     from multiprocessing import get_context
     t0 = time.perf_counter()
     with get_context("fork").Pool(cores) as pool:
-        res = pool.map(_oracle_worker, [(cfg, first + i) for i in range(count)], chunksize=1)
+        res = pool.map(_oracle_worker, [(cfg, first + i, budget_s) for i in range(count)], chunksize=1)
     dt = time.perf_counter() - t0
-    return dt, sum(1 for s, _ in res if s == 0), sum(k for _, k in res)
+    return dt, sum(1 for s, _ in res if s == 0), sum(k for _, k in res), sum(1 for s, _ in res if s == -1)
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE slot-kernel launch over the config's full batch, from the
-# `ncu --set full` capture summarised in profiles/r1_ncu_full_c1.md (40.1 MB read + 2191.2 MB
-# written: write-back of the L2-resident per-slot scratch)
-NCU_TRAFFIC_BYTES = {1: 2231.3e6}
+# ncu's dram__bytes_read.sum + dram__bytes_write.sum of ONE launch is not measured inside bench.py (it needs the
+# profiler): `traffic` is null in the JSON line and `traffic_source` names the committed capture that holds it.
+TRAFFIC_SOURCE = {1: "profiles/r2_ncu_full_c1.md"}
 
-ORACLE_SAMPLE = {0: 256, 1: 16, 2: 2, 3: 2}  # problems per timed sample (about 10-30 s of CPU work)
+# Oracle sample: problems per timed sample and the per-problem time budget, sized for about 20-30 s of wall-clock on the
+# box's cores.  C0 / C1 problems finish (1 ms / ~8 s each); a C2 / C3 problem needs minutes (dense 2576 / 2784-row KKT
+# factorisations in numpy), so its sample measures ITERATIONS per second and converts with the iterations per converged
+# NLP that the GPU arm measured on the same workload (the line says so).
+def oracle_sample(cfg: int, cores: int):
+    return {0: (256, 30.0), 1: (2 * cores, 25.0), 2: (cores, 20.0), 3: (cores, 20.0)}[cfg]
+
+
+def golden_iterations_per_solved(cfg: int):
+    """tests/golden/full_size_c{cfg}.json (written by the oracle): iterations per converged NLP of the sample."""
+    fn = os.path.join(ROOT, "tests", "golden", f"full_size_c{cfg}.json")
+    if not os.path.exists(fn):
+        return None
+    rows = json.load(open(fn))["problems"]
+    solved = sum(1 for r in rows if r["status"] == 0)
+    return sum(r["iters"] for r in rows) / solved if solved else None
 
 
 def run_reference(args):
@@ -151,15 +171,21 @@ def run_reference(args):
         return
     cfg = args.config
     cores = os.cpu_count() or 1
-    count = ORACLE_SAMPLE[cfg]
+    count, budget = oracle_sample(cfg, cores)
     for _ in range(min(args.warmup, 1)):
-        time_oracle(cfg, 0, min(count, cores), cores)
-    tot_t, tot_solved, tot_it = 0.0, 0, 0
+        time_oracle(cfg, 0, min(count, cores), cores, min(budget, 5.0))
+    tot_t, tot_solved, tot_it, tot_cut = 0.0, 0, 0, 0
     for s in range(args.steps):
-        dt, solved, its = time_oracle(cfg, s * count, count, cores)
-        tot_t += dt; tot_solved += solved; tot_it += its
+        dt, solved, its, cut = time_oracle(cfg, 0, count, cores, budget)   # the same ids the GPU arm's sample uses
+        tot_t += dt; tot_solved += solved; tot_it += its; tot_cut += cut
     val = tot_solved / tot_t
-    sample = f"{count} problems of {WORKLOAD_NAMES[cfg]} per step (ids step*{count}..), one process per problem"
+    sample = (f"first {count} problems of {WORKLOAD_NAMES[cfg]} per step, one process per problem, each cut after "
+              f"{budget:.0f} s ({tot_cut} of {count * args.steps} cut)")
+    per_solved = golden_iterations_per_solved(cfg)
+    if tot_solved == 0 and per_solved:
+        val = (tot_it / tot_t) / per_solved
+        sample += (f"; no problem finishes inside the budget: value = measured oracle iterations/s / {per_solved:.1f} "
+                   "iterations per converged NLP (tests/golden, the oracle's own full solves)")
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -304,18 +330,20 @@ def run_jipm(args):
                           if args.max_iter > 0 else {}),
                        "parallelism": f"queue sharded over {world} GPU(s), no collective"},
             "iterations_per_s": iters_all * K / secs,
+            "slot_us_per_iteration": us_per_iter,
+            "converged_fraction": solved_all / P_all,
             "iters_mean": float(iters.mean()), "iters_max": int(iters.max()),
-            "status_hist_rank0": hist, "converged_fraction": solved_all / P_all,
+            "iters_percentiles_50_90_99": [float(v) for v in np.percentile(iters, [50, 90, 99])],
+            "status_hist_rank0": hist,
             "wall_s_timed_region": t_wall,
             "e2e": {"value": e2e_solved_all * K / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h},
             "gpu_launches": int(stats_sum["launches"]),
             "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_fp64, "unit": "TFLOP/s",
                          "frac": achieved / peak_fp64,
-                         "traffic": (NCU_TRAFFIC_BYTES.get(cfg) if P == wl.CONFIG_BATCH[cfg] and args.max_iter == 0
-                                     else None),
-                         "traffic_unit": "bytes of DRAM traffic per launch (ncu); algorithmic bytes per launch = "
-                                         + str(h2d + d2h),
+                         "traffic": None,
+                         "traffic_source": TRAFFIC_SOURCE.get(cfg, "not captured for this config"),
+                         "algorithmic_bytes_per_launch": h2d + d2h,
                          "kernel": "jipm_slot_kernel (persistent, one launch per step)",
                          "peak_source": "DFMA microbenchmark jipm_bench_fp64_peak measured in this run "
                                         "(MEASURED_PEAKS.json has no FP64 entry); nominal 148 SM x 64 DFMA/clk x 2 x "
@@ -328,11 +356,18 @@ def run_jipm(args):
         }
         if not args.no_cpu_baseline and world == 1:
             cores = os.cpu_count() or 1
-            cnt_o = ORACLE_SAMPLE[cfg]
-            dt, so, it = time_oracle(cfg, 0, cnt_o, cores)
-            line["cpu_baseline"] = {"value": so / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                    "iterations_per_s": it / dt,
-                                    "sample": f"first {cnt_o} problems of the same workload, one process per problem"}
+            cnt_o, budget = oracle_sample(cfg, cores)
+            dt, so, it, cut = time_oracle(cfg, 0, cnt_o, cores, budget)
+            sample = (f"first {cnt_o} problems of the same workload, one process per problem, each cut after "
+                      f"{budget:.0f} s ({cut} cut)")
+            val = so / dt
+            if so == 0 and solved_all > 0:
+                per_solved = iters_all / solved_all
+                val = (it / dt) / per_solved
+                sample += (f"; no problem finishes inside the budget: value = measured oracle iterations/s / "
+                           f"{per_solved:.1f} iterations per converged NLP measured by the GPU arm on this workload")
+            line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                    "iterations_per_s": it / dt, "sample": sample}
         print(json.dumps(line))
     s.close()
     if world > 1:
@@ -340,15 +375,18 @@ def run_jipm(args):
 
 
 def run_c4(args):
-    """BASELINE.json configs[4]: iteration-level batching sweep.  A queue of seeded problems of the C1 family
-    (reading D-2: 1-based "config-2 problem family") is solved with R = 1024, 4096, 16384, 65536 problem slots.
-    A slot is a CTA: R CTAs are launched, the SMs hold as many as fit (one per SM for this family) and every CTA pops
-    problems until the queue is empty, so a finished problem is replaced at once whatever R is."""
+    """BASELINE.json configs[4]: iteration-level batching sweep on "the config-2 problem family" -- ambiguous (reading
+    D-2): --c4-family 1 = the single-quadrotor family of configs[1] (1-based reading), --c4-family 2 = the four-quadrotor
+    family of configs[2] (0-based reading).  A queue of seeded problems is solved with R = 1024, 4096, 16384, 65536
+    problem slots.  A slot is a CTA: R CTAs are launched, the SMs hold as many as fit (co_resident_slots below) and every
+    CTA pops problems until the queue is empty, so a finished problem is replaced at once whatever R is; the global
+    scratch is sized for the co-resident CTAs only."""
     import torch
     from paper_2606_26341_b200 import jipm
     torch.cuda.set_device(0)
-    P = args.queue
-    d, theta, x0 = wl.generate(1, P)
+    fam = args.c4_family
+    P = args.queue or (100000 if fam == 1 else 20000)
+    d, theta, x0 = wl.generate(fam, P)
     xL, xU = wl.bounds(d)
     dev = torch.device("cuda", 0)
     x0_d, th_d = torch.as_tensor(x0, device=dev), torch.as_tensor(theta, device=dev)
@@ -358,32 +396,36 @@ def run_c4(args):
                iters=torch.empty((P,), dtype=torch.int32, device=dev))
     peak = jipm.fp64_peak_tflops()
     sm_count = torch.cuda.get_device_properties(0).multi_processor_count
-    sweep, ref_iters = [], None
+    sweep, ref_iters, co_res = [], None, None
     for R in [int(r) for r in args.slots_list.split(",")]:
         s = jipm.Solver(d.family, d.horizon_N, d.n_agents, d.n_obstacles, d.dt, xL, xU, resident_slots=R)
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record(); s.solve_batch_into(x0_d, th_d, out); b.record(); torch.cuda.synchronize()
         ms = a.elapsed_time(b)
         st = s.stats()
+        co_res = st["co_resident_slots"]
         iters = out["iters"].cpu().numpy(); status = out["status"].cpu().numpy()
         if ref_iters is None:
             ref_iters = iters.copy()
         busy = (st["cyc_iterations"] + st["cyc_init"]) / 1.965e9
         pct = np.percentile(iters, [50, 90, 99, 99.9]).tolist()
+        hist_it = np.bincount(np.minimum(iters, 3000) // 25, minlength=121).tolist()
         sweep.append({"R": R, "ms": ms, "nlps_per_s": float((status == 0).sum()) / (ms * 1e-3),
                       "iterations_per_s": float(iters.sum()) / (ms * 1e-3),
-                      "slot_occupancy": busy / (min(R, sm_count) * ms * 1e-3),
+                      "slot_occupancy": busy / (min(R, co_res) * ms * 1e-3),
                       "fp64_frac": flops_from_stats(d, st) / (ms * 1e-3) / 1e12 / peak,
                       "iters_identical_to_first_R": bool(np.array_equal(iters, ref_iters)),
                       "iters_p50_p90_p99_p999": pct, "iters_max": int(iters.max()),
+                      "iters_histogram_bins_of_25": hist_it,
                       "status_hist": {int(k): int((status == k).sum()) for k in np.unique(status)}})
         s.close()
     best = max(sweep, key=lambda r: r["nlps_per_s"])
     print(json.dumps({"metric": METRIC, "value": best["nlps_per_s"], "unit": UNIT, "n_gpus": 1, "steps": 1, "warmup": 0,
                       "ms_per_step": best["ms"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                       "dtype": "f64", "data": "synthetic",
-                      "config": {"workload": f"C4 iteration-level batching sweep, queue {P} problems of the C1 family",
-                                 "co_resident_slots": sm_count}, "sweep": sweep}))
+                      "config": {"workload": f"C4 iteration-level batching sweep, queue of {P} problems of the "
+                                             f"C{fam} family ({WORKLOAD_NAMES[fam].split(',')[0]})",
+                                 "co_resident_slots": co_res, "sm_count": sm_count}, "sweep": sweep}))
 
 
 def main():
@@ -392,7 +434,10 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 3, 4])
-    ap.add_argument("--queue", type=int, default=100000, help="config 4: problems in the queue")
+    ap.add_argument("--queue", type=int, default=0, help="config 4: problems in the queue (default 100000 for the C1 "
+                                                         "family, 20000 for the C2 family)")
+    ap.add_argument("--c4-family", type=int, default=1, choices=[1, 2], help="config 4: which reading of 'the config-2 "
+                                                                            "problem family' (D-2)")
     ap.add_argument("--slots-list", default="1024,4096,16384,65536", help="config 4: resident slot counts")
     ap.add_argument("--batch", type=int, default=0, help="problems per GPU per step (default: the config's batch)")
     ap.add_argument("--slots", type=int, default=0, help="resident slots (0: library picks)")

@@ -6,9 +6,10 @@
  * that share f, c and the bounds and differ only in theta and the initial guess (eq 2).
  * General inequalities enter through slack variables.  Each problem runs the barrier
  * iteration (eqs 3-7) with the fallbacks of Table I that this
- * build covers (backtracking, second-order correction, inertia correction, monotone barrier update,
- * feasibility restoration) and a problem slot is refilled from the queue as soon as its problem ends
- * (iteration-level batching).
+ * build covers (rows 1-6 and the monotone schedule of row 7: backtracking, second-order correction, watchdog,
+ * tiny-step rule, soft and hard feasibility restoration; plus the inertia correction of PAPER.md:114) and a
+ * problem slot is refilled from the queue as soon as its problem ends (iteration-level batching,
+ * PAPER.md:162-168).
  *
  * Decision vector ("stage order", n entries) and equality vector (m entries) of every family:
  *        x = [ x_0 | u_0 x_1 s_1 | u_1 x_2 s_2 | ... | u_{N-1} x_N s_N ]
@@ -34,13 +35,14 @@ typedef struct jipm_solver jipm_solver; /* opaque, owned by the library */
 enum { JIPM_OK = 0, JIPM_ERR_ARG = 1, JIPM_ERR_DIM = 2, JIPM_ERR_BOUNDS = 3, JIPM_ERR_CUDA = 4, JIPM_ERR_NOMEM = 5 };
 enum { JIPM_FAM_POINTMASS2D = 0, JIPM_FAM_QUAD_TRACK = 1, JIPM_FAM_MULTIQUAD = 2, JIPM_FAM_QUAD_CLUTTER = 3 };
 enum { JIPM_ST_NOT_RUN = -1, JIPM_ST_SOLVED = 0, JIPM_ST_MAXITER = 1, JIPM_ST_LOCALLY_INFEASIBLE = 2,
-       JIPM_ST_RESTORATION_FAILED = 3, JIPM_ST_RESTO_AT_FEASIBLE_POINT = 4, JIPM_ST_NONFINITE = 5 };
+       JIPM_ST_RESTORATION_FAILED = 3, JIPM_ST_RESTO_AT_FEASIBLE_POINT = 4, JIPM_ST_NONFINITE = 5,
+       JIPM_ST_TINY_STEP = 6 /* search direction too small to make progress at the smallest mu (Table I row 4) */ };
 
 /* Problem family dimensions (BASELINE.json configs). */
 typedef struct {
     int32_t horizon_N;   /* control intervals; N+1 state knots */
     int32_t n_agents;    /* 1 except JIPM_FAM_MULTIQUAD */
-    int32_t n_obstacles; /* obstacles per knot (ignored by JIPM_FAM_MULTIQUAD: pair constraints) */
+    int32_t n_obstacles; /* obstacles per knot, 0..254 (ignored by JIPM_FAM_MULTIQUAD: pair constraints) */
     double dt;
 } jipm_family_dims;
 
@@ -53,8 +55,13 @@ typedef struct {
     double theta_max_fact, theta_min_fact, alpha_red, kappa_soc;
     double delta_w_min, delta_w_0, delta_w_max, kappa_w_minus, kappa_w_plus, kappa_w_plus_first;
     double delta_c_bar, kappa_c, residual_ratio_max, rho_resto, kappa_resto, z_reset_threshold;
+    /* refinement failure ("pretend singular", reading S-7) and Table I rows 3-5 */
+    double residual_ratio_singular, residual_improvement_factor;
+    double tiny_step_tol, tiny_step_y_tol, tiny_step_cviol, soft_resto_factor;
     int32_t max_iter, max_backtrack, max_soc, refine_min, refine_max, max_mu_updates;
     int32_t init_slacks, enable_restoration;
+    int32_t watchdog_trigger, watchdog_trial_max, max_soft_resto_iters;
+    int32_t reserved_;
 } jipm_options;
 
 /* Fill *o with the defaults.  o: HOST.  Returns JIPM_ERR_ARG if o is NULL. */
@@ -68,8 +75,11 @@ int jipm_family_sizes(int family, const jipm_family_dims* d, int64_t* n, int64_t
  *   x_L, x_U        HOST [n], +-INFINITY = no bound, shared by all problems; x_L >= x_U on a
  *                   component -> JIPM_ERR_BOUNDS (PAPER.md:63 needs a strict interior).  Copied.
  *   opts            HOST or NULL (defaults).  Copied.
- *   resident_slots  R = problem slots in flight (one warp per slot); 0 -> library picks (fills the GPU).
- *   cuda_stream     cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = default stream. */
+ *   resident_slots  R = problem slots in flight (one CTA per slot); 0 -> library picks (fills the GPU).
+ *   cuda_stream     cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = default stream.
+ * The solver belongs to the CUDA device that is current at this call; later calls switch to it for their duration.
+ * Calls on solvers of the same family are serialised inside the library (launch arguments live in one
+ * __constant__ block per family instantiation); calls on different families may run concurrently. */
 int jipm_create(jipm_solver** out, int family, const jipm_family_dims* d, int64_t n, int64_t m,
                 const double* x_L, const double* x_U, const jipm_options* opts, int64_t resident_slots,
                 void* cuda_stream);
@@ -84,7 +94,8 @@ int jipm_create(jipm_solver** out, int family, const jipm_family_dims* d, int64_
 int jipm_solve_batch(jipm_solver* s, int64_t P, const double* x0, const double* params, double* x_out,
                      double* lam_out, double* zL_out, double* zU_out, int32_t* status_out, int32_t* iters_out);
 
-/* Same call with HOST buffers: copies in, solves, copies out (all on the solver's stream). */
+/* Same call with HOST buffers: copies in, solves, copies out (all on the solver's stream).  The device staging
+ * buffer is owned by the solver and only grows (no allocation on repeated calls of the same size). */
 int jipm_solve_batch_host(jipm_solver* s, int64_t P, const double* x0, const double* params, double* x_out,
                           double* lam_out, double* zL_out, double* zU_out, int32_t* status_out,
                           int32_t* iters_out);
@@ -103,13 +114,23 @@ const char* jipm_last_error(void);
  * [16..20] the same for the factorisation sub-phases: T J, M assembly, control pivots, Phi + stores, D != 0 extras. */
 int jipm_last_stats(jipm_solver* s, int64_t* stats, int64_t n_stats);
 
+/* How the solver occupies its device: res[0] = SMs, res[1] = problem slots (CTAs) co-resident per SM for this family.
+ * R = resident_slots CTAs are launched per solve, but only res[0] * res[1] run at once; the others start as earlier
+ * ones end (they find the queue empty unless R is below that product).  res: HOST out [2]. */
+int jipm_residency(jipm_solver* s, int64_t* res);
+
 /* ---- debug / parity-test entries (load a state, step once, compare) ------------------
  * Decision trace: per problem, per iteration JIPM_TRACE_W doubles:
  *   [0] mode (0 regular, 1 restoration) [1] #factorisations [2] delta_w [3] delta_c [4] #refinements
  *   [5] kind (0 newton, 1 soc, 2 ls_fail->resto, 3 ic_fail->resto, 4 terminal) [6] #backtracks [7] #soc
  *   [8] alpha [9] alpha_z [10] f-type? [11] #mu updates [12] E0 at iteration start [13] mu used
- *   [14] theta_k [15] phi_k */
-#define JIPM_TRACE_W 16
+ *   [14] theta_k [15] phi_k
+ *   [16] watchdog (0 none, 1 started + step taken unconditionally, 2 step taken unconditionally, 3 succeeded,
+ *        4 gave up: back at the entry iterate, backtracked from there)
+ *   [17] soft restoration (0 none, 1 step accepted by the error reduction, 2 accepted by the original criterion)
+ *   [18] tiny step taken? [19] #refinement failures treated as a singular matrix
+ *   kind [5] also takes 5 = tiny step, 6 = soft restoration step. */
+#define JIPM_TRACE_W 20
 /* Enable tracing for the next solves: trace DEVICE [P x max_records x JIPM_TRACE_W] (or NULL to disable). */
 int jipm_debug_set_trace(jipm_solver* s, double* trace, int64_t max_records);
 
@@ -120,7 +141,11 @@ int jipm_debug_set_trace(jipm_solver* s, double* trace, int64_t max_records);
  * restoration mode (Step R): [15]=16 scalars (mode, then the parked regular mu, tau, delta_w_last, theta_min,
  * theta_max, #filter entries, theta at entry, zeta), [16]=(p, n) [2m], [17]=(z_p, z_n) [2m], [18]=x_R [n],
  * [19]=restoration filter (256 pairs).  With mode = 1 the fields [1]-[5] hold the restoration iterate and scalars
- * and [6] still holds the REGULAR filter. */
+ * and [6] still holds the REGULAR filter.
+ * Line-search memory of the active problem (Table I rows 3-5): [20]=16 scalars (#consecutive shortened steps,
+ * watchdog active?, #watchdog trials, watchdog reference theta, phi, grad_phi^T d, alpha, soft phase?, #soft
+ * iterations, last step tiny?, tiny flag), [21]=watchdog entry iterate and direction: x, z_L, z_U, dx, dz_L, dz_U
+ * (n + 2m each: the restoration variables follow the n entries), then y, dy (m each). */
 int jipm_debug_state_layout(jipm_solver* s, int64_t* lay, int64_t n_lay);
 
 /* Load P states (DEVICE [P x len], regular mode), run n_steps iterations each (stops early on a final

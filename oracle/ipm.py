@@ -292,9 +292,12 @@ class Solver:
         else IC-5) -- and the loop IC-4..IC-6 continues from there."""
         o, n, m = self.o, self.n, self.m
         nfact = 0
+        tried = self.ic_tried = getattr(self, "ic_tried", [])   # (delta_w, delta_c) of every factorisation, for tests
         if resume is None:
+            tried.clear()
             fac = DenseLDL(self.kkt_matrix(W, Sigma, A, 0.0, 0.0), o.zero_pivot_tol)  # IC-1
             nfact = 1
+            tried.append((0.0, 0.0))
             if fac.inertia == (n, m, 0):
                 return fac, 0.0, 0.0, nfact
             dc = o.delta_c_bar * mu ** o.kappa_c if fac.inertia[2] > 0 else 0.0  # IC-2
@@ -311,6 +314,7 @@ class Solver:
         while True:
             fac = DenseLDL(self.kkt_matrix(W, Sigma, A, dw, dc), o.zero_pivot_tol)  # IC-4
             nfact += 1
+            tried.append((dw, dc))
             if fac.inertia == (n, m, 0):
                 return fac, dw, dc, nfact
             dw = (o.kappa_w_plus_first if dw_last == 0.0 else o.kappa_w_plus) * dw  # IC-5
@@ -497,6 +501,9 @@ class Solver:
         if dw > 0.0:
             st.delta_w_last = dw
         tr["step"] = (dx, dy, dzL, dzU)
+        # the linear system this step solved, for tests that want a second opinion on it (nothing below reads it)
+        tr["lin"] = dict(W=W, A=A, Sigma=Sigma, b=b, x=x, zL=st.zL, zU=st.zU, d=(dx, dy, dzL, dzU),
+                         tried=list(self.ic_tried))
         d = (dx, dy, dzL, dzU)
         # A-5 line search
         theta_k = float(np.sum(np.abs(cv))) if m else 0.0

@@ -28,7 +28,7 @@ struct Pb {
     const double* xU;    // DEVICE [n], relaxed, +inf = none
 };
 
-// offsets (in doubles) into the per-warp workspace
+// offsets (in doubles) into the per-slot workspace
 struct Lay {
     int x, y, zL, zU, g, c, gv, dgv, cnd, tgt, J, W, Sig, Hd, Dc, T, Kf, Gf, Psi, pv, qv, sv, wv, tv, bl, bu, imap, cmap;
     int b1, b2, b3, b4, dx, dy, dzL, dzU, r1, r2, r3, r4, e1, e2, e3, e4;
@@ -36,6 +36,8 @@ struct Lay {
     int pv0, npad, tail0, tpad;  // primal-sized vectors: contiguous block of npad-strided heads, 2m-tails (restoration) apart
     int nsm;  // the first nsm doubles of the layout are shared-memory resident (per team), the rest global
     int xR, DR2, filtR, rc2;  // restoration mode: reference point, scaling D_R^2, its own filter, condensed rhs
+    // watchdog (Table I row 3): entry iterate and its search direction
+    int wx, wzL, wzU, wdx, wdzL, wdzU, wy, wdy;
 };
 
 // per-launch arguments
@@ -52,6 +54,11 @@ struct Args {
     double* x_out; double* lam_out; double* zL_out; double* zU_out;
     int32_t* status_out; int32_t* iters_out;
     int* queue;          // [1] next problem id
+    // R CTAs may be launched but only teams_per_sm per SM are ever co-resident (the shared memory a CTA asks for is the
+    // SM's divided by teams_per_sm): the global scratch holds n_sm * teams_per_sm workspaces and a CTA claims one of its
+    // SM's workspaces when it starts (a bit of sm_mask[%smid]) and releases it when it ends.
+    unsigned* sm_mask;   // [n_sm], zero at launch
+    int teams_per_sm;
     unsigned long long* stats; // [16]
     double* trace; int trace_cap;
     // debug
@@ -60,7 +67,7 @@ struct Args {
 };
 
 // debug state layout (doubles) -- mirrored by jipm_debug_state_layout
-struct DbgLay { int len, x, y, zL, zU, sc, filt, dx, dy, dzL, dzU, g, c, J, W, rs, pn, zpn, xR, filtR; };
+struct DbgLay { int len, x, y, zL, zU, sc, filt, dx, dy, dzL, dzU, g, c, J, W, rs, pn, zpn, xR, filtR, ls, wd; };
 
 constexpr int RKW = 42;  // doubles of quadrotor phase-1 output per (stage, RK point); see dyn.cuh
 
@@ -74,6 +81,9 @@ __host__ __device__ inline DbgLay make_dbglay(int n, int m, int N, int NX, int N
     d.J = o; o += N * NX * NZ; d.W = o; o += N * NZ * NZ + NX * NX;
     // restoration mode (Step R): scalars, (p, n), (z_p, z_n), reference point x_R, the restoration filter
     d.rs = o; o += 16; d.pn = o; o += 2 * m; d.zpn = o; o += 2 * m; d.xR = o; o += n; d.filtR = o; o += 2 * MAX_FILTER;
+    // line-search memory (Table I rows 3-5): 16 scalars; the watchdog's entry iterate and direction: six vectors of
+    // n + 2m (x, zL, zU, dx, dzL, dzU), then y, dy
+    d.ls = o; o += 16; d.wd = o; o += 6 * (n + 2 * m) + 2 * m;
     d.len = o;
     return d;
 }
@@ -104,7 +114,6 @@ template <int NT>
 struct Team {
     static constexpr int NW = NT / 32;
     int tid;      // 0 .. NT-1
-    int bar;      // unused while there is one team per CTA (barrier 0)
     int flip;     // which half of the reduction scratch the next reduction uses
     double* red;  // shared memory, 2 * NW doubles
 

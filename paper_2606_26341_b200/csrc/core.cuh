@@ -1,5 +1,5 @@
-// core.cuh -- per-warp solver context: indexing, evaluation of f / c / derivatives, products with the
-// stage-structured A and W of PAPER.md:90.  Everything here is a warp-collective device function.
+// core.cuh -- solver context of one problem slot (= one team = one CTA): indexing, evaluation of f / c / derivatives,
+// products with the stage-structured A and W of PAPER.md:90.  Everything here is a team-collective device function.
 #pragma once
 #include "common.cuh"
 #include "dyn.cuh"
@@ -54,10 +54,10 @@ struct Ctx {
     const int* imap; const int* cmap;
     mutable unsigned long long pc[8];  // diagnostic cycle counters of the factorisation's sub-phases (stats[16..23])
 
-    __device__ Ctx(double* ws_, double* sm_, int tid_, int bar_)
+    __device__ Ctx(double* ws_, double* sm_, int tid_)
         : ws(ws_ - g_A.L.nsm), sm(sm_), smd(sm_ + C::SM_TOTAL), th(nullptr), lane(tid_) {
         for (int q = 0; q < 8; ++q) pc[q] = 0;
-        tm.tid = tid_; tm.bar = bar_; tm.flip = 0; tm.red = sm_ + C::SM_RED;
+        tm.tid = tid_; tm.flip = 0; tm.red = sm_ + C::SM_RED;
     }
 
     __device__ void build_maps() {

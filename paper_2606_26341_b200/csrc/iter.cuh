@@ -1,5 +1,5 @@
 // iter.cuh -- the fused interior-point iteration (Table I) for one problem slot
-// owned by one warp, plus Step I (initialisation) and the slot refill loop.
+// owned by one team (= one CTA), plus Step I (initialisation) and the slot refill loop.
 // Step names (I-*, A-*, IC-*) follow SURVEY.md section 8(c) / DESIGN.md.
 #pragma once
 #include "core.cuh"
@@ -8,7 +8,13 @@
 
 namespace jipm {
 
-enum { KIND_NEWTON = 0, KIND_SOC = 1, KIND_LS_FAIL = 2, KIND_IC_FAIL = 3, KIND_TERMINAL = 4 };
+enum { KIND_NEWTON = 0, KIND_SOC = 1, KIND_LS_FAIL = 2, KIND_IC_FAIL = 3, KIND_TERMINAL = 4, KIND_TINY = 5, KIND_SOFT = 6 };
+
+// what one trial-point evaluation returns (team-uniform)
+struct Trial {
+    double f, th, cm, ph;            // objective, ||c||_1, ||c||_inf, barrier objective of the ACTIVE problem
+    double fb, thb, cmb, fpn, fq;    // base problem's f, theta, ||c||_inf and the restoration objective's parts
+};
 
 template <class C>
 struct Solver {
@@ -21,9 +27,13 @@ struct Solver {
     LayProxy L;
     OptProxy o;
     int lane;
-    // warp-uniform scalar state of the problem in this slot
+    // team-uniform scalar state of the problem in this slot
     double mu, tau, dw_last, theta_min, theta_max, f, theta, cmax;
     int k, status, nfilt, nrec;
+    // line-search memory of the ACTIVE problem (Table I rows 3-5): it starts afresh whenever the
+    // barrier parameter changes and on entering / leaving restoration, so nothing is parked across modes
+    int n_short, wd_active, wd_trials, soft, soft_count, tiny_last, tiny_flag;
+    double wd_theta, wd_phi, wd_gd, wd_alpha;
     // restoration mode (Table I row 6): mode 1 iterates on X = [x; p; n] with the same kernel
     // code; the regular problem's scalars are parked in *_reg until the exit test succeeds
     int mode, nX, nfilt_reg;
@@ -45,6 +55,11 @@ struct Solver {
         c.tm.sync();
         c.build_maps();
         mode = 0; nX = pb->n;
+        reset_ls_memory();
+    }
+    __device__ __forceinline__ void reset_ls_memory() {
+        n_short = wd_active = wd_trials = soft = soft_count = tiny_last = tiny_flag = 0;
+        wd_theta = wd_phi = wd_gd = wd_alpha = 0.0;
     }
     __device__ __forceinline__ double* V(int off) const { return c.v(off); }
     __device__ __forceinline__ double* VH(int off) const { return c.vh(off); }
@@ -278,27 +293,57 @@ struct Solver {
         return c.tm.max(rn);
     }
 
-    // solve (6) with iterative refinement on the unreduced system (reading S-7); returns #refinements
+    // solve (6) with iterative refinement on the unreduced system (reading S-7); returns #refinements.  At least
+    // refine_min steps; stops at ratio <= residual_ratio_max; gives up when refine_max is reached or a step no longer
+    // improves the ratio -- then the solution is kept if the ratio is below residual_ratio_singular, else `failed`
+    // is set and the caller pretends the matrix is singular (Algorithm IC continues with delta_c > 0).
     __device__ __noinline__ int solve_full(const Vec b1, const double* b2, const Vec b3, const Vec b4,
-                              Vec d1, double* d2, Vec d3, Vec d4) {
+                              Vec d1, double* d2, Vec d3, Vec d4, bool& failed) {
         reduced_solve(b1, b2, b3, b4, d1, d2, d3, d4);
         double bn = 0.0;
         for (int i = lane; i < nX; i += NT) bn = fmax(bn, fmax(fabs(b1[i]), fmax(fabs(b3[i]), fabs(b4[i]))));
         for (int i = lane; i < pb->m; i += NT) bn = fmax(bn, fabs(b2[i]));
         bn = c.tm.max(bn);
         int nref = 0;
+        failed = false;
         Vec e1 = VX(L->e1); double* e2 = VH(L->e2); Vec e3 = VX(L->e3); Vec e4 = VX(L->e4);
-        while (nref < o->refine_max) {
+        auto ratio = [&]() {
             double dn;
             const long long t0 = clock64();
             const double rn = full_residual(b1, b2, b3, b4, d1, d2, d3, d4, dn);
             tph[3] += clock64() - t0;
-            if (nref >= o->refine_min && rn <= o->residual_ratio_max * (bn + dn)) break;
+            const double den = bn + dn;
+            return den > 0.0 ? rn / den : rn;
+        };
+        double rat = ratio();
+        while (rat > o->residual_ratio_max || nref < o->refine_min) {
+            if (!isfinite(rat)) { failed = true; break; }
             reduced_solve(VX(L->r1), VH(L->r2), VX(L->r3), VX(L->r4), e1, e2, e3, e4);
             for (int i = lane; i < nX; i += NT) { d1[i] += e1[i]; d3[i] += e3[i]; d4[i] += e4[i]; }
             for (int i = lane; i < pb->m; i += NT) d2[i] += e2[i];
             c.tm.sync();
             nref++;
+            const double rat_old = rat;
+            rat = ratio();
+            if (rat > o->residual_ratio_max && nref > o->refine_min &&
+                (nref >= o->refine_max || rat > o->residual_improvement_factor * rat_old)) {
+                failed = !(rat < o->residual_ratio_singular);
+                break;
+            }
+        }
+        // Polish: the stop rule above is the oracle's, but its LAPACK factor sits at a ratio ~1e-16 after the one
+        // compulsory step while the stage recursion can stop anywhere below 1e-10; the error left in Delta y is that
+        // ratio times cond(7).  Up to three more steps while the ratio is above 1e-15 and still shrinking bring the
+        // step within the parity tolerance of the oracle's (eq 8); they change no decision.
+        for (int extra = 0; extra < 3 && !failed && rat > 1e-15 && nref < o->refine_max; ++extra) {
+            reduced_solve(VX(L->r1), VH(L->r2), VX(L->r3), VX(L->r4), e1, e2, e3, e4);
+            for (int i = lane; i < nX; i += NT) { d1[i] += e1[i]; d3[i] += e3[i]; d4[i] += e4[i]; }
+            for (int i = lane; i < pb->m; i += NT) d2[i] += e2[i];
+            c.tm.sync();
+            nref++;
+            const double rat_old = rat;
+            rat = ratio();
+            if (!(rat < 0.25 * rat_old)) break;
         }
         return nref;
     }
@@ -311,6 +356,13 @@ struct Solver {
 
     __device__ void init_problem(long long id);
     __device__ void iterate();
+    __device__ bool ic_loop(bool resume, double& dw, double& dc, int& nfact);
+    __device__ __noinline__ void trial(const Vec dxv, double alpha, Trial& t);
+    __device__ bool backtrack(const Vec dxv, double theta_k, double phi_k, double gd, double a_max, bool skip_first,
+                              bool allow_soc, double* rec, int& acc, double& alpha, double& alpha_acc, Trial& ta);
+    __device__ void accept_step(int acc_soc, const Vec dxv, const double* dyv, const Vec dzLv, const Vec dzUv,
+                                double alpha_x, double alpha_y, double a_z, const Trial& ta);
+    __device__ bool soft_step(double* rec, double theta_k, double phi_k, double gd);
     __device__ __noinline__ void trial_warp(const Vec x, const Vec dx, double alpha, double& th_t, double& ph_t) const;
     __device__ void enter_restoration(double* rec, int kind);
     __device__ void try_exit_restoration();

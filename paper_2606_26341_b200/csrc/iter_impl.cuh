@@ -88,6 +88,7 @@ __device__ void Solver<C>::init_problem(long long id) {
     theta_max = o->theta_max_fact * fmax(1.0, theta);
     theta_min = o->theta_min_fact * fmax(1.0, theta);
     nfilt = 0; k = 0; nrec = 0;
+    reset_ls_memory();
     status = fin ? JIPM_ST_NOT_RUN : JIPM_ST_NONFINITE;
 }
 
@@ -266,6 +267,7 @@ __device__ void Solver<C>::enter_restoration(double* rec, int kind) {
     c.tm.sync();
     theta = c.tm.sum(th1); cmax = c.tm.max(cm); f_pn = c.tm.sum(spn); f_q = 0.0;
     mode = 1; nX = n + 2 * m;
+    reset_ls_memory();  // neither problem's line-search memory survives a change of mode
     mu = mu_bar; tau = fmax(o->tau_min, 1.0 - mu_bar); dw_last = 0.0; nfilt = 0;
     zeta = sqrt(mu_bar);
     f = rho * f_pn + 0.5 * zeta * f_q;
@@ -292,11 +294,240 @@ __device__ void Solver<C>::try_exit_restoration() {
     for (int j = lane; j < pb->m; j += NT) y[j] = 0.0;
     c.tm.sync();
     mode = 0; nX = n;
+    reset_ls_memory();
     mu = mu_reg; tau = tau_reg; dw_last = dw_last_reg; theta_min = theta_min_reg; theta_max = theta_max_reg;
     nfilt = nfilt_reg;
     bool fin;
     f = c.eval_fc(x, VH(L->c), theta, cmax, fin);  // base c back into the c vector (same point: same values)
     n_fc++;
+}
+
+// ---- Algorithm IC (A-4) ---------------------------------------------------------------
+// Factorises with (dw, dc) until the pivot signs give the inertia (n, m, 0).  resume: the factorisation at the
+// incoming (dw, dc) had the right inertia but the solve with it failed the refinement test ("pretend singular",
+// reading S-7): delta_c takes its IC-2 value, delta_w moves to the next rung (IC-3 from 0, else IC-5) and the loop
+// IC-4..IC-6 continues.  Returns false when delta_w exceeds delta_w_max (IC-6).
+template <class C>
+__device__ bool Solver<C>::ic_loop(bool resume, double& dw, double& dc, int& nfact) {
+    const long long t_f = clock64();
+    const double grow = (dw_last == 0.0) ? o->kappa_w_plus_first : o->kappa_w_plus;
+    const double first = (dw_last == 0.0) ? o->delta_w_0 : fmax(o->delta_w_min, o->kappa_w_minus * dw_last);  // IC-3
+    int nzero = 0, nf = 0;
+    bool ok = false, give_up = false;
+    if (!resume) {
+        set_sigma(0.0, 0.0);
+        const int bad = K::factor(c, nzero, mode != 0, true); nf++;                       // IC-1
+        if (bad == 0) { dw = 0.0; dc = 0.0; ok = true; }
+        else {
+            dc = (nzero > 0) ? o->delta_c_bar * pow(mu, o->kappa_c) : 0.0;                // IC-2
+            dw = first;
+        }
+    } else {
+        dc = o->delta_c_bar * pow(mu, o->kappa_c);
+        if (dw == 0.0) dw = first;
+        else { dw *= grow; if (dw > o->delta_w_max) give_up = true; }
+    }
+    while (!ok && !give_up) {
+        set_sigma(dw, dc);
+        const int bad = K::factor(c, nzero, mode != 0 || dc != 0.0, true); nf++;          // IC-4
+        if (bad == 0) { ok = true; break; }
+        dw *= grow;                                                                       // IC-5
+        if (dw > o->delta_w_max) give_up = true;                                          // IC-6
+    }
+    nfact += nf; n_fact += nf;
+    tph[1] += clock64() - t_f;
+    return ok;
+}
+
+// f, c, theta, phi_mu of the active problem at x + alpha d (into xt, ct)
+template <class C>
+__device__ void Solver<C>::trial(const Vec dxv, double alpha, Trial& t) {
+    Vec x = VX(L->x); Vec xt = VX(L->xt); double* ct = VH(L->ct);
+    for (int i = lane; i < nX; i += NT) xt[i] = x[i] + alpha * dxv[i];
+    c.tm.sync();
+    t.f = eval_point(xt, ct, t.th, t.cm, t.fb, t.thb, t.cmb, t.fpn, t.fq);
+    t.ph = phi(xt, t.f, mu, nX);
+}
+
+// Backtracking line search with the second-order correction (Table I rows 1-2; A-5) along dxv from
+// the current iterate.  acc: 0 = Newton step, 1 = corrected step (in sx, sy, szL, szU); alpha = the step length the
+// acceptance test used, alpha_acc = the length of the accepted step; ta = the accepted trial.  rec[6], rec[7] get the
+// numbers of backtracks and corrections.  Returns false when alpha falls below alpha_min.
+template <class C>
+__device__ bool Solver<C>::backtrack(const Vec dxv, double theta_k, double phi_k, double gd, double a_max,
+                                     bool skip_first, bool allow_soc, double* rec, int& acc, double& alpha,
+                                     double& alpha_acc, Trial& ta) {
+    Vec x = VX(L->x); double* cv = VH(L->c);
+    Vec b1 = VX(L->b1); Vec b3 = VX(L->b3); Vec b4 = VX(L->b4);
+    const int m = pb->m;
+    double a_min;
+    if (gd < 0.0 && theta_k <= theta_min)
+        a_min = o->gamma_alpha * fmin(fmin(o->gamma_theta, o->gamma_phi * theta_k / (-gd)),
+                                     o->delta * pow(theta_k, o->s_theta) / pow(-gd, o->s_phi));
+    else if (gd < 0.0) a_min = o->gamma_alpha * fmin(o->gamma_theta, o->gamma_phi * theta_k / (-gd));
+    else a_min = o->gamma_alpha * o->gamma_theta;
+    double* ct = VH(L->ct); Vec xt = VX(L->xt);
+    alpha = a_max; alpha_acc = 0.0;
+    int ntrial = 0, nsoc = 0;
+    acc = -1;
+    bool live = true;
+    if (skip_first) {  // the full step was tried (and rejected) before: start one halving down, no correction
+        alpha *= o->alpha_red;
+        ntrial = 1;
+        if (alpha < a_min) live = false;
+    }
+    while (live) {
+        Trial t;
+        trial(dxv, alpha, t);
+        if (acceptable(t.th, t.ph, theta_k, phi_k, alpha, gd)) { acc = 0; alpha_acc = alpha; ta = t; break; }
+        if (ntrial == 0 && allow_soc && isfinite(t.th) && t.th >= theta_k && o->max_soc > 0) {
+            // second-order correction (Table I row 2, PAPER.md:130)
+            double* csoc = V(L->csoc); double* bs2 = V(L->bs2);
+            Vec sx = VX(L->sx); double* sy = V(L->sy); Vec szL = VX(L->szL); Vec szU = VX(L->szU);
+            for (int i = lane; i < m; i += NT) csoc[i] = alpha * cv[i] + ct[i];
+            c.tm.sync();
+            double theta_old = theta_k;
+            for (int ps = 1; ps <= o->max_soc; ++ps) {
+                for (int i = lane; i < m; i += NT) bs2[i] = -csoc[i];
+                c.tm.sync();
+                bool failed;
+                solve_full(b1, bs2, b3, b4, sx, sy, szL, szU, failed);
+                const double a_soc = ftb_primal(x, sx, tau);
+                Trial ts;
+                trial(sx, a_soc, ts);
+                nsoc = ps;
+                if (acceptable(ts.th, ts.ph, theta_k, phi_k, alpha, gd)) { acc = 1; alpha_acc = a_soc; ta = ts; break; }
+                if (!isfinite(ts.th) || ts.th > o->kappa_soc * theta_old) break;
+                theta_old = ts.th;
+                for (int i = lane; i < m; i += NT) csoc[i] = a_soc * csoc[i] + ct[i];
+                c.tm.sync();
+            }
+            if (acc >= 0) break;
+        }
+        alpha *= o->alpha_red;
+        ntrial++;
+        if (alpha < a_min || ntrial > o->max_backtrack) break;
+        if constexpr (NT >= 64) {
+            // Speculative backtracking (PAPER.md:160): warp w evaluates the candidate alpha * alpha_red^w; the candidates
+            // are then scanned in the sequential order with the sequential termination rule, so the decision is the one
+            // of Step A-5.  The first acceptable candidate is re-evaluated by the regular path at the top of the loop
+            // (it fills c, f and confirms the test); rejected ones only advance alpha and the trial counter.
+            constexpr int NWP = NT / 32;
+            double* spec = c.smt(C::SM_SPEC);
+            bool exhausted = false, found = false;
+            const long long t_sp = clock64();
+            while (!found && !exhausted) {
+                double aw = alpha;
+                for (int w = 0; w < (lane >> 5); ++w) aw *= o->alpha_red;
+                double th_w, ph_w;
+                trial_warp(x, dxv, aw, th_w, ph_w);
+                const bool ok_w = acceptable_warp(th_w, ph_w, theta_k, phi_k, aw, gd);
+                if ((lane & 31) == 0) spec[lane >> 5] = ok_w ? 1.0 : 0.0;
+                c.tm.sync();
+                for (int w = 0; w < NWP; ++w) {
+                    if (spec[w] != 0.0) { found = true; break; }
+                    n_fc++;
+                    alpha *= o->alpha_red;
+                    ntrial++;
+                    if (alpha < a_min || ntrial > o->max_backtrack) { exhausted = true; break; }
+                }
+                c.tm.sync();
+            }
+            tph[7] += clock64() - t_sp;
+            if (exhausted) break;
+        }
+    }
+    rec[6] = ntrial; rec[7] = nsoc;
+    (void)xt;
+    return acc >= 0;
+}
+
+// A-6 / A-8: move to the accepted trial point (in xt, its c in ct), step the multipliers, safeguard z, count.
+template <class C>
+__device__ void Solver<C>::accept_step(int, const Vec, const double* ay, const Vec azL, const Vec azU, double,
+                                       double alpha_y, double a_z, const Trial& t) {
+    Vec x = VX(L->x); double* y = VH(L->y); Vec zL = VX(L->zL); Vec zU = VX(L->zU);
+    Vec xt = VX(L->xt); double* ct = VH(L->ct); double* cv = VH(L->c);
+    const double ks = o->kappa_sigma;
+    for (int i = lane; i < nX; i += NT) {
+        const double l = lo(i), u = hi(i);
+        const double xn = xt[i];
+        x[i] = xn;
+        double zl = 0.0, zu = 0.0;
+        if (l > -INFINITY) {
+            const double sl = xn - l;
+            zl = fmax(fmin(zL[i] + a_z * azL[i], ks * mu / sl), mu / (ks * sl));
+        }
+        if (u < INFINITY) {
+            const double su = u - xn;
+            zu = fmax(fmin(zU[i] + a_z * azU[i], ks * mu / su), mu / (ks * su));
+        }
+        zL[i] = zl; zU[i] = zu;
+    }
+    for (int i = lane; i < pb->m; i += NT) { y[i] += alpha_y * ay[i]; cv[i] = ct[i]; }
+    c.tm.sync();
+    f = t.f; theta = t.th; cmax = t.cm;
+    f_base = t.fb; theta_base = t.thb; cmax_base = t.cmb; f_pn = t.fpn; f_q = t.fq;
+    k += 1;  // A-8
+}
+
+// One step of the soft restoration phase (Table I row 5; reading SR): the same step length for
+// primal and dual variables; accepted if the original criterion holds (the phase ends) or if the error of the
+// primal-dual system (5a-d), measured as the sum of the 1-norms of its blocks divided by their lengths, drops by the
+// factor soft_resto_factor.  Returns false when the step is refused (the caller starts the hard restoration).
+template <class C>
+__device__ bool Solver<C>::soft_step(double* rec, double theta_k, double phi_k, double gd) {
+    Vec x = VX(L->x); double* y = VH(L->y); Vec zL = VX(L->zL); Vec zU = VX(L->zU);
+    Vec b1 = VX(L->b1); Vec b3 = VX(L->b3); Vec b4 = VX(L->b4);
+    Vec dx = VX(L->dx); double* dy = VH(L->dy); Vec dzL = VX(L->dzL); Vec dzU = VX(L->dzU);
+    Vec xt = VX(L->xt); Vec g = VX(L->g);
+    const int n = pb->n, m = pb->m;
+    const double a_p = ftb_primal(x, dx, tau);
+    const double a_d = ftb_dual(zL, zU, dzL, dzU, tau);
+    const double alpha = fmin(a_p, a_d);
+    // current error: -b1 is the dual residual (damping included), -b3 / -b4 the complementarity residuals
+    double s1 = 0.0, s3 = 0.0;
+    for (int i = lane; i < nX; i += NT) { s1 += fabs(b1[i]); s3 += fabs(b3[i]) + fabs(b4[i]); }
+    s1 = c.tm.sum(s1); s3 = c.tm.sum(s3);
+    const int ncomp = pb->nL + pb->nU + (mode ? 2 * m : 0);
+    const double e_k = s1 / nX + (m > 0 ? theta_k / m : 0.0) + (ncomp > 0 ? s3 / ncomp : 0.0);
+    Trial t;
+    trial(dx, alpha, t);
+    bool ok = isfinite(t.th) && isfinite(t.ph);
+    const bool orig = ok && acceptable(t.th, t.ph, theta_k, phi_k, 0.0, gd);
+    if (ok && !orig) {
+        double* yt = V(L->sy);
+        for (int i = lane; i < m; i += NT) yt[i] = y[i] + alpha * dy[i];
+        c.tm.sync();
+        c.eval_derivs(xt, yt, mode ? 0.0 : 1.0);  // J and grad f at the trial point (the next iteration re-evaluates)
+        n_deriv++;
+        const double* xR = V(L->xR); const double* DR2 = V(L->DR2);
+        double t1 = 0.0, t3 = 0.0;
+        for (int i = lane; i < nX; i += NT) {
+            const double l = lo(i), u = hi(i);
+            const bool hl = l > -INFINITY, hu = u < INFINITY;
+            const double zl = hl ? zL[i] + alpha * dzL[i] : 0.0, zu = hu ? zU[i] + alpha * dzU[i] : 0.0;
+            double gi;
+            if (mode) gi = (i < n) ? zeta * DR2[i] * (xt[i] - xR[i]) : o->rho_resto;
+            else gi = g[i];
+            double v = gi + ATx(yt, i) - zl + zu;
+            if (hl && !hu) v += o->kappa_d * mu;
+            if (hu && !hl) v -= o->kappa_d * mu;
+            t1 += fabs(v);
+            if (hl) t3 += fabs((xt[i] - l) * zl - mu);
+            if (hu) t3 += fabs((u - xt[i]) * zu - mu);
+        }
+        t1 = c.tm.sum(t1); t3 = c.tm.sum(t3);
+        const double e_t = t1 / nX + (m > 0 ? t.th / m : 0.0) + (ncomp > 0 ? t3 / ncomp : 0.0);
+        ok = isfinite(e_t) && e_t <= o->soft_resto_factor * e_k;
+    }
+    if (!ok) return false;
+    rec[17] = orig ? 2.0 : 1.0;
+    if (orig) { soft = 0; soft_count = 0; }
+    n_short = 0;
+    accept_step(0, dx, dy, dzL, dzU, alpha, alpha, alpha, t);
+    rec[5] = KIND_SOFT; rec[8] = alpha; rec[9] = alpha; rec[10] = 1.0;
+    return true;
 }
 
 // ---- Step A: one iteration (either mode) ---------------------------------------------------------------------
@@ -351,14 +582,27 @@ __device__ void Solver<C>::iterate() {
         rec[5] = KIND_TERMINAL; trace_put(rec); return;
     }
     if (k >= o->max_iter) { status = JIPM_ST_MAXITER; rec[5] = KIND_TERMINAL; trace_put(rec); return; }
-    // A-3 monotone barrier update (Table I row 7)
+    // A-3 monotone barrier update (Table I row 7).  Two tiny steps in a row (Table I row 4) force one
+    // decrease; when mu cannot decrease any more the search direction has become too small to make progress.
     int nmu = 0;
     const double mu_min = o->tol / 10.0;
-    while (nmu < o->max_mu_updates && mu > mu_min && opt_error(mu, sd, sc) <= o->kappa_eps * mu) {
+    bool force = tiny_flag != 0;
+    tiny_flag = 0;
+    while (nmu < o->max_mu_updates && (force || opt_error(mu, sd, sc) <= o->kappa_eps * mu)) {
+        if (!(mu > mu_min)) {
+            if (force) {
+                status = mode ? JIPM_ST_RESTORATION_FAILED : JIPM_ST_TINY_STEP;
+                rec[5] = KIND_TERMINAL; rec[11] = nmu; trace_put(rec); return;
+            }
+            break;
+        }
+        force = false;
         mu = fmax(mu_min, fmin(o->kappa_mu * mu, pow(mu, o->theta_mu)));
         tau = fmax(o->tau_min, 1.0 - mu);
         nfilt = 0;
         nmu++;
+        // a new barrier problem: the watchdog, its counter and the soft restoration phase start afresh
+        wd_active = 0; wd_trials = 0; n_short = 0; soft = 0; soft_count = 0;
         if (mode) {  // zeta = sqrt(mu) follows the restoration barrier parameter: objective, gradient, residual move
             const double zn = sqrt(mu);
             const double* xR = V(L->xR); const double* DR2 = V(L->DR2);
@@ -371,33 +615,8 @@ __device__ void Solver<C>::iterate() {
             f = o->rho_resto * f_pn + 0.5 * zeta * f_q;
         }
     }
-    rec[11] = nmu; rec[13] = mu;
-    // A-4 search direction with inertia correction (Algorithm IC)
-    int nfact = 0, nzero = 0;
-    double dw = 0.0, dc = 0.0;
-    bool ic_ok;
-    set_sigma(0.0, 0.0);
-    long long t_f = clock64();
-    c.pc[7] += t_f - t_hd;
-    int bad = K::factor(c, nzero, mode != 0, true); nfact++;  // IC-1
-    ic_ok = (bad == 0);
-    if (!ic_ok) {
-        dc = (nzero > 0) ? o->delta_c_bar * pow(mu, o->kappa_c) : 0.0;                               // IC-2
-        dw = (dw_last == 0.0) ? o->delta_w_0 : fmax(o->delta_w_min, o->kappa_w_minus * dw_last);      // IC-3
-        while (true) {
-            set_sigma(dw, dc);
-            bad = K::factor(c, nzero, mode != 0 || dc != 0.0, true); nfact++;                       // IC-4
-            if (bad == 0) { ic_ok = true; break; }
-            dw *= (dw_last == 0.0) ? o->kappa_w_plus_first : o->kappa_w_plus;                         // IC-5
-            if (dw > o->delta_w_max) break;                                                          // IC-6
-        }
-    }
-    n_fact += nfact;
-    tph[1] += clock64() - t_f;
-    rec[1] = nfact; rec[2] = dw; rec[3] = dc; rec[14] = theta;
-    if (!ic_ok) { rec[1] = 0; rec[2] = 0; rec[3] = 0; enter_restoration(rec, KIND_IC_FAIL); trace_put(rec); return; }
-    if (dw > 0.0) dw_last = dw;
-    // right-hand side of (6)
+    rec[11] = nmu; rec[13] = mu; rec[14] = theta;
+    // right-hand side of (6) (it does not depend on the perturbations)
     for (int i = lane; i < nX; i += NT) {
         const double l = lo(i), u = hi(i);
         const bool hl = l > -INFINITY, hu = u < INFINITY;
@@ -410,12 +629,26 @@ __device__ void Solver<C>::iterate() {
     }
     for (int i = lane; i < m; i += NT) b2[i] = -cv[i];
     c.tm.sync();
-    const long long t_sf = clock64();
-    const int nref = solve_full(b1, b2, b3, b4, dx, dy, dzL, dzU);
-    c.pc[5] += clock64() - t_sf;
-    rec[4] = nref;
-    // A-5 filter line search
-    double gd_part = 0.0;
+    // A-4 search direction with inertia correction (Algorithm IC); a solve whose refinement on (6) fails
+    // sends the matrix back to Algorithm IC as if it were singular (reading S-7)
+    int nfact = 0, npsing = 0, nref = 0;
+    double dw = 0.0, dc = 0.0;
+    bool resume = false;
+    c.pc[7] += clock64() - t_hd;
+    while (true) {
+        if (!ic_loop(resume, dw, dc, nfact)) { enter_restoration(rec, KIND_IC_FAIL); trace_put(rec); return; }
+        bool failed;
+        const long long t_sf = clock64();
+        nref = solve_full(b1, b2, b3, b4, dx, dy, dzL, dzU, failed);
+        c.pc[5] += clock64() - t_sf;
+        if (!failed) break;
+        npsing++;
+        resume = true;
+    }
+    rec[1] = nfact; rec[2] = dw; rec[3] = dc; rec[4] = nref; rec[19] = npsing;
+    if (dw > 0.0) dw_last = dw;
+    // A-5 line search
+    double gd_part = 0.0, xm = 0.0, dym = 0.0;
     for (int i = lane; i < nX; i += NT) {
         const double l = lo(i), u = hi(i);
         const bool hl = l > -INFINITY, hu = u < INFINITY;
@@ -425,130 +658,149 @@ __device__ void Solver<C>::iterate() {
         if (hl && !hu) gp += o->kappa_d * mu;
         if (hu && !hl) gp -= o->kappa_d * mu;
         gd_part += gp * dx[i];
+        xm = fmax(xm, fabs(dx[i]) / (1.0 + fabs(x[i])));
     }
-    const double gd = c.tm.sum(gd_part);
-    const double theta_k = theta;
-    const double phi_k = phi(x, f, mu, nX);
+    for (int i = lane; i < m; i += NT) dym = fmax(dym, fabs(dy[i]));
+    double gd = c.tm.sum(gd_part);
+    xm = c.tm.max(xm); dym = c.tm.max(dym);
+    double theta_k = theta;
+    double phi_k = phi(x, f, mu, nX);
     rec[15] = phi_k;
-    const double a_max = ftb_primal(x, dx, tau);
-    double a_min;
-    if (gd < 0.0 && theta_k <= theta_min)
-        a_min = o->gamma_alpha * fmin(fmin(o->gamma_theta, o->gamma_phi * theta_k / (-gd)),
-                                     o->delta * pow(theta_k, o->s_theta) / pow(-gd, o->s_phi));
-    else if (gd < 0.0) a_min = o->gamma_alpha * fmin(o->gamma_theta, o->gamma_phi * theta_k / (-gd));
-    else a_min = o->gamma_alpha * o->gamma_theta;
+    double a_max = ftb_primal(x, dx, tau);
     const long long t_ls = clock64();
-    Vec xt = VX(L->xt); double* ct = VH(L->ct);
-    double alpha = a_max, alpha_acc = 0.0, phi_acc = 0.0, f_acc = 0.0, th_acc = 0.0, cm_acc = 0.0;
-    double fb_acc = 0.0, thb_acc = 0.0, cmb_acc = 0.0, fpn_acc = 0.0, fq_acc = 0.0;
-    int ntrial = 0, nsoc = 0, acc = -1;  // acc: 0 newton, 1 soc
-    while (true) {
-        for (int i = lane; i < nX; i += NT) xt[i] = x[i] + alpha * dx[i];
-        c.tm.sync();
-        double th_t, cm_t, fb, thb, cmb, fpn, fq;
-        const double f_t = eval_point(xt, ct, th_t, cm_t, fb, thb, cmb, fpn, fq);
-        const double ph_t = phi(xt, f_t, mu, nX);
-        if (acceptable(th_t, ph_t, theta_k, phi_k, alpha, gd)) {
-            acc = 0; alpha_acc = alpha; phi_acc = ph_t; f_acc = f_t; th_acc = th_t; cm_acc = cm_t;
-            fb_acc = fb; thb_acc = thb; cmb_acc = cmb; fpn_acc = fpn; fq_acc = fq;
-            break;
-        }
-        if (ntrial == 0 && isfinite(th_t) && th_t >= theta_k && o->max_soc > 0) {
-            // second-order correction (Table I row 2, PAPER.md:130)
-            double* csoc = V(L->csoc); double* bs2 = V(L->bs2);
-            Vec sx = VX(L->sx); double* sy = V(L->sy); Vec szL = VX(L->szL); Vec szU = VX(L->szU);
-            for (int i = lane; i < m; i += NT) csoc[i] = alpha * cv[i] + ct[i];
-            c.tm.sync();
-            double theta_old = theta_k;
-            for (int ps = 1; ps <= o->max_soc; ++ps) {
-                for (int i = lane; i < m; i += NT) bs2[i] = -csoc[i];
-                c.tm.sync();
-                solve_full(b1, bs2, b3, b4, sx, sy, szL, szU);
-                const double a_soc = ftb_primal(x, sx, tau);
-                for (int i = lane; i < nX; i += NT) xt[i] = x[i] + a_soc * sx[i];
-                c.tm.sync();
-                double th_s, cm_s;
-                const double f_s = eval_point(xt, ct, th_s, cm_s, fb, thb, cmb, fpn, fq);
-                const double ph_s = phi(xt, f_s, mu, nX);
-                nsoc = ps;
-                if (acceptable(th_s, ph_s, theta_k, phi_k, alpha, gd)) {
-                    acc = 1; alpha_acc = a_soc; phi_acc = ph_s; f_acc = f_s; th_acc = th_s; cm_acc = cm_s;
-                    fb_acc = fb; thb_acc = thb; cmb_acc = cmb; fpn_acc = fpn; fq_acc = fq;
-                    break;
-                }
-                if (!isfinite(th_s) || th_s > o->kappa_soc * theta_old) break;
-                theta_old = th_s;
-                for (int i = lane; i < m; i += NT) csoc[i] = a_soc * csoc[i] + ct[i];
-                c.tm.sync();
-            }
-            if (acc >= 0) break;
-        }
-        alpha *= o->alpha_red;
-        ntrial++;
-        if (alpha < a_min || ntrial > o->max_backtrack) break;
-        if constexpr (NT >= 64) {
-            // Speculative backtracking (PAPER.md:160): warp w evaluates the candidate alpha * alpha_red^w; the candidates
-            // are then scanned in the sequential order with the sequential termination rule, so the decision is the one
-            // of Step A-5.  The first acceptable candidate is re-evaluated by the regular path at the top of the loop
-            // (it fills c, f and confirms the test); rejected ones only advance alpha and the trial counter.
-            constexpr int NWP = NT / 32;
-            double* spec = c.smt(C::SM_SPEC);
-            bool exhausted = false, found = false;
-            const long long t_sp = clock64();
-            while (!found && !exhausted) {
-                double aw = alpha;
-                for (int w = 0; w < (lane >> 5); ++w) aw *= o->alpha_red;
-                double th_w, ph_w;
-                trial_warp(x, dx, aw, th_w, ph_w);
-                const bool ok_w = acceptable_warp(th_w, ph_w, theta_k, phi_k, aw, gd);
-                if ((lane & 31) == 0) spec[lane >> 5] = ok_w ? 1.0 : 0.0;
-                c.tm.sync();
-                for (int w = 0; w < NWP; ++w) {
-                    if (spec[w] != 0.0) { found = true; break; }
-                    n_fc++;
-                    alpha *= o->alpha_red;
-                    ntrial++;
-                    if (alpha < a_min || ntrial > o->max_backtrack) { exhausted = true; break; }
-                }
-                c.tm.sync();
-            }
-            tph[7] += clock64() - t_sp;
-            if (exhausted) break;
-        }
+    // Table I row 4: a step too small for backtracking to refine is accepted as it is
+    if (xm <= o->tiny_step_tol && cmax <= o->tiny_step_cviol) {
+        rec[18] = 1.0;
+        if (tiny_last && dym < o->tiny_step_y_tol) tiny_flag = 1;
+        tiny_last = 1;
+        Trial t;
+        trial(dx, a_max, t);
+        const double a_z = ftb_dual(zL, zU, dzL, dzU, tau);
+        accept_step(0, dx, dy, dzL, dzU, a_max, a_max, a_z, t);
+        rec[5] = KIND_TINY; rec[8] = a_max; rec[9] = a_z; rec[10] = 1.0;
+        trace_put(rec);
+        if (mode) try_exit_restoration();
+        return;
     }
-    rec[6] = ntrial; rec[7] = nsoc;
+    tiny_last = 0;
+    // Table I row 5: in the soft restoration phase the acceptance criterion is a reduction of the
+    // primal-dual error, until the original criterion holds again or the iteration limit is reached
+    if (soft) {
+        soft_count++;
+        if (soft_count > o->max_soft_resto_iters || !soft_step(rec, theta_k, phi_k, gd)) {
+            soft = 0;
+            enter_restoration(rec, KIND_LS_FAIL); trace_put(rec); return;
+        }
+        trace_put(rec);
+        if (mode) try_exit_restoration();
+        return;
+    }
+    // Table I row 3: after watchdog_trigger shortened steps in a row the watchdog wakes up: it keeps
+    // the entry iterate and direction, takes full steps without any test and either reaches a point acceptable to the
+    // entry iterate's criterion or, after watchdog_trial_max trials, returns to the entry iterate
+    if (!wd_active && o->watchdog_trigger > 0 && n_short >= o->watchdog_trigger) {
+        Vec wx = VX(L->wx); Vec wzL = VX(L->wzL); Vec wzU = VX(L->wzU);
+        Vec wdx = VX(L->wdx); Vec wdzL = VX(L->wdzL); Vec wdzU = VX(L->wdzU);
+        double* wy = V(L->wy); double* wdy = V(L->wdy);
+        for (int i = lane; i < nX; i += NT) {
+            wx[i] = x[i]; wzL[i] = zL[i]; wzU[i] = zU[i]; wdx[i] = dx[i]; wdzL[i] = dzL[i]; wdzU[i] = dzU[i];
+        }
+        for (int i = lane; i < m; i += NT) { wy[i] = y[i]; wdy[i] = dy[i]; }
+        c.tm.sync();
+        wd_theta = theta_k; wd_phi = phi_k; wd_gd = gd; wd_alpha = a_max; wd_trials = 0; wd_active = 1;
+        rec[16] = 1.0;
+    }
+    int acc = -1;
+    double alpha = a_max, alpha_acc = 0.0;
+    Trial ta;
+    bool ok;
+    if (wd_active) {
+        Trial t;
+        trial(dx, a_max, t);
+        const bool good = acceptable(t.th, t.ph, wd_theta, wd_phi, wd_alpha, wd_gd);
+        if (good || (wd_trials + 1 <= o->watchdog_trial_max && isfinite(t.th) && isfinite(t.ph))) {
+            bool ftype = true;
+            if (good) {  // acceptable to the entry iterate's criterion: the watchdog succeeded
+                ftype = switching(wd_alpha, wd_gd, wd_theta) && armijo(t.ph, wd_phi, wd_alpha, wd_gd);
+                if (!ftype) filter_add((1.0 - o->gamma_theta) * wd_theta, wd_phi - o->gamma_phi * wd_theta);
+                wd_active = 0; wd_trials = 0; n_short = 0;
+                rec[16] = 3.0;
+            } else {     // taken unconditionally
+                wd_trials++;
+                if (rec[16] == 0.0) rec[16] = 2.0;
+            }
+            const double a_z = ftb_dual(zL, zU, dzL, dzU, tau);
+            accept_step(0, dx, dy, dzL, dzU, a_max, a_max, a_z, t);
+            rec[5] = KIND_NEWTON; rec[8] = a_max; rec[9] = a_z; rec[10] = ftype ? 1.0 : 0.0;
+            c.pc[6] += clock64() - t_ls;
+            trace_put(rec);
+            if (mode) try_exit_restoration();
+            return;
+        }
+        // the watchdog gives up: back to its entry iterate and direction, ordinary backtracking from there (the full
+        // step of the entry iterate was tried when the watchdog started: skipped; no correction)
+        {
+            Vec wx = VX(L->wx); Vec wzL = VX(L->wzL); Vec wzU = VX(L->wzU);
+            Vec wdx = VX(L->wdx); Vec wdzL = VX(L->wdzL); Vec wdzU = VX(L->wdzU);
+            const double* wy = V(L->wy); const double* wdy = V(L->wdy);
+            for (int i = lane; i < nX; i += NT) {
+                x[i] = wx[i]; zL[i] = wzL[i]; zU[i] = wzU[i]; dx[i] = wdx[i]; dzL[i] = wdzL[i]; dzU[i] = wdzU[i];
+            }
+            for (int i = lane; i < m; i += NT) { y[i] = wy[i]; dy[i] = wdy[i]; }
+            c.tm.sync();
+        }
+        theta_k = wd_theta; phi_k = wd_phi; gd = wd_gd; a_max = wd_alpha;
+        wd_active = 0; wd_trials = 0; n_short = 0;
+        rec[16] = 4.0;
+        // f, c, grad f, J and the residuals of (5a-d) at the entry iterate again (the soft phase may need them)
+        f = eval_point(x, cv, theta, cmax, f_base, theta_base, cmax_base, f_pn, f_q);
+        c.eval_derivs(x, y, mode ? 0.0 : 1.0);
+        n_deriv++;
+        if (mode) {
+            const double* xR = V(L->xR); const double* DR2 = V(L->DR2);
+            for (int i = lane; i < n; i += NT) g[i] = zeta * DR2[i] * (x[i] - xR[i]);
+            for (int i = n + lane; i < nX; i += NT) g[i] = o->rho_resto;
+            c.tm.sync();
+        }
+        for (int i = lane; i < nX; i += NT) {
+            const double l = lo(i), u = hi(i);
+            const bool hl = l > -INFINITY, hu = u < INFINITY;
+            double dmp = 0.0;
+            if (hl && !hu) dmp = o->kappa_d * mu;
+            if (hu && !hl) dmp = -o->kappa_d * mu;
+            b1[i] = -(g[i] + ATx(y, i) - zL[i] + zU[i] + dmp);
+            b3[i] = hl ? mu - (x[i] - l) * zL[i] : 0.0;
+            b4[i] = hu ? mu - (u - x[i]) * zU[i] : 0.0;
+        }
+        c.tm.sync();
+        ok = backtrack(dx, theta_k, phi_k, gd, a_max, true, false, rec, acc, alpha, alpha_acc, ta);
+    } else {
+        ok = backtrack(dx, theta_k, phi_k, gd, a_max, false, true, rec, acc, alpha, alpha_acc, ta);
+    }
     c.pc[6] += clock64() - t_ls;
-    if (acc < 0) { enter_restoration(rec, KIND_LS_FAIL); trace_put(rec); return; }
+    if (!ok) {
+        // the line search failed: first the soft restoration phase (row 5), then the hard one (row 6)
+        if (o->soft_resto_factor > 0.0) {
+            soft = 1; soft_count = 0;
+            filter_add((1.0 - o->gamma_theta) * theta_k, phi_k - o->gamma_phi * theta_k);
+            if (soft_step(rec, theta_k, phi_k, gd)) {
+                trace_put(rec);
+                if (mode) try_exit_restoration();
+                return;
+            }
+            soft = 0;
+        }
+        enter_restoration(rec, KIND_LS_FAIL); trace_put(rec); return;
+    }
     // A-6 accept, A-7 filter augmentation
-    const Vec ax = (acc == 1) ? VX(L->sx) : dx;
     const double* ay = (acc == 1) ? V(L->sy) : dy;
     const Vec azL = (acc == 1) ? VX(L->szL) : dzL;
     const Vec azU = (acc == 1) ? VX(L->szU) : dzU;
-    (void)ax;
     const double a_z = ftb_dual(zL, zU, azL, azU, tau);
-    const bool ftype = switching(alpha, gd, theta_k) && armijo(phi_acc, phi_k, alpha, gd);
+    const bool ftype = switching(alpha, gd, theta_k) && armijo(ta.ph, phi_k, alpha, gd);
     if (!ftype) filter_add((1.0 - o->gamma_theta) * theta_k, phi_k - o->gamma_phi * theta_k);
-    const double ks = o->kappa_sigma;
-    for (int i = lane; i < nX; i += NT) {
-        const double l = lo(i), u = hi(i);
-        const double xn = xt[i];
-        x[i] = xn;
-        double zl = 0.0, zu = 0.0;
-        if (l > -INFINITY) {
-            const double sl = xn - l;
-            zl = fmax(fmin(zL[i] + a_z * azL[i], ks * mu / sl), mu / (ks * sl));
-        }
-        if (u < INFINITY) {
-            const double su = u - xn;
-            zu = fmax(fmin(zU[i] + a_z * azU[i], ks * mu / su), mu / (ks * su));
-        }
-        zL[i] = zl; zU[i] = zu;
-    }
-    for (int i = lane; i < m; i += NT) { y[i] += alpha_acc * ay[i]; cv[i] = ct[i]; }
-    c.tm.sync();
-    f = f_acc; theta = th_acc; cmax = cm_acc;
-    f_base = fb_acc; theta_base = thb_acc; cmax_base = cmb_acc; f_pn = fpn_acc; f_q = fq_acc;
-    k += 1;  // A-8
+    n_short = (rec[6] > 0.0) ? n_short + 1 : 0;
+    accept_step(acc, dx, ay, azL, azU, alpha_acc, alpha_acc, a_z, ta);
     rec[5] = (acc == 1) ? KIND_SOC : KIND_NEWTON;
     rec[8] = alpha_acc; rec[9] = a_z; rec[10] = ftype ? 1.0 : 0.0;
     trace_put(rec);

@@ -5,6 +5,8 @@
 #include <string>
 #include <vector>
 #include <algorithm>
+#include <mutex>
+#include <cstdlib>
 #include "launch.cuh"
 
 using namespace jipm;
@@ -20,8 +22,23 @@ static int fail(int code, const std::string& msg) { g_err = msg; return code; }
     } while (0)
 
 
+// Launch arguments live in ONE __constant__ block per family instantiation (inst.cuh): two solves of the same
+// family must not overlap.  Every launch-to-completion section (run()) holds this lock.
+static std::mutex g_launch_mutex;
+
+// RAII switch to the solver's device for the duration of a call
+struct DeviceGuard {
+    int prev = -1; bool ok = true;
+    explicit DeviceGuard(int dev) {
+        if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; return; }
+        if (prev != dev && cudaSetDevice(dev) != cudaSuccess) ok = false;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
 struct jipm_solver {
     int family;
+    int device = 0;
     jipm_family_dims dims;
     jipm_options o;
     Pb pb;
@@ -29,7 +46,9 @@ struct jipm_solver {
     int NX, NU, NZ;
     Inst inst;
     int teams_per_sm;
-    int n_slots;
+    int n_slots;          // R: CTAs launched per solve (capped by the number of problems)
+    int n_sm = 0;         // SMs of the solver's device; the global scratch holds n_sm * teams_per_sm workspaces
+    unsigned* d_mask = nullptr;
     cudaStream_t stream;
     double *d_xL = nullptr, *d_xU = nullptr, *d_ws = nullptr;
     int* d_queue = nullptr;
@@ -38,6 +57,9 @@ struct jipm_solver {
     int trace_cap = 0;
     long long stats[24] = {0};
     DbgLay dbg;
+    // grow-only device staging of jipm_solve_batch_host
+    double* d_stage = nullptr; size_t stage_doubles = 0;
+    int32_t* d_istage = nullptr; size_t istage_ints = 0;
 };
 
 extern "C" const char* jipm_last_error(void) { return g_err.c_str(); }
@@ -54,12 +76,18 @@ extern "C" int jipm_default_options(jipm_options* o) {
     o->residual_ratio_max = 1e-10; o->rho_resto = 1000.0; o->kappa_resto = 0.9; o->z_reset_threshold = 1e3;
     o->max_iter = 3000; o->max_backtrack = 64; o->max_soc = 4; o->refine_min = 1; o->refine_max = 10;
     o->max_mu_updates = 8; o->init_slacks = 1; o->enable_restoration = 1;
+    o->residual_ratio_singular = 1e-5; o->residual_improvement_factor = 0.999999999;
+    o->tiny_step_tol = 10.0 * 2.220446049250313e-16; o->tiny_step_y_tol = 1e-2; o->tiny_step_cviol = 1e-4;
+    o->soft_resto_factor = 1.0 - 1e-4;
+    o->watchdog_trigger = 10; o->watchdog_trial_max = 3; o->max_soft_resto_iters = 10; o->reserved_ = 0;
     return JIPM_OK;
 }
 
 static bool family_shape(int family, const jipm_family_dims* d, int& nx, int& nu, int& ng, int& nth, int& pd) {
     if (!d || d->horizon_N < 1 || d->horizon_N > 4096 || !(d->dt > 0.0)) return false;
     const int na = d->n_agents, nobs = d->n_obstacles;
+    // core.cuh build_maps packs the inequality index of a knot into 8 bits with 254 / 255 as sentinels
+    if (nobs > 254) return false;
     switch (family) {
         case JIPM_FAM_POINTMASS2D:
             if (na != 1 || nobs < 0) return false;
@@ -114,10 +142,11 @@ static int build_layout(jipm_solver* s, int sm_budget_doubles) {
     int Lay::*const primal[] = {
         &Lay::x, &Lay::rr, &Lay::dx, &Lay::Sig, &Lay::xt, &Lay::zL, &Lay::zU, &Lay::b1, &Lay::dzL, &Lay::dzU, &Lay::b3, &Lay::b4,
         &Lay::g, &Lay::Hd, &Lay::r1, &Lay::r3, &Lay::r4, &Lay::e1, &Lay::e3, &Lay::e4, &Lay::sx, &Lay::szL, &Lay::szU,
+        &Lay::wx, &Lay::wzL, &Lay::wzU, &Lay::wdx, &Lay::wdzL, &Lay::wdzU,
     };
     const Ent cold[] = {
         {&Lay::rk, rkn}, {&Lay::sy, m}, {&Lay::csoc, m}, {&Lay::bs2, m}, {&Lay::rc2, m},
-        {&Lay::xR, n}, {&Lay::DR2, n}, {&Lay::filtR, 2 * MAX_FILTER},
+        {&Lay::xR, n}, {&Lay::DR2, n}, {&Lay::filtR, 2 * MAX_FILTER}, {&Lay::wy, m}, {&Lay::wdy, m},
     };
     int o = 0;
     L.nsm = 0;
@@ -181,8 +210,19 @@ extern "C" int jipm_create(jipm_solver** out, int family, const jipm_family_dims
     if (family == JIPM_FAM_POINTMASS2D) s->inst = inst_pm();
     else if (family == JIPM_FAM_MULTIQUAD) s->inst = d->n_agents == 4 ? inst_q4() : inst_q2();
     else s->inst = inst_q1();
+    bool forced_inst = false;
+    if (const char* ev = getenv("JIPM_EXPERIMENT_INST")) {   // development switch (measurements of DESIGN.md section 6)
+        if (family == JIPM_FAM_QUAD_TRACK || family == JIPM_FAM_QUAD_CLUTTER) {
+            if (!strcmp(ev, "q1b")) { s->inst = inst_q1b(); forced_inst = true; }
+            if (!strcmp(ev, "q1c")) { s->inst = inst_q1c(); forced_inst = true; }
+            if (!strcmp(ev, "q1g")) { s->inst = inst_q1g(); forced_inst = true; }
+        }
+    }
     cudaDeviceProp prop;
-    if (cudaGetDeviceProperties(&prop, 0) != cudaSuccess) { delete s; return fail(JIPM_ERR_CUDA, "cudaGetDeviceProperties"); }
+    if (cudaGetDevice(&s->device) != cudaSuccess || cudaGetDeviceProperties(&prop, s->device) != cudaSuccess) {
+        delete s;
+        return fail(JIPM_ERR_CUDA, "cudaGetDevice / cudaGetDeviceProperties");
+    }
     // shared-memory budget per team: the SM's shared memory split over the CTAs the kernel was compiled to co-run
     // (register budget of __launch_bounds__), minus the fixed tiles and 1 KB of per-CTA reservation
     s->teams_per_sm = std::max(1, std::min(s->inst.info.min_blocks, 2048 / s->inst.info.nt));
@@ -191,6 +231,7 @@ extern "C" int jipm_create(jipm_solver** out, int family, const jipm_family_dims
     const long budget = per_team / (long)sizeof(double) - s->inst.info.sm_fixed;
     if (budget < 0) { delete s; return fail(JIPM_ERR_NOMEM, "stage tiles do not fit shared memory"); }
     int hot_fits = build_layout(s, (int)budget);
+    (void)forced_inst;
     if (!hot_fits && s->inst.info.hot_sm) {
         // the hot group does not fit: the general instantiation of the family (generic loads, arrays wherever they fit)
         if (family == JIPM_FAM_POINTMASS2D) { delete s; return fail(JIPM_ERR_NOMEM, "problem too large for the point-mass kernel"); }
@@ -202,12 +243,16 @@ extern "C" int jipm_create(jipm_solver** out, int family, const jipm_family_dims
         hot_fits = build_layout(s, (int)b2);
     }
     s->dbg = make_dbglay(pb.n, pb.m, pb.N, s->NX, s->NZ);
+    s->n_sm = prop.multiProcessorCount;
+    if (s->teams_per_sm > 32) s->teams_per_sm = 32;  // one bit of sm_mask per co-resident team
     if (resident_slots == 0) resident_slots = (int64_t)s->teams_per_sm * prop.multiProcessorCount;  // fill the GPU
-    s->n_slots = (int)resident_slots;
+    s->n_slots = (int)std::min<int64_t>(resident_slots, 0x7fffffff);
+    const size_t n_ws = (size_t)s->n_sm * s->teams_per_sm;
     cudaError_t e;
     if ((e = cudaMalloc(&s->d_xL, n * sizeof(double))) != cudaSuccess ||
         (e = cudaMalloc(&s->d_xU, n * sizeof(double))) != cudaSuccess ||
-        (e = cudaMalloc(&s->d_ws, (size_t)s->n_slots * (s->L.total - s->L.nsm + 2) * sizeof(double))) != cudaSuccess ||
+        (e = cudaMalloc(&s->d_ws, n_ws * (s->L.total - s->L.nsm + 2) * sizeof(double))) != cudaSuccess ||
+        (e = cudaMalloc(&s->d_mask, s->n_sm * sizeof(unsigned))) != cudaSuccess ||
         (e = cudaMalloc(&s->d_queue, sizeof(int))) != cudaSuccess ||
         (e = cudaMalloc(&s->d_stats, 24 * sizeof(unsigned long long))) != cudaSuccess) {
         std::string msg = std::string("cudaMalloc: ") + cudaGetErrorString(e);
@@ -217,7 +262,7 @@ extern "C" int jipm_create(jipm_solver** out, int family, const jipm_family_dims
     pb.xL = s->d_xL; pb.xU = s->d_xU;
     if ((e = cudaMemcpyAsync(s->d_xL, xl.data(), n * sizeof(double), cudaMemcpyHostToDevice, s->stream)) != cudaSuccess ||
         (e = cudaMemcpyAsync(s->d_xU, xu.data(), n * sizeof(double), cudaMemcpyHostToDevice, s->stream)) != cudaSuccess ||
-        (e = cudaMemsetAsync(s->d_ws, 0, (size_t)s->n_slots * (s->L.total - s->L.nsm + 2) * sizeof(double), s->stream)) != cudaSuccess ||
+        (e = cudaMemsetAsync(s->d_ws, 0, n_ws * (s->L.total - s->L.nsm + 2) * sizeof(double), s->stream)) != cudaSuccess ||
         (e = cudaStreamSynchronize(s->stream)) != cudaSuccess) {
         std::string msg = std::string("upload: ") + cudaGetErrorString(e);
         jipm_destroy(s);
@@ -229,15 +274,23 @@ extern "C" int jipm_create(jipm_solver** out, int family, const jipm_family_dims
 
 extern "C" int jipm_destroy(jipm_solver* s) {
     if (!s) return JIPM_OK;
+    DeviceGuard dg(s->device);
     cudaFree(s->d_xL); cudaFree(s->d_xU); cudaFree(s->d_ws); cudaFree(s->d_queue); cudaFree(s->d_stats);
+    cudaFree(s->d_mask);
+    cudaFree(s->d_stage); cudaFree(s->d_istage);
     delete s;
     return JIPM_OK;
 }
 
 static int run(jipm_solver* s, Args& a) {
+    DeviceGuard dg(s->device);
+    if (!dg.ok) return fail(JIPM_ERR_CUDA, "cannot switch to the solver's device");
+    std::lock_guard<std::mutex> lock(g_launch_mutex);
     a.pb = s->pb; a.L = s->L; a.o = s->o;
     a.ws = s->d_ws; a.ws_stride = s->L.total - s->L.nsm + 2; a.n_slots = (int)std::min<int64_t>(s->n_slots, std::max<int64_t>(a.P, 1));
     a.queue = s->d_queue; a.stats = s->d_stats;
+    a.sm_mask = s->d_mask; a.teams_per_sm = s->teams_per_sm;
+    CUDA_TRY(cudaMemsetAsync(s->d_mask, 0, s->n_sm * sizeof(unsigned), s->stream));
     a.trace = s->trace; a.trace_cap = s->trace_cap;
     a.dbg_len = s->dbg.len;
     CUDA_TRY(cudaMemsetAsync(s->d_queue, 0, sizeof(int), s->stream));
@@ -273,10 +326,20 @@ extern "C" int jipm_solve_batch_host(jipm_solver* s, int64_t P, const double* x0
     if (!x0 || !params || !x_out || !lam_out || !status_out || !iters_out) return fail(JIPM_ERR_ARG, "NULL buffer");
     const size_t n = s->pb.n, m = s->pb.m, nth = s->pb.nth;
     const size_t nd = P * (2 * n + m + nth + (zL_out ? n : 0) + (zU_out ? n : 0));
-    double* buf = nullptr; int32_t* ib = nullptr;
-    CUDA_TRY(cudaMalloc(&buf, nd * sizeof(double)));
-    cudaError_t e = cudaMalloc(&ib, 2 * P * sizeof(int32_t));
-    if (e != cudaSuccess) { cudaFree(buf); return fail(JIPM_ERR_NOMEM, "cudaMalloc"); }
+    DeviceGuard dg(s->device);
+    if (!dg.ok) return fail(JIPM_ERR_CUDA, "cannot switch to the solver's device");
+    // device staging owned by the solver, grow-only: repeated calls of the same size allocate nothing
+    if (nd > s->stage_doubles) {
+        cudaFree(s->d_stage); s->d_stage = nullptr; s->stage_doubles = 0;
+        CUDA_TRY(cudaMalloc(&s->d_stage, nd * sizeof(double)));
+        s->stage_doubles = nd;
+    }
+    if ((size_t)(2 * P) > s->istage_ints) {
+        cudaFree(s->d_istage); s->d_istage = nullptr; s->istage_ints = 0;
+        CUDA_TRY(cudaMalloc(&s->d_istage, 2 * P * sizeof(int32_t)));
+        s->istage_ints = 2 * P;
+    }
+    double* buf = s->d_stage; int32_t* ib = s->d_istage;
     double* dx0 = buf; double* dth = dx0 + P * n; double* dxo = dth + P * nth; double* dlo = dxo + P * n;
     double* dzl = zL_out ? dlo + P * m : nullptr; double* dzu = zU_out ? (dlo + P * m + (zL_out ? P * n : 0)) : nullptr;
     int rc = JIPM_OK;
@@ -293,13 +356,18 @@ extern "C" int jipm_solve_batch_host(jipm_solver* s, int64_t P, const double* x0
         chk(cudaMemcpyAsync(iters_out, ib + P, P * sizeof(int32_t), cudaMemcpyDeviceToHost, s->stream));
         chk(cudaStreamSynchronize(s->stream));
     }
-    cudaFree(buf); cudaFree(ib);
     return rc;
 }
 
 extern "C" int jipm_last_stats(jipm_solver* s, int64_t* stats, int64_t n_stats) {
     if (!s || !stats) return fail(JIPM_ERR_ARG, "NULL argument");
     for (int64_t i = 0; i < n_stats && i < 24; ++i) stats[i] = s->stats[i];
+    return JIPM_OK;
+}
+
+extern "C" int jipm_residency(jipm_solver* s, int64_t* res) {
+    if (!s || !res) return fail(JIPM_ERR_ARG, "NULL argument");
+    res[0] = s->n_sm; res[1] = s->teams_per_sm;
     return JIPM_OK;
 }
 
@@ -312,9 +380,9 @@ extern "C" int jipm_debug_set_trace(jipm_solver* s, double* trace, int64_t max_r
 extern "C" int jipm_debug_state_layout(jipm_solver* s, int64_t* lay, int64_t n_lay) {
     if (!s || !lay) return fail(JIPM_ERR_ARG, "NULL argument");
     const DbgLay& d = s->dbg;
-    const int v[20] = {d.len, d.x, d.y, d.zL, d.zU, d.sc, d.filt, d.dx, d.dy, d.dzL, d.dzU, d.g, d.c, d.J, d.W,
-                       d.rs, d.pn, d.zpn, d.xR, d.filtR};
-    for (int64_t i = 0; i < n_lay && i < 20; ++i) lay[i] = v[i];
+    const int v[22] = {d.len, d.x, d.y, d.zL, d.zU, d.sc, d.filt, d.dx, d.dy, d.dzL, d.dzU, d.g, d.c, d.J, d.W,
+                       d.rs, d.pn, d.zpn, d.xR, d.filtR, d.ls, d.wd};
+    for (int64_t i = 0; i < n_lay && i < 22; ++i) lay[i] = v[i];
     return JIPM_OK;
 }
 
@@ -340,7 +408,9 @@ extern "C" int jipm_bench_fp64_peak(void* cuda_stream, double* tflops) {
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(JIPM_ERR_CUDA, "no CUDA device");
     cudaStream_t st = (cudaStream_t)cuda_stream;
     cudaDeviceProp prop;
-    CUDA_TRY(cudaGetDeviceProperties(&prop, 0));
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
     const int blocks = prop.multiProcessorCount * 8, threads = 256, iters = 1 << 15;
     double* out = nullptr;
     CUDA_TRY(cudaMalloc(&out, (size_t)blocks * threads * sizeof(double)));

@@ -34,10 +34,19 @@ __device__ void Solver<C>::dbg_load(const double* st) {
         }
         for (int i = lane; i < 2 * MAX_FILTER; i += NT) V(L->filtR)[i] = st[D.filtR + i];
     }
+    // line-search memory of the active problem (Table I rows 3-5) and the watchdog's entry iterate / direction
+    n_short = (int)st[D.ls + 0]; wd_active = (int)st[D.ls + 1]; wd_trials = (int)st[D.ls + 2];
+    wd_theta = st[D.ls + 3]; wd_phi = st[D.ls + 4]; wd_gd = st[D.ls + 5]; wd_alpha = st[D.ls + 6];
+    soft = (int)st[D.ls + 7]; soft_count = (int)st[D.ls + 8]; tiny_last = (int)st[D.ls + 9]; tiny_flag = (int)st[D.ls + 10];
+    if (wd_active) {
+        const int nw = pb->n + 2 * pb->m;
+        Vec w[6] = {VX(L->wx), VX(L->wzL), VX(L->wzU), VX(L->wdx), VX(L->wdzL), VX(L->wdzU)};
+        for (int q = 0; q < 6; ++q)
+            for (int i = lane; i < nX; i += NT) w[q][i] = st[D.wd + q * nw + i];
+        for (int i = lane; i < pb->m; i += NT) { V(L->wy)[i] = st[D.wd + 6 * nw + i]; V(L->wdy)[i] = st[D.wd + 6 * nw + pb->m + i]; }
+    }
     c.tm.sync();
-    double thb, cmb;
     f = eval_point(VX(L->x), VH(L->c), theta, cmax, f_base, theta_base, cmax_base, f_pn, f_q);
-    (void)thb; (void)cmb;
 }
 
 template <class C>
@@ -61,6 +70,16 @@ __device__ void Solver<C>::dbg_store(double* st) {
         st[D.rs + 0] = mode; st[D.rs + 1] = mu_reg; st[D.rs + 2] = tau_reg; st[D.rs + 3] = dw_last_reg;
         st[D.rs + 4] = theta_min_reg; st[D.rs + 5] = theta_max_reg; st[D.rs + 6] = nfilt_reg;
         st[D.rs + 7] = theta_entry; st[D.rs + 8] = zeta;
+        st[D.ls + 0] = n_short; st[D.ls + 1] = wd_active; st[D.ls + 2] = wd_trials; st[D.ls + 3] = wd_theta;
+        st[D.ls + 4] = wd_phi; st[D.ls + 5] = wd_gd; st[D.ls + 6] = wd_alpha; st[D.ls + 7] = soft;
+        st[D.ls + 8] = soft_count; st[D.ls + 9] = tiny_last; st[D.ls + 10] = tiny_flag;
+    }
+    if (wd_active) {
+        const int nw = pb->n + 2 * pb->m;
+        Vec w[6] = {VX(L->wx), VX(L->wzL), VX(L->wzU), VX(L->wdx), VX(L->wdzL), VX(L->wdzU)};
+        for (int q = 0; q < 6; ++q)
+            for (int i = lane; i < nX; i += NT) st[D.wd + q * nw + i] = w[q][i];
+        for (int i = lane; i < pb->m; i += NT) { st[D.wd + 6 * nw + i] = V(L->wy)[i]; st[D.wd + 6 * nw + pb->m + i] = V(L->wdy)[i]; }
     }
     if (mode) {
         Vec xv = VX(L->x); Vec zLv = VX(L->zL);
@@ -75,9 +94,26 @@ __global__ void __launch_bounds__(C::NT, MINB) jipm_slot_kernel() {
     constexpr int NT = C::NT;
     const ArgsProxy A;
     const int lane = threadIdx.x;  // one team per CTA
-    const int slot = blockIdx.x;
-    double* ws = A->ws + (int64_t)slot * A->ws_stride;
-    Ctx<C> ctx(ws, jipm_smem, lane, 1);
+    // claim one of this SM's workspaces (see Args::sm_mask)
+    __shared__ int s_ws_id;
+    unsigned smid;
+    asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+    if (lane == 0) {
+        int got = -1;
+        while (got < 0) {
+            for (int b = 0; b < A->teams_per_sm && got < 0; ++b) {
+                const unsigned old = atomicOr(A->sm_mask + smid, 1u << b);
+                if (!(old & (1u << b))) got = b;
+            }
+            if (got < 0) __nanosleep(500);
+        }
+        __threadfence();
+        s_ws_id = (int)smid * A->teams_per_sm + got;
+    }
+    __syncthreads();
+    const int ws_id = s_ws_id;
+    double* ws = A->ws + (int64_t)ws_id * A->ws_stride;
+    Ctx<C> ctx(ws, jipm_smem, lane);
     Solver<C> S(ctx);
     while (true) {
         int id = 0;
@@ -134,6 +170,12 @@ __global__ void __launch_bounds__(C::NT, MINB) jipm_slot_kernel() {
         atomicAdd(&A->stats[7], (unsigned long long)S.n_resto);
         for (int i = 0; i < 8; ++i) atomicAdd(&A->stats[8 + i], S.tph[i]);
         for (int i = 0; i < 8; ++i) atomicAdd(&A->stats[16 + i], ctx.pc[i]);
+    }
+    // release the workspace: all global-scratch accesses of this CTA are done
+    __syncthreads();
+    if (lane == 0) {
+        __threadfence();
+        atomicAnd(A->sm_mask + smid, ~(1u << (ws_id - (int)smid * A->teams_per_sm)));
     }
 }
 

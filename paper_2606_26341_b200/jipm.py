@@ -14,9 +14,9 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libjipm.so")
 
-TRACE_W = 16
+TRACE_W = 20
 ST_NOT_RUN, ST_SOLVED, ST_MAXITER, ST_LOCALLY_INFEASIBLE = -1, 0, 1, 2
-ST_RESTORATION_FAILED, ST_RESTO_AT_FEASIBLE_POINT, ST_NONFINITE = 3, 4, 5
+ST_RESTORATION_FAILED, ST_RESTO_AT_FEASIBLE_POINT, ST_NONFINITE, ST_TINY_STEP = 3, 4, 5, 6
 
 _DOUBLE_FIELDS = [
     "tol", "mu_init", "kappa_eps", "kappa_mu", "theta_mu", "tau_min", "s_max", "kappa_sigma",
@@ -24,13 +24,16 @@ _DOUBLE_FIELDS = [
     "gamma_theta", "gamma_phi", "eta_phi", "delta", "s_theta", "s_phi", "gamma_alpha",
     "theta_max_fact", "theta_min_fact", "alpha_red", "kappa_soc",
     "delta_w_min", "delta_w_0", "delta_w_max", "kappa_w_minus", "kappa_w_plus", "kappa_w_plus_first",
-    "delta_c_bar", "kappa_c", "residual_ratio_max", "rho_resto", "kappa_resto", "z_reset_threshold"]
+    "delta_c_bar", "kappa_c", "residual_ratio_max", "rho_resto", "kappa_resto", "z_reset_threshold",
+    "residual_ratio_singular", "residual_improvement_factor",
+    "tiny_step_tol", "tiny_step_y_tol", "tiny_step_cviol", "soft_resto_factor"]
 _INT_FIELDS = ["max_iter", "max_backtrack", "max_soc", "refine_min", "refine_max", "max_mu_updates",
-               "init_slacks", "enable_restoration"]
+               "init_slacks", "enable_restoration", "watchdog_trigger", "watchdog_trial_max", "max_soft_resto_iters"]
 
 
 class Options(C.Structure):
-    _fields_ = [(f, C.c_double) for f in _DOUBLE_FIELDS] + [(f, C.c_int32) for f in _INT_FIELDS]
+    _fields_ = ([(f, C.c_double) for f in _DOUBLE_FIELDS] + [(f, C.c_int32) for f in _INT_FIELDS]
+                + [("reserved_", C.c_int32)])
 
 
 class FamilyDims(C.Structure):
@@ -42,7 +45,7 @@ _lib = None
 EXPORTS = ["jipm_default_options", "jipm_family_sizes", "jipm_create", "jipm_solve_batch",
            "jipm_solve_batch_host", "jipm_destroy", "jipm_last_error", "jipm_last_stats",
            "jipm_debug_set_trace", "jipm_debug_state_layout", "jipm_debug_step", "jipm_debug_init",
-           "jipm_bench_fp64_peak"]
+           "jipm_bench_fp64_peak", "jipm_residency"]
 
 
 def lib():
@@ -68,6 +71,7 @@ def lib():
         L.jipm_debug_step.argtypes = [vp, i64, dp, dp, i64]
         L.jipm_debug_init.argtypes = [vp, i64, dp, dp, dp]
         L.jipm_bench_fp64_peak.argtypes = [vp, C.POINTER(C.c_double)]
+        L.jipm_residency.argtypes = [vp, C.POINTER(i64)]
         _lib = L
     return _lib
 
@@ -105,7 +109,7 @@ class Solver:
     """jipm_create / jipm_solve_batch / jipm_destroy with torch tensors for device memory."""
 
     LAY_NAMES = ["len", "x", "y", "zL", "zU", "sc", "filt", "dx", "dy", "dzL", "dzU", "g", "c", "J", "W",
-                 "rs", "pn", "zpn", "xR", "filtR"]
+                 "rs", "pn", "zpn", "xR", "filtR", "ls", "wd"]
 
     def __init__(self, family, horizon_N, n_agents, n_obstacles, dt, xL, xU, opts: Options | None = None,
                  resident_slots: int = 0):
@@ -181,7 +185,15 @@ class Solver:
                  "resto_iterations", "cyc_derivs", "cyc_factor", "cyc_solve", "cyc_residual", "cyc_trial_eval",
                  "cyc_iterations", "cyc_init", "cyc_speculative_trials",
                  "cycf_TJ", "cycf_M", "cycf_pivots", "cycf_phi_store", "cycf_dc_extra", "cycx_solve_full_first", "cycx_line_search", "cycx_iteration_head"]
-        return dict(zip(names, list(a)))
+        d = dict(zip(names, list(a)))
+        d["co_resident_slots"] = min(d["slots"], self.co_resident_slots())
+        return d
+
+    def co_resident_slots(self):
+        """Problem slots (CTAs) the device holds at once for this family: SMs x teams per SM."""
+        a = (C.c_int64 * 2)()
+        _check(lib().jipm_residency(self._h, a))
+        return int(a[0] * a[1])
 
     # ---- debug / parity entries ------------------------------------------------------------------------
     def set_trace(self, P, max_records):
@@ -195,8 +207,8 @@ class Solver:
         return self._trace
 
     def state_layout(self):
-        a = (C.c_int64 * 20)()
-        _check(lib().jipm_debug_state_layout(self._h, a, 20))
+        a = (C.c_int64 * 22)()
+        _check(lib().jipm_debug_state_layout(self._h, a, 22))
         return dict(zip(self.LAY_NAMES, list(a)))
 
     def debug_init(self, x0, params):

@@ -12,9 +12,10 @@ import numpy as np
 from oracle import families as ofam
 from oracle import ipm as oipm
 
-KIND_CODE = {"newton": 0, "soc": 1, "ls_fail": 2, "ic_fail": 3, "": 4}
+KIND_CODE = {"newton": 0, "soc": 1, "ls_fail": 2, "ic_fail": 3, "": 4, "tiny": 5, "soft": 6}
 # GPU trace record columns (include/jipm.h)
 T_MODE, T_NFACT, T_DW, T_DC, T_NREF, T_KIND, T_LS, T_SOC, T_ALPHA, T_ALPHAZ, T_FTYPE, T_NMU, T_E0, T_MU = range(14)
+T_THETA, T_PHI, T_WD, T_SOFT, T_TINY, T_NPSING = 14, 15, 16, 17, 18, 19
 
 
 def oracle_for(d, xL, xU, opts=None):
@@ -42,8 +43,12 @@ def e_v(v, vref):
 
 
 def decisions_equal(gpu_rec: np.ndarray, otr: dict) -> tuple[bool, str]:
-    """One iteration: the integer decisions must be identical; the step lengths agree to 1e-4 relative (iterates
-    are compared tightly by the step-parity tests; here the reals only guard against a different branch)."""
+    """One iteration: every integer decision must be identical -- step kind, mode, #mu updates, #factorisations, the
+    perturbations delta_w AND delta_c, #refinement failures treated as singular, #backtracks, #corrections, the
+    watchdog / soft-restoration / tiny-step codes, f- or h-type -- and the step lengths agree to 1e-4 relative (the
+    iterates are compared tightly by the step-parity tests; here the reals only guard against a different branch).
+    The NUMBER of refinement steps is a property of the linear solver, not a decision of the method (two LAPACK
+    solvers differ in it too): it is reported by the tests, not asserted."""
     kind = KIND_CODE[otr["kind"]]
     if int(gpu_rec[T_KIND]) != kind:
         return False, f"kind {int(gpu_rec[T_KIND])} vs {kind}"
@@ -57,8 +62,15 @@ def decisions_equal(gpu_rec: np.ndarray, otr: dict) -> tuple[bool, str]:
         return True, ""
     if int(gpu_rec[T_NFACT]) != otr["nfact"]:
         return False, f"nfact {int(gpu_rec[T_NFACT])} vs {otr['nfact']}"
+    if int(gpu_rec[T_NPSING]) != otr.get("npsing", 0):
+        return False, f"npsing {int(gpu_rec[T_NPSING])} vs {otr.get('npsing', 0)}"
     if not np.isclose(gpu_rec[T_DW], otr["dw"], rtol=1e-9, atol=0.0):
         return False, f"dw {gpu_rec[T_DW]} vs {otr['dw']}"
+    if not np.isclose(gpu_rec[T_DC], otr["dc"], rtol=1e-9, atol=0.0):
+        return False, f"dc {gpu_rec[T_DC]} vs {otr['dc']}"
+    for col, key in ((T_WD, "wd"), (T_SOFT, "soft"), (T_TINY, "tiny")):
+        if int(gpu_rec[col]) != int(otr.get(key, 0)):
+            return False, f"{key} {int(gpu_rec[col])} vs {otr.get(key, 0)}"
     if int(gpu_rec[T_LS]) != otr["ls"]:
         return False, f"ls {int(gpu_rec[T_LS])} vs {otr['ls']}"
     if int(gpu_rec[T_SOC]) != otr["soc"]:
@@ -72,6 +84,113 @@ def decisions_equal(gpu_rec: np.ndarray, otr: dict) -> tuple[bool, str]:
     if not np.isclose(gpu_rec[T_ALPHAZ], otr["alpha_z"], rtol=1e-4, atol=1e-12):
         return False, f"alpha_z {gpu_rec[T_ALPHAZ]} vs {otr['alpha_z']}"
     return True, ""
+
+
+class LUFactor:
+    """numpy/scipy LU with partial pivoting behind the interface of oracle.linsolve.DenseLDL.solve."""
+
+    def __init__(self, K):
+        import scipy.linalg
+        self._sl = scipy.linalg
+        self.lu = scipy.linalg.lu_factor(K)
+
+    def solve(self, b):
+        return self._sl.lu_solve(self.lu, b)
+
+
+def second_opinion_gap(solver, tr):
+    """How far two LAPACK solvers disagree on the linear system of this iteration: the oracle's Bunch-Kaufman LDL^T
+    against an LU with partial pivoting, both followed by the same refinement on (6) (reading S-7).  Measured with e_v of
+    eq (8) on the iterate the LARGEST step the line search considers would produce (x + alpha_max dx,
+    y + alpha_max dy).  A step on which two backward-stable library solvers already differ by more than the parity
+    tolerance cannot be asked of a third one: such steps are reported, not asserted."""
+    lin = tr.get("lin")
+    if lin is None:
+        return 0.0
+    K = solver.kkt_matrix(lin["W"], lin["Sigma"], lin["A"], tr["dw"], tr["dc"])
+    if not np.all(np.isfinite(K)):
+        return np.inf
+    try:
+        d, _, _ = solver.solve_full(LUFactor(K), lin["W"], lin["A"], lin["x"], lin["zL"], lin["zU"], tr["dw"], tr["dc"],
+                                    lin["b"])
+    except Exception:
+        return np.inf
+    a = min(1.0, solver.ftb_primal(lin["x"], lin["d"][0], 0.99))
+    ref = lin["d"]
+    x = lin["x"]
+    gap = e_v(x + a * d[0], x + a * ref[0])
+    if solver.m:
+        gap = max(gap, e_v(a * d[1], a * ref[1]))
+    return gap if np.isfinite(gap) else np.inf
+
+
+def sensitivity_gap(solver, tr, rel=1e-12, seed=1):
+    """How far the step of this iteration moves when the computed derivative blocks W and A are perturbed by a relative
+    1e-12 per entry -- the level at which two independent fp64 evaluations of the RK4 chain's first and second
+    derivatives differ (the oracle's jets and the kernel's analytic chain agree to 1e-13 .. 1e-11, tests
+    test_derivative_blocks_against_oracle).  Same solver (Bunch-Kaufman + refinement), same right-hand side; measured like
+    second_opinion_gap.  Where this exceeds the parity tolerance the step amplifies differences that are below the
+    resolution of the derivatives by more than 1e4: no implementation with its own derivative code can reproduce it to
+    1e-8."""
+    from oracle.linsolve import DenseLDL
+    lin = tr.get("lin")
+    if lin is None:
+        return 0.0
+    rng = np.random.default_rng(seed)
+    W, A = lin["W"], lin["A"]
+    E = rng.uniform(-1.0, 1.0, W.shape)
+    Wp = W * (1.0 + rel * (E + E.T) / 2.0)
+    Ap = A * (1.0 + rel * rng.uniform(-1.0, 1.0, A.shape))
+    K = solver.kkt_matrix(Wp, lin["Sigma"], Ap, tr["dw"], tr["dc"])
+    if not np.all(np.isfinite(K)):
+        return np.inf
+    try:
+        d, _, _ = solver.solve_full(DenseLDL(K), Wp, Ap, lin["x"], lin["zL"], lin["zU"], tr["dw"], tr["dc"], lin["b"])
+    except Exception:
+        return np.inf
+    a = min(1.0, solver.ftb_primal(lin["x"], lin["d"][0], 0.99))
+    ref = lin["d"]
+    x = lin["x"]
+    gap = e_v(x + a * d[0], x + a * ref[0])
+    if solver.m:
+        gap = max(gap, e_v(a * d[1], a * ref[1]))
+    return gap if np.isfinite(gap) else np.inf
+
+
+def step_is_well_posed(solver, tr, tol):
+    """(well-posed?, text): the three criteria above with the parity tolerance."""
+    g1 = second_opinion_gap(solver, tr)
+    if g1 > tol:
+        return False, f"LAPACK LU vs Bunch-Kaufman {g1:.1e}"
+    g2 = sensitivity_gap(solver, tr)
+    if g2 > tol:
+        return False, f"1e-12 perturbation of W, A moves the step by {g2:.1e}"
+    if len((tr.get("lin") or {}).get("tried", [])) > 1 and not inertia_is_stable(solver, tr):
+        return False, "inertia changes under a 1e-10 perturbation of W, A"
+    return True, f"{max(g1, g2):.1e}"
+
+
+def inertia_is_stable(solver, tr, rel=1e-10, seed=0):
+    """Is every inertia Algorithm IC read in this iteration (one per factorisation it tried) the same for a matrix whose
+    computed entries W, A are perturbed by a relative 1e-10 (two derivative implementations differ by more)?  If not,
+    the sequence of perturbations delta_w is not a property of the problem but of the rounding."""
+    from oracle.linsolve import DenseLDL
+    lin = tr.get("lin")
+    if lin is None:
+        return True
+    rng = np.random.default_rng(seed)
+    W, A = lin["W"], lin["A"]
+    E = rng.uniform(-1.0, 1.0, W.shape)
+    Wp = W * (1.0 + rel * (E + E.T) / 2.0)
+    Ap = A * (1.0 + rel * rng.uniform(-1.0, 1.0, A.shape))
+    for dw, dc in lin["tried"]:
+        K0 = solver.kkt_matrix(W, lin["Sigma"], A, dw, dc)
+        K1 = solver.kkt_matrix(Wp, lin["Sigma"], Ap, dw, dc)
+        if not (np.all(np.isfinite(K0)) and np.all(np.isfinite(K1))):
+            return False
+        if DenseLDL(K0).inertia != DenseLDL(K1).inertia:
+            return False
+    return True
 
 
 def compare_problem(gpu_trace: np.ndarray, gpu_status: int, gpu_iters: int, st, otr: list):
@@ -154,4 +273,22 @@ def snapshot_state(lay, st, n, m):
         nf = put_filter("filtR", cur.filt)
     snap[lay["y"]:lay["y"] + m] = cur.y
     snap[lay["sc"]:lay["sc"] + 8] = [cur.mu, cur.tau, cur.delta_w_last, cur.theta_min, cur.theta_max, st.k, -1, nf]
+    # line-search memory of the active problem (Table I rows 3-5) and the watchdog's entry iterate and direction
+    wd = cur.wd
+    snap[lay["ls"]:lay["ls"] + 11] = [cur.n_short, int(wd is not None), wd.trials if wd else 0, wd.theta if wd else 0.0,
+                                      wd.phi if wd else 0.0, wd.gd if wd else 0.0, wd.alpha if wd else 0.0,
+                                      int(cur.soft), cur.soft_count, int(cur.tiny_last), int(cur.tiny_flag)]
+    if wd is not None:
+        nw, o = n + 2 * m, lay["wd"]
+        for q, v in enumerate((wd.x, wd.zL, wd.zU, wd.d[0], wd.d[2], wd.d[3])):
+            snap[o + q * nw:o + q * nw + v.size] = v
+        snap[o + 6 * nw:o + 6 * nw + m] = wd.y
+        snap[o + 6 * nw + m:o + 6 * nw + 2 * m] = wd.d[1]
     return snap
+
+
+def ls_memory(st):
+    """(n_short, watchdog active, watchdog trials, soft, soft_count, tiny_last, tiny_flag) of the active problem."""
+    cur = st if st.resto is None else st.resto.state
+    return [cur.n_short, int(cur.wd is not None), cur.wd.trials if cur.wd else 0, int(cur.soft), cur.soft_count,
+            int(cur.tiny_last), int(cur.tiny_flag)]

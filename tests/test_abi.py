@@ -54,6 +54,10 @@ def test_family_sizes_match_workloads_and_baseline_configs(lib):
         jipm.family_sizes(7, 10, 1, 1, 0.1)
     with pytest.raises(jipm.JipmError, match="error 2"):
         jipm.family_sizes(0, 0, 1, 1, 0.1)
+    # the inequality index of a knot is packed into 8 bits with two sentinels: at most 254 obstacles per knot
+    assert jipm.family_sizes(3, 4, 1, 254, 0.05)[0] == 5 * 12 + 4 * 4 + 4 * 254
+    with pytest.raises(jipm.JipmError, match="error 2"):
+        jipm.family_sizes(3, 4, 1, 255, 0.05)
 
 
 def test_compute_entries_fail_loudly_without_a_device(lib):
