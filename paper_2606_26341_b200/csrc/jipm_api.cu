@@ -216,6 +216,9 @@ extern "C" int jipm_create(jipm_solver** out, int family, const jipm_family_dims
             if (!strcmp(ev, "q1b")) { s->inst = inst_q1b(); forced_inst = true; }
             if (!strcmp(ev, "q1c")) { s->inst = inst_q1c(); forced_inst = true; }
             if (!strcmp(ev, "q1g")) { s->inst = inst_q1g(); forced_inst = true; }
+            if (!strcmp(ev, "q1d")) { s->inst = inst_q1d(); forced_inst = true; }
+            if (!strcmp(ev, "q1e")) { s->inst = inst_q1e(); forced_inst = true; }
+            if (!strcmp(ev, "q1h")) { s->inst = inst_q1h(); forced_inst = true; }
         }
     }
     cudaDeviceProp prop;

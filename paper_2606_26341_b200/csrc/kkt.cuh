@@ -44,6 +44,18 @@ struct Kkt {
         else return p / AU;
     }
 
+    // Tile loop with a compile-time trip count: thread `lane` visits the elements lane, lane + NT, ... of an NE-element
+    // tile.  Fully unrolled, so that the independent dependent-chains of a thread's elements interleave (a team of 128
+    // or 64 threads owns 2 - 4 elements of a 16 x 16 tile; run one after the other they would double the phase's latency).
+    template <int NE, class F>
+    __device__ static __forceinline__ void tile_for(int lane, F f) {
+#pragma unroll
+        for (int r = 0; r < (NE + NT - 1) / NT; ++r) {
+            const int e = lane + r * NT;
+            if (NE % NT == 0 || e < NE) f(e);
+        }
+    }
+
     // dot product with 4 independent partial sums (dependent-chain latency / 4), compile-time length and strides: fully unrolled, immediate offsets
     template <int LEN, int SA, int SB>
     __device__ static __forceinline__ double dotc(const double* a, const double* b) {
@@ -104,7 +116,7 @@ struct Kkt {
 #pragma unroll
                 for (int l = i + 1; l < G; ++l) A[j][l] -= A[j][i] * A[i][l];
         }
-        for (int e = c.lane; e < NE; e += NT) {
+        tile_for<NE>(c.lane, [&](int e) {
             const int a = e / LD, b = e % LD;
             const int ia = a - p0, ib = b - p0;
             const bool ain = ia >= 0 && ia < G, bin = ib >= 0 && ib < G;
@@ -125,7 +137,7 @@ struct Kkt {
                 D -= Cv[i] * rb;
             }
             dst[e] = D;
-        }
+        });
     }
     // pivots p0 .. p0+n-1 in groups of four (then two, then one); src / dst are swapped after every phase
     template <int LD, int NE, int NP>
@@ -161,11 +173,11 @@ struct Kkt {
         double* dst = wk + NX * NX;
         first();
         gj_range<NX, NX * NX, NX>(c, src, dst, 0, bad, nzero);
-        for (int e = c.lane; e < NX * NX; e += NT) {
+        tile_for<NX * NX>(c.lane, [&](int e) {
             const int i = e / NX, q = e % NX;
             const double v = 0.5 * (dotc<NX, 1, LDP>(src + i * NX, Pm + q) + dotc<NX, 1, LDP>(src + q * NX, Pm + i));
             sT[e] = v; Tg[e] = v;
-        }
+        });
         c.tm.sync();
     }
 
@@ -231,16 +243,16 @@ struct Kkt {
                 c.tm.sync();
             }
             // TJ = T_{k+1} J_k
-            for (int e = lane; e < NX * NZ; e += NT) {
+            tile_for<NX * NZ>(lane, [&](int e) {
                 const int l = e / NZ, j = e % NZ;
                 const int aj = col_agent(j);
                 sTJ[e] = dotc<AX, 1, LDJ>(sT + l * NX + AX * aj, sJ + AX * aj * LDJ + j);
-            }
+            });
             c.tm.sync();
             { const long long t2 = clock64(); c.pc[0] += t2 - tq; tq = t2; }
             // M = Q_k + J^T (T J) + condensed slacks
             const double* Wg = c.Wk(k);
-            for (int e = lane; e < NZ * NZ; e += NT) {
+            tile_for<NZ * NZ>(lane, [&](int e) {
                 const int a = e / NZ, j = e % NZ;
                 const int aa = col_agent(a);
                 double m = dotc<AX, LDJ, NZ>(sJ + AX * aa * LDJ + a, sTJ + AX * aa * NZ + j);
@@ -249,7 +261,7 @@ struct Kkt {
                 if (k >= 1 && ng > 0 && a < NX && j < NX && a % AX < PD && j % AX < PD)
                     m += cnd[(k - 1) * NPOS * NPOS + (PD * (a / AX) + a % AX) * NPOS + PD * (j / AX) + j % AX];
                 tA[e] = m;
-            }
+            });
             c.tm.sync();
             { const long long t2 = clock64(); c.pc[1] += t2 - tq; tq = t2; }
             // Gauss-Jordan pivots on the controls NX .. NZ-1, four per barrier: every element from the previous tile
@@ -262,7 +274,7 @@ struct Kkt {
             double* Pg = c.vh(c.L->Psi) + k * NX * NX;
             double* Tg = c.vh(c.L->T) + k * NX * NX;
             const int r1 = c.icd(k);
-            for (int e = lane; e < NX * NX; e += NT) {
+            tile_for<NX * NX>(lane, [&](int e) {
                 const int i = e / NX, a = e % NX;
                 const int ai = row_agent(i);
                 const double phi = sJ[i * LDJ + a] - dotc<AU, 1, NZ>(sJ + i * LDJ + NX + AU * ai, src + (NX + AU * ai) * NZ + a);
@@ -280,7 +292,7 @@ struct Kkt {
                     const double tn = 0.5 * (src[i * NZ + a] + src[a * NZ + i]);
                     sT[e] = tn; Tg[e] = tn;
                 }
-            }
+            });
             for (int e = lane; e < NU * NX; e += NT) Kg[e] = src[(NX + e / NX) * NZ + e % NX];
             for (int e = lane; e < NU * NU; e += NT) Gg[e] = src[(NX + e / NU) * NZ + NX + e % NU];
             c.tm.sync();
@@ -289,10 +301,10 @@ struct Kkt {
                 // Psi = (I - D_{k+1} T_{k+1}) Phi inside the first pivot phase, then P_k -> T_k = (I + P_k D_k)^{-1} P_k
                 const int r0 = c.icd(k + 1);
                 transform_T<NZ>(c, dst, src, sT, Tg, bad, nzero, [&] {
-                    for (int e = lane; e < NX * NX; e += NT) {
+                    tile_for<NX * NX>(lane, [&](int e) {
                         const int i = e / NX, a = e % NX;
                         Pg[e] = sTJ[e] - Dc[r0 + i] * dotc<NX, 1, NX>(sT + i * NX, sTJ + a);
-                    }
+                    });
                 });
                 c.pc[4] += clock64() - tq;
             }
@@ -367,6 +379,7 @@ struct Kkt {
         double* hv = c.vh(c.L->tv);    // N x NU     : h_k, then uo_k, then u_k
         double* sv = c.vh(c.L->sv);    // N x NX     : scratch (st_k, B uo_k, A x_k + B u_k)
         // ---- phase 0a ----
+#pragma unroll 2
         for (int e = lane; e < (N + 1) * NX; e += NT) {
             const int k = e / NX, i = e % NX;
             double v = rp[c.ix(k) + i];
@@ -374,12 +387,14 @@ struct Kkt {
             if (k >= 1 && ii < PD && pb->ng > 0) v += cond_rhs(c, rp, rc, k, ag, ii);
             pv[e] = v;
         }
+#pragma unroll 2
         for (int e = lane; e < N * NX; e += NT) {
             const int k = e / NX, i = e % NX;
             wv[e] = dotc<NX, NX, 1>(Tf + (k + 1) * NX * NX + i, rc + c.icd(k + 1));  // T symmetric
         }
         c.tm.sync();
         // ---- phase 0b: h_k ----
+#pragma unroll 2
         for (int e = lane; e < N * NU; e += NT) {
             const int k = e / NU, p = e % NU;
             const int ap = ctl_agent(p);
@@ -387,6 +402,7 @@ struct Kkt {
         }
         c.tm.sync();
         // ---- phase 0c: q_k ----
+#pragma unroll 2
         for (int e = lane; e < N * NX; e += NT) {
             const int k = e / NX, i = e % NX;
             const int ai = row_agent(i);
@@ -412,23 +428,27 @@ struct Kkt {
             for (int e = lane; e < N * NX; e += NT) wv[e] -= pv[e + NX];
         }
         c.tm.sync();
+#pragma unroll 2
         for (int e = lane; e < N * NU; e += NT) {
             const int k = e / NU, p = e % NU;
             const int ap = ctl_agent(p);
             sv[e] = rp[c.iu(k) + p] - dotc<AX, LDJ, 1>(c.Jk(k) + AX * ap * LDJ + NX + p, wv + k * NX + AX * ap);  // st_k
         }
         c.tm.sync();
+#pragma unroll 2
         for (int e = lane; e < N * NU; e += NT) {
             const int k = e / NU, p = e % NU;
             hv[e] = dotc<NU, 1, 1>(Gf + k * NU * NU + p * NU, sv + k * NU);  // uo_k = G st_k
         }
         c.tm.sync();
+#pragma unroll 2
         for (int e = lane; e < N * NX; e += NT) {
             const int k = e / NX, i = e % NX;
             const int ai = row_agent(i);
             sv[e] = dotc<AU, 1, 1>(c.Jk(k) + i * LDJ + NX + AU * ai, hv + k * NU + AU * ai);  // B uo_k   (st_k is dead)
         }
         c.tm.sync();
+#pragma unroll 2
         for (int e = lane; e < N * NX; e += NT) {
             const int k = e / NX, i = e % NX, r0 = c.icd(k + 1);
             double v = sv[e] + rc[r0 + i];
@@ -457,12 +477,14 @@ struct Kkt {
         c.tm.sync();
         // ---- phase 4 ----
         for (int e = lane; e < N * NX; e += NT) dx[c.ix(e / NX + 1) + e % NX] = pv[e + NX];
+#pragma unroll 2
         for (int e = lane; e < N * NU; e += NT) {
             const int k = e / NU, p = e % NU;
             const double u = hv[e] - dotc<NX, 1, 1>(Kf + k * NU * NX + p * NX, pv + k * NX);
             hv[e] = u; dx[c.iu(k) + p] = u;
         }
         c.tm.sync();
+#pragma unroll 2
         for (int e = lane; e < N * NX; e += NT) {
             const int k = e / NX, i = e % NX;
             const int ai = row_agent(i);
@@ -470,6 +492,7 @@ struct Kkt {
                     dotc<AU, 1, 1>(c.Jk(k) + i * LDJ + NX + AU * ai, hv + k * NU + AU * ai);
         }
         c.tm.sync();
+#pragma unroll 2
         for (int e = lane; e < N * NX; e += NT) {
             const int k = e / NX, i = e % NX;
             const double nu = wv[e] + dotc<NX, NX, 1>(Tf + (k + 1) * NX * NX + i, sv + k * NX);
