@@ -32,7 +32,8 @@ struct Cfg {
     static constexpr int SM_G_END = SM_G + (Dyn::AX == 12 ? NGRP * 7 * 16 : 0);
     static constexpr int SM_RED = (SM_TILE_END > SM_G_END) ? SM_TILE_END : SM_G_END;
     static constexpr int SM_SPEC = SM_RED + 2 * (NT / 32) + 2;  // (theta, phi) of the speculative trials, one pair per warp
-    static constexpr int SM_TOTAL = SM_SPEC + 2 * (NT / 32);
+    static constexpr int SM_CNT = SM_SPEC + 2 * (NT / 32);  // 16 diagnostic cycle counters (64-bit), written by thread 0
+    static constexpr int SM_TOTAL = SM_CNT + 16;
 };
 
 template <class C>
@@ -52,11 +53,19 @@ struct Ctx {
     //   imap[i] of primal entry i: (k << 16) | (j << 8) | a   a < NZ: entry a of z_k = (x_k, u_k); a = 255: slack j of knot k
     //   cmap[r] of equality row r: (k << 16) | (j << 8) | rr  rr < NX: row rr of dyn_{k+1}; 255: inequality j of knot k; 254: x_0 row
     const int* imap; const int* cmap;
-    mutable unsigned long long pc[8];  // diagnostic cycle counters of the factorisation's sub-phases (stats[16..23])
+    // Diagnostic cycle counters live in shared memory and only thread 0 updates them (as registers of every thread they
+    // cost 32 registers of a kernel that is register-bound): 0-7 = phases of the iteration (stats[8..15]), 8-15 = the
+    // factorisation's sub-phases and iteration blocks (stats[16..23]).
+    __device__ __forceinline__ void tick(int idx, long long cycles) const {
+        if (lane == 0) reinterpret_cast<unsigned long long*>(jipm_smem + C::SM_CNT)[idx] += (unsigned long long)cycles;
+    }
+    __device__ __forceinline__ unsigned long long counter(int idx) const {
+        return reinterpret_cast<unsigned long long*>(jipm_smem + C::SM_CNT)[idx];
+    }
 
     __device__ Ctx(double* ws_, double* sm_, int tid_)
         : ws(ws_ - g_A.L.nsm), sm(sm_), smd(sm_ + C::SM_TOTAL), th(nullptr), lane(tid_) {
-        for (int q = 0; q < 8; ++q) pc[q] = 0;
+        if (tid_ < 16) reinterpret_cast<unsigned long long*>(jipm_smem + C::SM_CNT)[tid_] = 0ull;
         tm.tid = tid_; tm.flip = 0; tm.red = sm_ + C::SM_RED;
     }
 

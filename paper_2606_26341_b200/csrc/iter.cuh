@@ -43,12 +43,10 @@ struct Solver {
     unsigned n_fact, n_solve, n_deriv, n_fc, n_iter, n_resto;
     // SM-clock cycles this team spent in: 0 derivatives, 1 factorisations, 2 KKT solves, 3 residuals of (6),
     // 4 trial-point evaluations, 5 whole iterations, 6 Step I, 7 (spare)
-    unsigned long long tph[8];
     double* bl; double* bu;
 
     __device__ Solver(X& c_) : c(c_), lane(c_.lane) {
         n_fact = n_solve = n_deriv = n_fc = n_iter = n_resto = 0;
-        for (int q = 0; q < 8; ++q) tph[q] = 0;
         // the shared bounds, copied next to the iterate once per kernel
         bl = c.vh(L->bl); bu = c.vh(L->bu);
         for (int q = lane; q < pb->n; q += NT) { bl[q] = pb->xL[q]; bu[q] = pb->xU[q]; }
@@ -244,7 +242,7 @@ struct Solver {
         }
         const long long t0 = clock64();
         K::solve(c, rr.a, rc, d1.a, d2, mode != 0 || dc_cur != 0.0);
-        tph[2] += clock64() - t0;
+        c.tick(2, clock64() - t0);
         n_solve++;
         if (mode) {
             for (int j = lane; j < m; j += NT) {
@@ -311,7 +309,7 @@ struct Solver {
             double dn;
             const long long t0 = clock64();
             const double rn = full_residual(b1, b2, b3, b4, d1, d2, d3, d4, dn);
-            tph[3] += clock64() - t0;
+            c.tick(3, clock64() - t0);
             const double den = bn + dn;
             return den > 0.0 ? rn / den : rn;
         };

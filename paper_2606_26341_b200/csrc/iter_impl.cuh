@@ -101,7 +101,7 @@ __device__ double Solver<C>::eval_point(const Vec xt, double* ct, double& th_t, 
     bool fin;
     const long long t0 = clock64();
     fb = c.eval_fc(xt.a, ct, thb, cmb, fin);
-    tph[4] += clock64() - t0;
+    c.tick(4, clock64() - t0);
     n_fc++;
     if (!mode) { th_t = thb; cm_t = cmb; fpn = 0.0; fq = 0.0; return fb; }
     const int n = pb->n, m = pb->m;
@@ -335,7 +335,7 @@ __device__ bool Solver<C>::ic_loop(bool resume, double& dw, double& dc, int& nfa
         if (dw > o->delta_w_max) give_up = true;                                          // IC-6
     }
     nfact += nf; n_fact += nf;
-    tph[1] += clock64() - t_f;
+    c.tick(1, clock64() - t_f);
     return ok;
 }
 
@@ -433,7 +433,7 @@ __device__ bool Solver<C>::backtrack(const Vec dxv, double theta_k, double phi_k
                 }
                 c.tm.sync();
             }
-            tph[7] += clock64() - t_sp;
+            c.tick(7, clock64() - t_sp);
             if (exhausted) break;
         }
     }
@@ -548,7 +548,7 @@ __device__ void Solver<C>::iterate() {
     const long long t_it = clock64();
     c.eval_derivs(x, y, mode ? 0.0 : 1.0);
     const long long t_hd = clock64();
-    tph[0] += t_hd - t_it;
+    c.tick(0, t_hd - t_it);
     n_deriv++;
     if (mode) {
         const double* xR = V(L->xR); const double* DR2 = V(L->DR2);
@@ -634,13 +634,13 @@ __device__ void Solver<C>::iterate() {
     int nfact = 0, npsing = 0, nref = 0;
     double dw = 0.0, dc = 0.0;
     bool resume = false;
-    c.pc[7] += clock64() - t_hd;
+    c.tick(15, clock64() - t_hd);
     while (true) {
         if (!ic_loop(resume, dw, dc, nfact)) { enter_restoration(rec, KIND_IC_FAIL); trace_put(rec); return; }
         bool failed;
         const long long t_sf = clock64();
         nref = solve_full(b1, b2, b3, b4, dx, dy, dzL, dzU, failed);
-        c.pc[5] += clock64() - t_sf;
+        c.tick(13, clock64() - t_sf);
         if (!failed) break;
         npsing++;
         resume = true;
@@ -732,7 +732,7 @@ __device__ void Solver<C>::iterate() {
             const double a_z = ftb_dual(zL, zU, dzL, dzU, tau);
             accept_step(0, dx, dy, dzL, dzU, a_max, a_max, a_z, t);
             rec[5] = KIND_NEWTON; rec[8] = a_max; rec[9] = a_z; rec[10] = ftype ? 1.0 : 0.0;
-            c.pc[6] += clock64() - t_ls;
+            c.tick(14, clock64() - t_ls);
             trace_put(rec);
             if (mode) try_exit_restoration();
             return;
@@ -777,7 +777,7 @@ __device__ void Solver<C>::iterate() {
     } else {
         ok = backtrack(dx, theta_k, phi_k, gd, a_max, false, true, rec, acc, alpha, alpha_acc, ta);
     }
-    c.pc[6] += clock64() - t_ls;
+    c.tick(14, clock64() - t_ls);
     if (!ok) {
         // the line search failed: first the soft restoration phase (row 5), then the hard one (row 6)
         if (o->soft_resto_factor > 0.0) {

@@ -6,7 +6,6 @@
 #include <vector>
 #include <algorithm>
 #include <mutex>
-#include <cstdlib>
 #include "launch.cuh"
 
 using namespace jipm;
@@ -210,17 +209,6 @@ extern "C" int jipm_create(jipm_solver** out, int family, const jipm_family_dims
     if (family == JIPM_FAM_POINTMASS2D) s->inst = inst_pm();
     else if (family == JIPM_FAM_MULTIQUAD) s->inst = d->n_agents == 4 ? inst_q4() : inst_q2();
     else s->inst = inst_q1();
-    bool forced_inst = false;
-    if (const char* ev = getenv("JIPM_EXPERIMENT_INST")) {   // development switch (measurements of DESIGN.md section 6)
-        if (family == JIPM_FAM_QUAD_TRACK || family == JIPM_FAM_QUAD_CLUTTER) {
-            if (!strcmp(ev, "q1b")) { s->inst = inst_q1b(); forced_inst = true; }
-            if (!strcmp(ev, "q1c")) { s->inst = inst_q1c(); forced_inst = true; }
-            if (!strcmp(ev, "q1g")) { s->inst = inst_q1g(); forced_inst = true; }
-            if (!strcmp(ev, "q1d")) { s->inst = inst_q1d(); forced_inst = true; }
-            if (!strcmp(ev, "q1e")) { s->inst = inst_q1e(); forced_inst = true; }
-            if (!strcmp(ev, "q1h")) { s->inst = inst_q1h(); forced_inst = true; }
-        }
-    }
     cudaDeviceProp prop;
     if (cudaGetDevice(&s->device) != cudaSuccess || cudaGetDeviceProperties(&prop, s->device) != cudaSuccess) {
         delete s;
@@ -234,7 +222,6 @@ extern "C" int jipm_create(jipm_solver** out, int family, const jipm_family_dims
     const long budget = per_team / (long)sizeof(double) - s->inst.info.sm_fixed;
     if (budget < 0) { delete s; return fail(JIPM_ERR_NOMEM, "stage tiles do not fit shared memory"); }
     int hot_fits = build_layout(s, (int)budget);
-    (void)forced_inst;
     if (!hot_fits && s->inst.info.hot_sm) {
         // the hot group does not fit: the general instantiation of the family (generic loads, arrays wherever they fit)
         if (family == JIPM_FAM_POINTMASS2D) { delete s; return fail(JIPM_ERR_NOMEM, "problem too large for the point-mass kernel"); }

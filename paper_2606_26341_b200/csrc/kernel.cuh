@@ -153,9 +153,9 @@ __global__ void __launch_bounds__(C::NT, MINB) jipm_slot_kernel() {
                 S.dbg_store(A->dbg_state + (int64_t)id * A->dbg_len);
             } else {
                 const long long t1 = clock64();
-                S.tph[6] += t1 - t0i;
+                ctx.tick(6, t1 - t0i);
                 while (S.status == JIPM_ST_NOT_RUN) S.iterate();
-                S.tph[5] += clock64() - t1;
+                ctx.tick(5, clock64() - t1);
                 S.write_outputs();
             }
         }
@@ -168,8 +168,7 @@ __global__ void __launch_bounds__(C::NT, MINB) jipm_slot_kernel() {
         atomicAdd(&A->stats[3], (unsigned long long)S.n_deriv);
         atomicAdd(&A->stats[4], (unsigned long long)S.n_fc);
         atomicAdd(&A->stats[7], (unsigned long long)S.n_resto);
-        for (int i = 0; i < 8; ++i) atomicAdd(&A->stats[8 + i], S.tph[i]);
-        for (int i = 0; i < 8; ++i) atomicAdd(&A->stats[16 + i], ctx.pc[i]);
+        for (int i = 0; i < 16; ++i) atomicAdd(&A->stats[8 + i], ctx.counter(i));
     }
     // release the workspace: all global-scratch accesses of this CTA are done
     __syncthreads();

@@ -249,7 +249,7 @@ struct Kkt {
                 sTJ[e] = dotc<AX, 1, LDJ>(sT + l * NX + AX * aj, sJ + AX * aj * LDJ + j);
             });
             c.tm.sync();
-            { const long long t2 = clock64(); c.pc[0] += t2 - tq; tq = t2; }
+            { const long long t2 = clock64(); c.tick(8, t2 - tq); tq = t2; }
             // M = Q_k + J^T (T J) + condensed slacks
             const double* Wg = c.Wk(k);
             tile_for<NZ * NZ>(lane, [&](int e) {
@@ -263,11 +263,11 @@ struct Kkt {
                 tA[e] = m;
             });
             c.tm.sync();
-            { const long long t2 = clock64(); c.pc[1] += t2 - tq; tq = t2; }
+            { const long long t2 = clock64(); c.tick(9, t2 - tq); tq = t2; }
             // Gauss-Jordan pivots on the controls NX .. NZ-1, four per barrier: every element from the previous tile
             double* src = tA; double* dst = tB;
             gj_range<NZ, NZ * NZ, NU>(c, src, dst, NX, bad, nzero);
-            { const long long t2 = clock64(); c.pc[2] += t2 - tq; tq = t2; }
+            { const long long t2 = clock64(); c.tick(10, t2 - tq); tq = t2; }
             // src: [[P_k, -Kf^T], [Kf, G]].  Phi = A - B Kf; stores
             double* Kg = c.vh(c.L->Kf) + k * NU * NX;
             double* Gg = c.vh(c.L->Gf) + k * NU * NU;
@@ -296,7 +296,7 @@ struct Kkt {
             for (int e = lane; e < NU * NX; e += NT) Kg[e] = src[(NX + e / NX) * NZ + e % NX];
             for (int e = lane; e < NU * NU; e += NT) Gg[e] = src[(NX + e / NU) * NZ + NX + e % NU];
             c.tm.sync();
-            { const long long t2 = clock64(); c.pc[3] += t2 - tq; tq = t2; }
+            { const long long t2 = clock64(); c.tick(11, t2 - tq); tq = t2; }
             if (any_dc) {
                 // Psi = (I - D_{k+1} T_{k+1}) Phi inside the first pivot phase, then P_k -> T_k = (I + P_k D_k)^{-1} P_k
                 const int r0 = c.icd(k + 1);
@@ -306,7 +306,7 @@ struct Kkt {
                         Pg[e] = sTJ[e] - Dc[r0 + i] * dotc<NX, 1, NX>(sT + i * NX, sTJ + a);
                     });
                 });
-                c.pc[4] += clock64() - tq;
+                c.tick(12, clock64() - tq);
             }
         }
         return bad;

@@ -19,11 +19,6 @@ struct Inst { InstInfo info; launch_fn launch; };
 Inst inst_pm();
 Inst inst_q1();
 Inst inst_q1g();
-Inst inst_q1b();
-Inst inst_q1c();
-Inst inst_q1d();
-Inst inst_q1e();
-Inst inst_q1h();
 Inst inst_q2();
 Inst inst_q4();
 cudaError_t launch_fp64_peak(double* out, int blocks, int threads, int iters, cudaStream_t st);
