@@ -37,7 +37,9 @@ UNIT = "NLPs/s"
 WORKLOAD_NAMES = {0: "C0 2-D point-mass NMPC N=10, batch 256",
                   1: "C1 single-quadrotor tracking RK4 N=20 3 obstacles, batch 4096",
                   2: "C2 4-quadrotor collision-free navigation N=20, batch 2048",
-                  3: "C3 quadrotor in clutter N=30 32 obstacles, batch 8192"}
+                  3: "C3 quadrotor in clutter N=30 32 obstacles, batch 8192",
+                  5: "N3 the paper's own vehicle (PAPER.md:174-180): 13-state quaternion quadrotor, dt 0.1, 30 knots, "
+                     "sector navigation with 3 obstacles, batch 2000"}
 
 
 # ---------------------------------------------------------------------------------------------------------
@@ -56,6 +58,12 @@ def algorithmic_flops(d: wl.Dims) -> dict:
     if d.family == wl.FAM_POINTMASS2D:
         fc = N * 12 + (N + 1) * 6 + N * ng * 8
         deriv = fc + 4 * n
+    elif d.family == wl.FAM_QUAT_NAV:
+        ode = 90   # flops of one evaluation of the polynomial quaternion dynamics
+        fc = N * (4 * ode + 13 * 10) + (N + 1) * 9 + N * ng * 10
+        # matrix-free chain: 4 RK points x (ode + adjoint product 110) and 17 columns x 4 points x (Jacobian-vector
+        # product 100 + contracted-Hessian-vector product 150 + the 17 x 17 accumulation 578)
+        deriv = N * (4 * (ode + 110) + 17 * 4 * (100 + 150 + 578)) + 6 * n
     else:
         ode = 110  # flops of one continuous-dynamics evaluation (sincos counted as 2 x 20)
         fc = N * na * (4 * ode + 12 * 10) + (N + 1) * na * 9 + N * ng * 10
@@ -152,7 +160,7 @@ TRAFFIC_SOURCE = {1: "profiles/r2_ncu_full_c1.md"}
 # factorisations in numpy), so its sample measures ITERATIONS per second and converts with the iterations per converged
 # NLP that the GPU arm measured on the same workload (the line says so).
 def oracle_sample(cfg: int, cores: int):
-    return {0: (256, 30.0), 1: (2 * cores, 25.0), 2: (cores, 20.0), 3: (cores, 20.0)}[cfg]
+    return {0: (256, 30.0), 1: (cores, 25.0), 2: (cores, 20.0), 3: (cores, 20.0), 5: (cores, 25.0)}[cfg]
 
 
 def golden_iterations_per_solved(cfg: int):
@@ -433,7 +441,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 3, 4])
+    ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 3, 4, 5])
     ap.add_argument("--queue", type=int, default=0, help="config 4: problems in the queue (default 100000 for the C1 "
                                                          "family, 20000 for the C2 family)")
     ap.add_argument("--c4-family", type=int, default=1, choices=[1, 2], help="config 4: which reading of 'the config-2 "

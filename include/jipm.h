@@ -33,7 +33,8 @@ extern "C" {
 typedef struct jipm_solver jipm_solver; /* opaque, owned by the library */
 
 enum { JIPM_OK = 0, JIPM_ERR_ARG = 1, JIPM_ERR_DIM = 2, JIPM_ERR_BOUNDS = 3, JIPM_ERR_CUDA = 4, JIPM_ERR_NOMEM = 5 };
-enum { JIPM_FAM_POINTMASS2D = 0, JIPM_FAM_QUAD_TRACK = 1, JIPM_FAM_MULTIQUAD = 2, JIPM_FAM_QUAD_CLUTTER = 3 };
+enum { JIPM_FAM_POINTMASS2D = 0, JIPM_FAM_QUAD_TRACK = 1, JIPM_FAM_MULTIQUAD = 2, JIPM_FAM_QUAD_CLUTTER = 3,
+       JIPM_FAM_QUAT_NAV = 4 /* the paper's own vehicle: 13-state quaternion quadrotor, rotor speeds */ };
 enum { JIPM_ST_NOT_RUN = -1, JIPM_ST_SOLVED = 0, JIPM_ST_MAXITER = 1, JIPM_ST_LOCALLY_INFEASIBLE = 2,
        JIPM_ST_RESTORATION_FAILED = 3, JIPM_ST_RESTO_AT_FEASIBLE_POINT = 4, JIPM_ST_NONFINITE = 5,
        JIPM_ST_TINY_STEP = 6 /* search direction too small to make progress at the smallest mu (Table I row 4) */ };
@@ -61,7 +62,8 @@ typedef struct {
     int32_t max_iter, max_backtrack, max_soc, refine_min, refine_max, max_mu_updates;
     int32_t init_slacks, enable_restoration;
     int32_t watchdog_trigger, watchdog_trial_max, max_soft_resto_iters;
-    int32_t reserved_;
+    int32_t polish_max; /* extra refinement steps (<= this many) taken after the stop rule is met while the residual ratio
+                           is above 1e-15 and still shrinking: accuracy of the step only, no decision depends on it */
 } jipm_options;
 
 /* Fill *o with the defaults.  o: HOST.  Returns JIPM_ERR_ARG if o is NULL. */

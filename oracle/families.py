@@ -12,6 +12,8 @@ Decision vector, stage order (same layout the C ABI documents in include/jipm.h)
     x = [ x_0 | u_0 x_1 s_1 | ... | u_{N-1} x_N s_N ],   c = [ x_0 - xhat0 | dyn_1 g_1 | ... | dyn_N g_N ]
     dyn_k = x_k - F(x_{k-1},u_{k-1}),   g_k = h(x_k) - s_k  (h >= 0 are the obstacle / separation inequalities)
 Quadrotor model: SURVEY.md Appendix C (12 states: p, ZYX Euler (phi,theta,psi), world velocity v, body rates w).
+Family 4 is the paper's own vehicle: 13 states (p, quaternion q, BODY velocity v, body rates w), four
+rotor speeds as inputs; the paper gives no parameters, the ones used are DESIGN.md reading N3.
 """
 from __future__ import annotations
 
@@ -19,7 +21,7 @@ import numpy as np
 
 from .jets import Jet
 
-FAM_POINTMASS2D, FAM_QUAD_TRACK, FAM_MULTIQUAD, FAM_QUAD_CLUTTER = 0, 1, 2, 3
+FAM_POINTMASS2D, FAM_QUAD_TRACK, FAM_MULTIQUAD, FAM_QUAD_CLUTTER, FAM_QUAT_NAV = 0, 1, 2, 3, 4
 
 G_ACC = 9.81
 MASS = 1.0
@@ -63,13 +65,48 @@ def quad_ode(x, u):
     return [vx, vy, vz, dph, dth, dps, dvx, dvy, dvz, dwp, dwq, dwr]
 
 
-def quad_rk4(x, u, h):
+KF_ROTOR = 1.0      # thrust of rotor i = KF_ROTOR * u_i^2 (rotor speeds in units that make this 1)
+KM_ROTOR = 0.02     # drag torque of rotor i = KM_ROTOR * u_i^2
+
+
+def quat_ode(x, u):
+    """13-state rigid body: p world position, q = (w, x, y, z) attitude (body -> world), v BODY linear
+    velocity, w body angular velocity; u = four rotor speeds.
+        pdot = R(q) v;  qdot = 1/2 q (x) (0, w);  vdot = -w x v + R(q)^T (0,0,-g) + (0,0,T/m);  wdot = J^-1 (tau - w x J w)."""
+    qw, qx, qy, qz = x[3], x[4], x[5], x[6]
+    vx, vy, vz = x[7], x[8], x[9]
+    wx, wy, wz = x[10], x[11], x[12]
+    # rotation matrix of the (unnormalised) quaternion, row by row
+    r00, r01, r02 = 1.0 - 2.0 * (qy * qy + qz * qz), 2.0 * (qx * qy - qw * qz), 2.0 * (qx * qz + qw * qy)
+    r10, r11, r12 = 2.0 * (qx * qy + qw * qz), 1.0 - 2.0 * (qx * qx + qz * qz), 2.0 * (qy * qz - qw * qx)
+    r20, r21, r22 = 2.0 * (qx * qz - qw * qy), 2.0 * (qy * qz + qw * qx), 1.0 - 2.0 * (qx * qx + qy * qy)
+    dp = [r00 * vx + r01 * vy + r02 * vz, r10 * vx + r11 * vy + r12 * vz, r20 * vx + r21 * vy + r22 * vz]
+    dq = [(qx * wx + qy * wy + qz * wz) * (-0.5), (qw * wx + qy * wz - qz * wy) * 0.5,
+          (qw * wy + qz * wx - qx * wz) * 0.5, (qw * wz + qx * wy - qy * wx) * 0.5]
+    f = [KF_ROTOR * (ui * ui) for ui in u]
+    T = f[0] + f[1] + f[2] + f[3]
+    # gravity seen from the body: R^T (0, 0, -g) = -g * (third ROW of R)
+    dv = [-(wy * vz - wz * vy) - G_ACC * r20, -(wz * vx - wx * vz) - G_ACC * r21,
+          -(wx * vy - wy * vx) - G_ACC * r22 + T * (1.0 / MASS)]
+    tx = ARM * (f[1] - f[3])
+    ty = ARM * (f[2] - f[0])
+    tz = (KM_ROTOR / KF_ROTOR) * (f[0] - f[1] + f[2] - f[3])
+    dw = [(tx - (JZ - JY) * wy * wz) * (1.0 / JX), (ty - (JX - JZ) * wz * wx) * (1.0 / JY),
+          (tz - (JY - JX) * wx * wy) * (1.0 / JZ)]
+    return dp + dq + dv + dw
+
+
+def rk4(ode, x, u, h):
     """One classical RK4 step with zero-order-hold input."""
-    k1 = quad_ode(x, u)
-    k2 = quad_ode([xi + (0.5 * h) * ki for xi, ki in zip(x, k1)], u)
-    k3 = quad_ode([xi + (0.5 * h) * ki for xi, ki in zip(x, k2)], u)
-    k4 = quad_ode([xi + h * ki for xi, ki in zip(x, k3)], u)
+    k1 = ode(x, u)
+    k2 = ode([xi + (0.5 * h) * ki for xi, ki in zip(x, k1)], u)
+    k3 = ode([xi + (0.5 * h) * ki for xi, ki in zip(x, k2)], u)
+    k4 = ode([xi + h * ki for xi, ki in zip(x, k3)], u)
     return [xi + (h / 6.0) * (a + 2.0 * b + 2.0 * c + d) for xi, a, b, c, d in zip(x, k1, k2, k3, k4)]
+
+
+def quad_rk4(x, u, h):
+    return rk4(quad_ode, x, u, h)
 
 
 class Problem:
@@ -77,10 +114,12 @@ class Problem:
 
     def __init__(self, family: int, horizon_N: int, n_agents: int, n_obstacles: int, dt: float):
         self.family, self.N, self.na, self.nobs, self.dt = family, horizon_N, n_agents, n_obstacles, dt
+        self.ax, self.au = (4, 2) if family == FAM_POINTMASS2D else ((13, 4) if family == FAM_QUAT_NAV else (12, 4))
+        self.ode = quat_ode if family == FAM_QUAT_NAV else quad_ode
         if family == FAM_POINTMASS2D:
             self.nx, self.nu, self.pdim, self.ru = 4, 2, 2, 0.1
         else:
-            self.nx, self.nu, self.pdim, self.ru = 12 * n_agents, 4 * n_agents, 3, 0.01
+            self.nx, self.nu, self.pdim, self.ru = self.ax * n_agents, self.au * n_agents, 3, 0.01
         self.ng = n_agents * (n_agents - 1) // 2 if family == FAM_MULTIQUAD else n_obstacles
         N = self.N
         self.blk = self.nu + self.nx + self.ng
@@ -107,6 +146,8 @@ class Problem:
     def bounds(self):
         xL, xU = np.full(self.n, -np.inf), np.full(self.n, np.inf)
         lo, hi = (-1.0, 1.0) if self.family == FAM_POINTMASS2D else (0.0, MASS * G_ACC / 2.0)
+        if self.family == FAM_QUAT_NAV:   # rotor speeds: thrust per rotor KF u^2 <= m g / 2
+            hi = float(np.sqrt(MASS * G_ACC / 2.0 / KF_ROTOR))
         for k in range(self.N):
             xL[self.iu(k):self.iu(k) + self.nu] = lo
             xU[self.iu(k):self.iu(k) + self.nu] = hi
@@ -129,18 +170,20 @@ class Problem:
         if self.family == FAM_MULTIQUAD:
             o = 12 * self.na + 3 * agent
             return th[o:o + 3]
+        if self.family == FAM_QUAT_NAV:
+            return th[13:16]
         return th[12:15]
 
     def obstacle(self, th, j):
         if self.family == FAM_POINTMASS2D:
             o = 6 + 3 * j
             return th[o:o + 2], th[o + 2]
-        o = (14 if self.family == FAM_QUAD_TRACK else 15) + 4 * j
+        o = {FAM_QUAD_TRACK: 14, FAM_QUAD_CLUTTER: 15, FAM_QUAT_NAV: 16}[self.family] + 4 * j
         return th[o:o + 3], th[o + 3]
 
     def pos_index(self, k, agent=0):
         """Index in x of the position of one agent at knot k."""
-        return self.ix(k) + (12 * agent if self.family != FAM_POINTMASS2D else 0)
+        return self.ix(k) + (self.ax * agent if self.family != FAM_POINTMASS2D else 0)
 
     # ---- objective (quadratic) -----------------------------------------------------------------
     def f(self, x, th):
@@ -202,20 +245,21 @@ class Problem:
         F = np.zeros((N, nx))
         Jac = np.zeros((N, nx, nx + nu))
         Hes = np.zeros((N, nx, nx + nu, nx + nu))
+        ax, au = self.ax, self.au
         for a in range(self.na):
-            cols = list(range(12 * a, 12 * a + 12)) + list(range(nx + 4 * a, nx + 4 * a + 4))
+            cols = list(range(ax * a, ax * a + ax)) + list(range(nx + au * a, nx + au * a + au))
             za = Z[:, cols]
             if order == 0:
-                out = quad_rk4([za[:, i] for i in range(12)], [za[:, 12 + i] for i in range(4)], h)
-                F[:, 12 * a:12 * a + 12] = np.stack(out, axis=1)
+                out = rk4(self.ode, [za[:, i] for i in range(ax)], [za[:, ax + i] for i in range(au)], h)
+                F[:, ax * a:ax * a + ax] = np.stack(out, axis=1)
                 continue
             v = Jet.variables(za)
-            out = quad_rk4(v[:12], v[12:], h)
+            out = rk4(self.ode, v[:ax], v[ax:], h)
             for i, o in enumerate(out):
-                F[:, 12 * a + i] = o.v
-                Jac[:, 12 * a + i, cols] = o.g
+                F[:, ax * a + i] = o.v
+                Jac[:, ax * a + i, cols] = o.g
                 if order == 2:
-                    Hes[np.ix_(range(N), [12 * a + i], cols, cols)] = o.H[:, None, :, :]
+                    Hes[np.ix_(range(N), [ax * a + i], cols, cols)] = o.H[:, None, :, :]
         if order == 0:
             return F
         return (F, Jac) if order == 1 else (F, Jac, Hes)

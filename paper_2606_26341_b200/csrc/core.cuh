@@ -29,7 +29,7 @@ struct Cfg {
     // the staging of the Hessian columns aliases the factorisation tiles M, M2, TJ, K (derivative evaluation and
     // factorisation are never live at the same time)
     static constexpr int SM_G = SM_M;
-    static constexpr int SM_G_END = SM_G + (Dyn::AX == 12 ? NGRP * 7 * 16 : 0);
+    static constexpr int SM_G_END = SM_G + (Dyn::AX == 12 ? NGRP * 7 * 16 : (Dyn::AX == 13 ? (NT / 32) * 17 * 17 : 0));
     static constexpr int SM_RED = (SM_TILE_END > SM_G_END) ? SM_TILE_END : SM_G_END;
     static constexpr int SM_SPEC = SM_RED + 2 * (NT / 32) + 2;  // (theta, phi) of the speculative trials, one pair per warp
     static constexpr int SM_CNT = SM_SPEC + 2 * (NT / 32);  // 16 diagnostic cycle counters (64-bit), written by thread 0
@@ -273,13 +273,16 @@ struct Ctx {
         if (k < pb->N) {
             const double* Wc = Wk(k) + a; const double* dxk = d + ix(k); const double* duk = d + iu(k);
 #pragma unroll 4
-            for (int b = 0; b < NX; b += 2) { s0 += Wc[b * NZ] * dxk[b]; s1 += Wc[(b + 1) * NZ] * dxk[b + 1]; }
+            for (int b = 0; b + 1 < NX; b += 2) { s0 += Wc[b * NZ] * dxk[b]; s1 += Wc[(b + 1) * NZ] * dxk[b + 1]; }
+            if constexpr (NX & 1) s0 += Wc[(NX - 1) * NZ] * dxk[NX - 1];
 #pragma unroll 4
-            for (int b = 0; b < NU; b += 2) { s0 += Wc[(NX + b) * NZ] * duk[b]; s1 += Wc[(NX + b + 1) * NZ] * duk[b + 1]; }
+            for (int b = 0; b + 1 < NU; b += 2) { s0 += Wc[(NX + b) * NZ] * duk[b]; s1 += Wc[(NX + b + 1) * NZ] * duk[b + 1]; }
+            if constexpr (NU & 1) s0 += Wc[(NX + NU - 1) * NZ] * duk[NU - 1];
         } else {
             const double* Wc = Wk(k) + a; const double* dxk = d + ix(k);
 #pragma unroll 4
-            for (int b = 0; b < NX; b += 2) { s0 += Wc[b * NX] * dxk[b]; s1 += Wc[(b + 1) * NX] * dxk[b + 1]; }
+            for (int b = 0; b + 1 < NX; b += 2) { s0 += Wc[b * NX] * dxk[b]; s1 += Wc[(b + 1) * NX] * dxk[b + 1]; }
+            if constexpr (NX & 1) s0 += Wc[(NX - 1) * NX] * dxk[NX - 1];
         }
         return s0 + s1;
     }

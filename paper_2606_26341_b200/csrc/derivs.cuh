@@ -24,6 +24,112 @@ __device__ void Ctx<C>::dyn_derivs(const double* x, const double* y) {
         }
         for (int it = lane; it < N * NZ * NZ + NX * NX; it += NT) vh(L->W)[it] = 0.0;
         tm.sync();
+    } else if constexpr (std::is_same<typename C::Dyn, QuatDyn>::value) {
+        // 13-state quaternion vehicle: the same RK4 chain as below, matrix-free: the products with Df and with the
+        // adjoint-contracted Hessian at each RK point come from the generated functions of dyn_quat_gen.cuh.
+        //   xi_1 = x, xi_{s+1} = x + a_{s+1} h f(xi_s);   mu_4 = b_4 lam, mu_{s-1} = b_{s-1} lam + a_s h Df_x(xi_s)^T mu_s
+        //   column j of the chain: Y_1 = e_j, K_s = Df(xi_s) (Y_s, e_u), Y_{s+1} = e_j + a_{s+1} h K_s, J e_j = e_j + h sum b_s K_s
+        //   lam^T Hess F = sum_s (Y_s, e_u)^T [sum_i mu_s,i Hess f_i(xi_s)] (Y_s, e_u)
+        const double h = pb->dt;
+        double* rk = v(L->rk);
+        // ---- phase 1: thread <-> stage: the RK points and their adjoint weights ----
+        for (int k = lane; k < N; k += NT) {
+            double xa[13], ua[4], lam[13], kk[13], xi[13];
+#pragma unroll
+            for (int i = 0; i < 13; ++i) { xa[i] = x[ix(k) + i]; lam[i] = -y[icd(k + 1) + i]; }
+#pragma unroll
+            for (int i = 0; i < 4; ++i) ua[i] = x[iu(k) + i];
+            double* out = rk + (k * 4) * RKW;
+#pragma unroll
+            for (int i = 0; i < 13; ++i) { xi[i] = xa[i]; out[i] = xi[i]; }
+#pragma unroll 1
+            for (int s = 1; s < 4; ++s) {
+                quat_ode(xi, ua, kk);
+                const double as = (s == 3) ? h : 0.5 * h;
+#pragma unroll
+                for (int i = 0; i < 13; ++i) { xi[i] = xa[i] + as * kk[i]; out[s * RKW + i] = xi[i]; }
+            }
+            double mu[13], t[13];
+#pragma unroll
+            for (int i = 0; i < 13; ++i) mu[i] = (h / 6.0) * lam[i];
+#pragma unroll 1
+            for (int s = 3; s >= 0; --s) {
+#pragma unroll
+                for (int i = 0; i < 13; ++i) out[s * RKW + 13 + i] = mu[i];
+                if (s > 0) {
+#pragma unroll
+                    for (int i = 0; i < 13; ++i) xi[i] = out[s * RKW + i];
+                    quat_vjp(xi, ua, mu, t);
+                    const double as = (s == 3) ? h : 0.5 * h;
+                    const double bprev = (s == 1) ? h / 6.0 : h / 3.0;
+#pragma unroll
+                    for (int i = 0; i < 13; ++i) mu[i] = bprev * lam[i] + as * t[i];
+                }
+            }
+        }
+        tm.sync();
+        // ---- phase 2: warp <-> stage, lane j < 17 <-> column j of z = (x(13), u(4)) ----
+        constexpr int NWP = NT / 32;
+        const int wid = lane >> 5, j = lane & 31;
+        const bool act = j < 17;
+        double* sV = smt(C::SM_G) + wid * (17 * 17);
+        for (int k0 = 0; k0 < N; k0 += NWP) {
+            const int k = k0 + wid;
+            const bool valid = k < N;
+            const int kc = valid ? k : N - 1;
+            double Y[13], Jc[13], Hc[17], uj[4], ua[4];
+#pragma unroll
+            for (int i = 0; i < 13; ++i) { Y[i] = (i == j) ? 1.0 : 0.0; Jc[i] = Y[i]; }
+#pragma unroll
+            for (int i = 0; i < 4; ++i) { uj[i] = (j == 13 + i) ? 1.0 : 0.0; ua[i] = x[iu(kc) + i]; }
+#pragma unroll
+            for (int i = 0; i < 17; ++i) Hc[i] = 0.0;
+#pragma unroll 1
+            for (int s = 0; s < 4; ++s) {
+                const double* in = rk + (kc * 4 + s) * RKW;
+                double xi[13], mu[13], K[13], V[17], t[17];
+#pragma unroll
+                for (int i = 0; i < 13; ++i) { xi[i] = in[i]; mu[i] = in[13 + i]; K[i] = 0.0; }
+#pragma unroll
+                for (int i = 0; i < 13; ++i) V[i] = Y[i];
+#pragma unroll
+                for (int i = 0; i < 4; ++i) V[13 + i] = uj[i];
+                if (act) {
+#pragma unroll
+                    for (int e = 0; e < 17; ++e) sV[e * 17 + j] = V[e];
+                    quat_hvp(xi, ua, mu, V, t);
+                    quat_jvp(xi, ua, Y, uj, K);
+                }
+                __syncwarp();
+                if (act) {
+#pragma unroll
+                    for (int c2 = 0; c2 < 17; ++c2) {
+                        double acc = Hc[c2];
+#pragma unroll
+                        for (int e = 0; e < 17; ++e) acc += sV[e * 17 + c2] * t[e];
+                        Hc[c2] = acc;
+                    }
+                }
+                __syncwarp();
+                const double bw = (s == 0 || s == 3) ? h / 6.0 : h / 3.0;
+                const double an = (s == 2) ? h : 0.5 * h;
+#pragma unroll
+                for (int i = 0; i < 13; ++i) {
+                    Jc[i] += bw * K[i];
+                    Y[i] = ((i == j) ? 1.0 : 0.0) + an * K[i];
+                }
+            }
+            if (valid && act) {
+                double* Jb = Jk(k);
+#pragma unroll
+                for (int i = 0; i < 13; ++i) Jb[i * LDJ + j] = Jc[i];
+                double* Wb = Wk(k);
+#pragma unroll
+                for (int c2 = 0; c2 < 17; ++c2) Wb[c2 * NZ + j] = Hc[c2];
+            }
+        }
+        for (int it = lane; it < NX * NX; it += NT) Wk(N)[it] = 0.0;
+        tm.sync();
     } else {
         const double h = pb->dt;
         double* rk = v(L->rk);

@@ -13,6 +13,7 @@
 // (half-warp <-> stage, lane <-> column of z=(x,u)) propagates the 16 columns.
 #pragma once
 #include "common.cuh"
+#include "dyn_quat_gen.cuh"
 
 namespace jipm {
 
@@ -27,6 +28,29 @@ struct PointmassDyn {
         out[1] = x[1] + h * x[3] + 0.5 * h * h * u[1];
         out[2] = x[2] + h * u[0];
         out[3] = x[3] + h * u[1];
+    }
+};
+
+// The paper's own vehicle: 13 states (p, quaternion, body velocity, body rates), four rotor speeds.
+// ode / Jacobian-vector / transposed-Jacobian-vector / contracted-Hessian-vector products are generated from the model
+// equations by gen_quat_dyn.py (dyn_quat_gen.cuh); derivs.cuh chains them through the four RK4 points.
+struct QuatDyn {
+    static constexpr int AX = 13, AU = 4, PD = 3, AZ = 17;
+    static constexpr int RK_SCRATCH = 4 * RKW;
+    __device__ static void F(const double* x, const double* u, double h, double* out) {
+        double k1[13], k2[13], k3[13], k4[13], xi[13];
+        quat_ode(x, u, k1);
+#pragma unroll
+        for (int i = 0; i < 13; ++i) xi[i] = x[i] + (0.5 * h) * k1[i];
+        quat_ode(xi, u, k2);
+#pragma unroll
+        for (int i = 0; i < 13; ++i) xi[i] = x[i] + (0.5 * h) * k2[i];
+        quat_ode(xi, u, k3);
+#pragma unroll
+        for (int i = 0; i < 13; ++i) xi[i] = x[i] + h * k3[i];
+        quat_ode(xi, u, k4);
+#pragma unroll
+        for (int i = 0; i < 13; ++i) out[i] = x[i] + (h / 6.0) * (k1[i] + 2.0 * k2[i] + 2.0 * k3[i] + k4[i]);
     }
 };
 

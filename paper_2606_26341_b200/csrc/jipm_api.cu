@@ -78,7 +78,7 @@ extern "C" int jipm_default_options(jipm_options* o) {
     o->residual_ratio_singular = 1e-5; o->residual_improvement_factor = 0.999999999;
     o->tiny_step_tol = 10.0 * 2.220446049250313e-16; o->tiny_step_y_tol = 1e-2; o->tiny_step_cviol = 1e-4;
     o->soft_resto_factor = 1.0 - 1e-4;
-    o->watchdog_trigger = 10; o->watchdog_trial_max = 3; o->max_soft_resto_iters = 10; o->reserved_ = 0;
+    o->watchdog_trigger = 10; o->watchdog_trial_max = 3; o->max_soft_resto_iters = 10; o->polish_max = 3;
     return JIPM_OK;
 }
 
@@ -97,6 +97,9 @@ static bool family_shape(int family, const jipm_family_dims* d, int& nx, int& nu
         case JIPM_FAM_QUAD_CLUTTER:
             if (na != 1 || nobs < 0) return false;
             nx = 12; nu = 4; ng = nobs; nth = 12 + 3 + 4 * nobs; pd = 3; return true;
+        case JIPM_FAM_QUAT_NAV:
+            if (na != 1 || nobs < 0) return false;
+            nx = 13; nu = 4; ng = nobs; nth = 13 + 3 + 4 * nobs; pd = 3; return true;
         case JIPM_FAM_MULTIQUAD:
             if (na != 2 && na != 4) return false;
             nx = 12 * na; nu = 4 * na; ng = na * (na - 1) / 2; nth = 12 * na + 3 * na; pd = 3; return true;
@@ -192,8 +195,8 @@ extern "C" int jipm_create(jipm_solver** out, int family, const jipm_family_dims
     pb.family = family; pb.N = d->horizon_N; pb.ng = ng; pb.na = d->n_agents; pb.nobs = d->n_obstacles;
     pb.n = (int)n; pb.m = (int)m; pb.nth = nth; pb.blk = nu + nx + ng; pb.cblk = nx + ng;
     pb.dt = d->dt; pb.ru = (family == JIPM_FAM_POINTMASS2D) ? 0.1 : 0.01;
-    pb.th_obs = (family == JIPM_FAM_POINTMASS2D) ? 6 : (family == JIPM_FAM_QUAD_TRACK ? 14 : 15);
-    pb.th_goal = (family == JIPM_FAM_POINTMASS2D) ? 4 : (family == JIPM_FAM_MULTIQUAD ? 12 * d->n_agents : 12);
+    pb.th_obs = (family == JIPM_FAM_POINTMASS2D) ? 6 : (family == JIPM_FAM_QUAD_TRACK ? 14 : (family == JIPM_FAM_QUAT_NAV ? 16 : 15));
+    pb.th_goal = (family == JIPM_FAM_POINTMASS2D) ? 4 : (family == JIPM_FAM_MULTIQUAD ? 12 * d->n_agents : (family == JIPM_FAM_QUAT_NAV ? 13 : 12));
     // Step I-1: relax finite bounds; PAPER.md:63 needs x_L < x_U
     std::vector<double> xl(n), xu(n);
     pb.nL = pb.nU = 0;
@@ -208,6 +211,7 @@ extern "C" int jipm_create(jipm_solver** out, int family, const jipm_family_dims
     }
     if (family == JIPM_FAM_POINTMASS2D) s->inst = inst_pm();
     else if (family == JIPM_FAM_MULTIQUAD) s->inst = d->n_agents == 4 ? inst_q4() : inst_q2();
+    else if (family == JIPM_FAM_QUAT_NAV) s->inst = inst_qt();
     else s->inst = inst_q1();
     cudaDeviceProp prop;
     if (cudaGetDevice(&s->device) != cudaSuccess || cudaGetDeviceProperties(&prop, s->device) != cudaSuccess) {

@@ -21,6 +21,7 @@ Inst inst_q1();
 Inst inst_q1g();
 Inst inst_q2();
 Inst inst_q4();
+Inst inst_qt();
 cudaError_t launch_fp64_peak(double* out, int blocks, int threads, int iters, cudaStream_t st);
 
 }  // namespace jipm

@@ -33,7 +33,7 @@ _INT_FIELDS = ["max_iter", "max_backtrack", "max_soc", "refine_min", "refine_max
 
 class Options(C.Structure):
     _fields_ = ([(f, C.c_double) for f in _DOUBLE_FIELDS] + [(f, C.c_int32) for f in _INT_FIELDS]
-                + [("reserved_", C.c_int32)])
+                + [("polish_max", C.c_int32)])
 
 
 class FamilyDims(C.Structure):

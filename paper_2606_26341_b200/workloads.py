@@ -27,6 +27,7 @@ FAM_POINTMASS2D = 0
 FAM_QUAD_TRACK = 1
 FAM_MULTIQUAD = 2
 FAM_QUAD_CLUTTER = 3
+FAM_QUAT_NAV = 4        # the paper's own vehicle: 13-state quaternion quadrotor, rotor-speed inputs
 
 GRAV = 9.81
 QUAD_MASS = 1.0
@@ -43,6 +44,8 @@ class Dims:
 
     @property
     def nx(self) -> int:
+        if self.family == FAM_QUAT_NAV:
+            return 13
         return 4 if self.family == FAM_POINTMASS2D else 12 * self.n_agents
 
     @property
@@ -73,6 +76,8 @@ class Dims:
             return 12 + 2 + 4 * self.n_obstacles
         if self.family == FAM_MULTIQUAD:
             return 12 * self.n_agents + 3 * self.n_agents
+        if self.family == FAM_QUAT_NAV:
+            return 13 + 3 + 4 * self.n_obstacles
         return 12 + 3 + 4 * self.n_obstacles
 
     # index helpers (stage order) -------------------------------------------------------------
@@ -107,6 +112,8 @@ def config_dims(cfg: int, horizon_N: int | None = None, n_obstacles: int | None 
         d = Dims(FAM_MULTIQUAD, 20, 4, 0, 0.05)
     elif cfg == 3:
         d = Dims(FAM_QUAD_CLUTTER, 30, 1, 32, 0.05)
+    elif cfg == 5:   # NEXT-3: the paper's own formulation: dt 0.1, 30 knots (29 intervals), 506 variables
+        d = Dims(FAM_QUAT_NAV, 29, 1, 3, 0.1)
     else:
         raise ValueError(cfg)
     return Dims(d.family,
@@ -116,7 +123,7 @@ def config_dims(cfg: int, horizon_N: int | None = None, n_obstacles: int | None 
                 d.dt)
 
 
-CONFIG_BATCH = {0: 256, 1: 4096, 2: 2048, 3: 8192}
+CONFIG_BATCH = {0: 256, 1: 4096, 2: 2048, 3: 8192, 5: 2000}
 
 
 # ------------------------------------------------------------------------------------------------
@@ -160,6 +167,8 @@ def bounds(d: Dims) -> tuple[np.ndarray, np.ndarray]:
     xU = np.full(d.n, np.inf)
     if d.family == FAM_POINTMASS2D:
         ulo, uhi = -1.0, 1.0
+    elif d.family == FAM_QUAT_NAV:   # rotor speeds, thrust per rotor u^2 <= m g / 2
+        ulo, uhi = 0.0, math.sqrt(QUAD_MASS * GRAV / 2.0)
     else:
         ulo, uhi = 0.0, QUAD_MASS * GRAV / 2.0
     for k in range(d.horizon_N):
@@ -193,6 +202,31 @@ def generate(cfg: int, P: int, d: Dims | None = None, first_id: int = 0, stream:
         return d, theta, x0
 
     hover = QUAD_MASS * GRAV / 4.0
+    if d.family == FAM_QUAT_NAV:
+        # Sector navigation (stands in for PAPER.md:186-205, whose generator is not given): every vehicle flies to a
+        # common goal (0, 0, 1) from a start on a 6 m arc around it, angle ~ U(-90, 90) degrees (the 180-degree sector),
+        # altitude 1 + U(-0.5, 0.5); the obstacles sit in the central 90 degrees between arc and goal: centre at
+        # distance U(2, 4) and angle U(-45, 45) degrees, altitude 1 + U(-0.5, 0.5), radius U(0.3, 0.6).  Level attitude
+        # (q = (1, 0, 0, 0)), at rest; initial guess: stay put with the hover rotor speed sqrt(m g / 4).
+        xh = np.zeros((P, 13))
+        ang = dr.u(-0.5 * math.pi, 0.5 * math.pi, 1)[:, 0]
+        xh[:, 0], xh[:, 1] = 6.0 * np.cos(ang), 6.0 * np.sin(ang)
+        xh[:, 2] = 1.0 + dr.u(-0.5, 0.5, 1)[:, 0]
+        xh[:, 3] = 1.0
+        theta[:, 0:13] = xh
+        theta[:, 13:16] = np.array([0.0, 0.0, 1.0])
+        for j in range(d.n_obstacles):
+            rad = dr.u(2.0, 4.0, 1)[:, 0]
+            a2 = dr.u(-0.25 * math.pi, 0.25 * math.pi, 1)[:, 0]
+            theta[:, 16 + 4 * j] = rad * np.cos(a2)
+            theta[:, 17 + 4 * j] = rad * np.sin(a2)
+            theta[:, 18 + 4 * j] = 1.0 + dr.u(-0.5, 0.5, 1)[:, 0]
+            theta[:, 19 + 4 * j] = dr.u(0.3, 0.6, 1)[:, 0]
+        for k in range(N + 1):
+            x0[:, d.ix(k):d.ix(k) + 13] = xh
+        for k in range(N):
+            x0[:, d.iu(k):d.iu(k) + nu] = math.sqrt(hover)
+        return d, theta, x0
     if d.family == FAM_QUAD_TRACK:
         xh = np.zeros((P, 12))
         xh[:, 0:3] = dr.u(-3, 3, 3)

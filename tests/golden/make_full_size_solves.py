@@ -1,5 +1,5 @@
-"""Writes tests/golden/full_size_c{1,2,3}.json: the ORACLE's results on the first problems of BASELINE.json configs[1..3]
-at their FULL dimensions (status, iteration count, objective, positions of every knot of x*, and the largest pitch angle
+"""Writes tests/golden/full_size_c{1,2,3,5}.json: the ORACLE's results on the first problems of BASELINE.json configs[1..3]
+(and of workload 5, the paper's own 13-state quaternion vehicle) at their FULL dimensions (status, iteration count, objective, positions of every knot of x*, and the largest pitch angle
 the iterates reached -- the 12-state Euler model of SURVEY.md Appendix C is singular at |pitch| = pi/2).  The GPU tests
 compare against these files instead of re-running the dense oracle (minutes per problem at n = 1448 / 1452).
 
@@ -23,8 +23,8 @@ import numpy as np  # noqa: E402
 from oracle import families as ofam, ipm as oipm  # noqa: E402
 from paper_2606_26341_b200 import workloads as wl  # noqa: E402
 
-COUNT = {1: 48, 2: 16, 3: 32}
-MAX_ITER = {1: 3000, 2: 600, 3: 1500}   # the oracle is cut here; a problem that reaches the cap is stored as such
+COUNT = {1: 48, 2: 16, 3: 32, 5: 48}
+MAX_ITER = {1: 3000, 2: 600, 3: 1500, 5: 3000}   # the oracle is cut here; a problem that reaches the cap is stored as such
 
 
 def solve_one(args):
@@ -41,14 +41,14 @@ def solve_one(args):
     pitch, n_resto, kinds = 0.0, 0, {}
     while st.status == oipm.ST_NOT_RUN:
         x = st.x if st.resto is None else st.resto.state.x[:d.n]
-        if d.family != wl.FAM_POINTMASS2D:
+        if d.family in (wl.FAM_QUAD_TRACK, wl.FAM_MULTIQUAD, wl.FAM_QUAD_CLUTTER):   # the Euler-angle families
             pitch = max(pitch, max(abs(x[prob.ix(k) + 12 * a + 4]) for k in range(d.horizon_N + 1) for a in range(d.n_agents)))
         tr = s.iterate(st, th)
         n_resto += int(tr.get("mode", 0) == 1)
         for key in ("wd", "soft", "tiny", "npsing"):
             if tr.get(key):
                 kinds[key] = kinds.get(key, 0) + 1
-    pos = [[float(v) for v in st.x[prob.ix(k) + 12 * a: prob.ix(k) + 12 * a + 3]]
+    pos = [[float(v) for v in st.x[prob.ix(k) + prob.ax * a: prob.ix(k) + prob.ax * a + 3]]
            for k in range(d.horizon_N + 1) for a in range(d.n_agents)]
     return dict(id=idx, status=int(st.status), iters=int(st.k), f=float(prob.f(st.x, th)), max_pitch=float(pitch),
                 resto_iters=n_resto, fallbacks=kinds, positions=pos, seconds=round(time.time() - t0, 1))

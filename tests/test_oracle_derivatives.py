@@ -9,7 +9,8 @@ from oracle.jets import Jet
 from paper_2606_26341_b200 import workloads as wl
 from helpers import fd_grad, fd_jac
 
-CASES = [(0, {}), (1, dict(horizon_N=3)), (2, dict(horizon_N=2, n_agents=2)), (3, dict(horizon_N=3, n_obstacles=4))]
+CASES = [(0, {}), (1, dict(horizon_N=3)), (2, dict(horizon_N=2, n_agents=2)), (3, dict(horizon_N=3, n_obstacles=4)),
+         (5, dict(horizon_N=3))]
 
 
 def make(cfg, kw, P=2):
@@ -125,3 +126,36 @@ def test_layout_matches_workloads(cfg, kw):
     assert np.max(np.abs(c[:p.nx])) == 0.0
     for k in range(1, p.N + 1):
         assert np.max(np.abs(c[p.ic_g(k):p.ic_g(k) + p.ng])) < 1e-12
+
+
+def test_quat_ode_against_rotation_library_and_cross_products():
+    """The 13-state vehicle of PAPER.md:174 (family 4) against an independent statement: R(q) from
+    scipy.spatial.transform.Rotation; pdot = R v_body; vdot = -w x v + R^T (0,0,-g) + (0,0,T/m) with numpy.cross;
+    wdot = J^-1 (tau - w x J w); and the quaternion kinematics through the rotation it generates:
+    R(q + eps qdot) = R(q) (I + eps [w]x) + O(eps^2) for a unit quaternion."""
+    from scipy.spatial.transform import Rotation
+    rng = np.random.default_rng(3)
+    for _ in range(10):
+        q = rng.normal(size=4)
+        q /= np.linalg.norm(q)
+        x = np.concatenate([rng.uniform(-1, 1, 3), q, rng.uniform(-2, 2, 3), rng.uniform(-3, 3, 3)])
+        u = rng.uniform(0.3, 2.0, 4)
+        got = np.array(fam.quat_ode(list(x), list(u)), dtype=float)
+        R = Rotation.from_quat([q[1], q[2], q[3], q[0]]).as_matrix()      # scipy order: (x, y, z, w)
+        v, w = x[7:10], x[10:13]
+        f = u ** 2
+        T = f.sum()
+        Jm = np.diag([0.01, 0.01, 0.02])
+        tau = np.array([0.2 * (f[1] - f[3]), 0.2 * (f[2] - f[0]), 0.02 * (f[0] - f[1] + f[2] - f[3])])
+        np.testing.assert_allclose(got[0:3], R @ v, rtol=1e-12, atol=1e-12)
+        np.testing.assert_allclose(got[7:10], -np.cross(w, v) + R.T @ np.array([0, 0, -9.81]) + np.array([0, 0, T]), rtol=1e-12,
+                                   atol=1e-12)
+        np.testing.assert_allclose(got[10:13], np.linalg.solve(Jm, tau - np.cross(w, Jm @ w)), rtol=1e-12, atol=1e-12)
+        eps = 1e-6
+        q2 = q + eps * got[3:7]
+        R2 = Rotation.from_quat([q2[1], q2[2], q2[3], q2[0]]).as_matrix()
+        wx = np.array([[0, -w[2], w[1]], [w[2], 0, -w[0]], [-w[1], w[0], 0]])
+        np.testing.assert_allclose(R2, R @ (np.eye(3) + eps * wx), atol=5e-11)
+    # hover: level, at rest, rotor speed sqrt(m g / 4): an equilibrium
+    xh = np.array([1.0, 2.0, 3.0, 1, 0, 0, 0, 0, 0, 0, 0, 0, 0])
+    assert np.max(np.abs(fam.quat_ode(list(xh), [np.sqrt(9.81 / 4)] * 4))) < 1e-14
