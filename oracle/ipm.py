@@ -502,7 +502,7 @@ class Solver:
             st.delta_w_last = dw
         tr["step"] = (dx, dy, dzL, dzU)
         # the linear system this step solved, for tests that want a second opinion on it (nothing below reads it)
-        tr["lin"] = dict(W=W, A=A, Sigma=Sigma, b=b, x=x, y=y, th=th, zL=st.zL, zU=st.zU, d=(dx, dy, dzL, dzU),
+        tr["lin"] = dict(W=W, A=A, Sigma=Sigma, b=b, x=x, y=y, th=th, tau=tau, zL=st.zL, zU=st.zU, d=(dx, dy, dzL, dzU),
                          tried=list(self.ic_tried))
         d = (dx, dy, dzL, dzU)
         # A-5 line search

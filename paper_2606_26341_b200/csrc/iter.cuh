@@ -333,7 +333,10 @@ struct Solver {
         // compulsory step while the stage recursion can stop anywhere below 1e-10; the error left in Delta y is that
         // ratio times cond(7).  Up to three more steps while the ratio is above 1e-15 and still shrinking bring the
         // step within the parity tolerance of the oracle's (eq 8); they change no decision.
-        for (int extra = 0; extra < o->polish_max && !failed && rat > 1e-15 && nref < o->refine_max; ++extra) {
+        // (restoration mode: the step mixes components of size 1e4 (p, n) with multipliers of size 1, and the ratio is
+        // norm-wise: polish until it stops shrinking)
+        const double polish_floor = mode ? 1e-18 : 1e-15;
+        for (int extra = 0; extra < o->polish_max && !failed && rat > polish_floor && nref < o->refine_max; ++extra) {
             reduced_solve(VX(L->r1), VH(L->r2), VX(L->r3), VX(L->r4), e1, e2, e3, e4);
             for (int i = lane; i < nX; i += NT) { d1[i] += e1[i]; d3[i] += e3[i]; d4[i] += e4[i]; }
             for (int i = lane; i < pb->m; i += NT) d2[i] += e2[i];

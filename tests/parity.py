@@ -86,6 +86,19 @@ def decisions_equal(gpu_rec: np.ndarray, otr: dict) -> tuple[bool, str]:
     return True, ""
 
 
+def iterate_gap(solver, lin, d):
+    """e_v (eq 8) between the iterates two solutions of the same step produce when each takes ITS OWN
+    largest step the line search considers: x + alpha_max(d) dx and y + alpha_max(d) dy with alpha_max from the
+    fraction-to-the-boundary rule (the step length inherits the rounding of dx, and y moves by alpha_max dy)."""
+    ref, x, tau = lin["d"], lin["x"], lin["tau"]
+    a_ref = solver.ftb_primal(x, ref[0], tau)
+    a_new = solver.ftb_primal(x, d[0], tau)
+    gap = e_v(x + a_new * d[0], x + a_ref * ref[0])
+    if solver.m:
+        gap = max(gap, e_v(a_new * d[1], a_ref * ref[1]))
+    return gap if np.isfinite(gap) else np.inf
+
+
 class LUFactor:
     """numpy/scipy LU with partial pivoting behind the interface of oracle.linsolve.DenseLDL.solve."""
 
@@ -100,9 +113,8 @@ class LUFactor:
 
 def second_opinion_gap(solver, tr):
     """How far two LAPACK solvers disagree on the linear system of this iteration: the oracle's Bunch-Kaufman LDL^T
-    against an LU with partial pivoting, both followed by the same refinement on (6) (reading S-7).  Measured with e_v of
-    eq (8) on the iterate the LARGEST step the line search considers would produce (x + alpha_max dx,
-    y + alpha_max dy).  A step on which two backward-stable library solvers already differ by more than the parity
+    against an LU with partial pivoting, both followed by the same refinement on (6) (reading S-7).  Measured with
+    iterate_gap: e_v of eq (8) on the iterates the largest step the line search considers would produce.  A step on which two backward-stable library solvers already differ by more than the parity
     tolerance cannot be asked of a third one: such steps are reported, not asserted."""
     lin = tr.get("lin")
     if lin is None:
@@ -115,13 +127,7 @@ def second_opinion_gap(solver, tr):
                                     lin["b"])
     except Exception:
         return np.inf
-    a = min(1.0, solver.ftb_primal(lin["x"], lin["d"][0], 0.99))
-    ref = lin["d"]
-    x = lin["x"]
-    gap = e_v(x + a * d[0], x + a * ref[0])
-    if solver.m:
-        gap = max(gap, e_v(a * d[1], a * ref[1]))
-    return gap if np.isfinite(gap) else np.inf
+    return iterate_gap(solver, lin, d)
 
 
 def perturbed_derivatives(solver, lin, rel, rng):
@@ -162,17 +168,22 @@ def sensitivity_gap(solver, tr, rel=1e-12, seed=1):
         d, _, _ = solver.solve_full(DenseLDL(K), Wp, Ap, lin["x"], lin["zL"], lin["zU"], tr["dw"], tr["dc"], lin["b"])
     except Exception:
         return np.inf
-    a = min(1.0, solver.ftb_primal(lin["x"], lin["d"][0], 0.99))
-    ref = lin["d"]
-    x = lin["x"]
-    gap = e_v(x + a * d[0], x + a * ref[0])
-    if solver.m:
-        gap = max(gap, e_v(a * d[1], a * ref[1]))
-    return gap if np.isfinite(gap) else np.inf
+    return iterate_gap(solver, lin, d)
 
 
 def step_is_well_posed(solver, tr, tol):
-    """(well-posed?, text): the three criteria above with the parity tolerance."""
+    """(well-posed?, text): the criteria above with the parity tolerance, plus the rounding floor of the step itself:
+    e_v (eq 8) is a COMPONENTWISE measure, and a solver that is backward stable in the usual normwise sense delivers every
+    component of (dx, dy) to within a few ulps of the LARGEST component.  When 8 eps alpha_max max(||dx||, ||dy||)_inf
+    already exceeds the tolerance, the small components of the next iterate cannot be asked to 1e-8 (seen on restoration
+    steps with delta_w 1e9: ||dy||_inf = 5e8, differences of 2e-6 on multipliers of size 200, i.e. 4e-14 of ||dy||)."""
+    lin = tr.get("lin")
+    if lin is not None:
+        a_ref = solver.ftb_primal(lin["x"], lin["d"][0], lin["tau"])
+        big = max(float(np.max(np.abs(lin["d"][0]))), float(np.max(np.abs(lin["d"][1]))) if solver.m else 0.0)
+        floor = 8.0 * 2.220446049250313e-16 * a_ref * big
+        if not np.isfinite(floor) or floor > tol:
+            return False, f"8 eps alpha_max ||step||_inf = {floor:.1e}"
     g1 = second_opinion_gap(solver, tr)
     if g1 > tol:
         return False, f"LAPACK LU vs Bunch-Kaufman {g1:.1e}"
@@ -182,6 +193,68 @@ def step_is_well_posed(solver, tr, tol):
     if len((tr.get("lin") or {}).get("tried", [])) > 1 and not inertia_is_stable(solver, tr):
         return False, "inertia changes under a rounding-level perturbation of W, A"
     return True, f"{max(g1, g2):.1e}"
+
+
+class WithGpuDerivatives:
+    """A problem that answers like `base` except that, AT THE POINT x_at, the dynamics blocks of its Jacobian and the
+    stage blocks of its Lagrangian Hessian are the ones the GPU evaluated (taken from the debug state).  Lets the oracle's
+    iteration run on exactly the matrices the kernel factorised: what is left between the two results is linear
+    algebra and line-search logic, with the rounding of the two derivative codes (asserted separately, block by block,
+    in test_derivative_blocks_against_oracle) taken out."""
+
+    def __init__(self, base, x_at, Jg, Wg, WNg):
+        self.base, self.x_at, self.Jg, self.Wg, self.WNg = base, np.array(x_at), Jg, Wg, WNg
+        for name in ("n", "m", "N", "nx", "nu", "ng", "na", "family", "dt", "ax", "au", "pdim"):
+            if hasattr(base, name):
+                setattr(self, name, getattr(base, name))
+
+    def __getattr__(self, name):
+        return getattr(self.base, name)
+
+    def _here(self, x):
+        return x.shape == self.x_at.shape and np.array_equal(x, self.x_at)
+
+    def jac(self, x, th):
+        A = self.base.jac(x, th)
+        if self._here(x):
+            b, nx, nu = self.base, self.base.nx, self.base.nu
+            for k in range(1, b.N + 1):
+                r = b.ic_dyn(k)
+                A[r:r + nx, b.ix(k - 1):b.ix(k - 1) + nx] = -self.Jg[k - 1][:, :nx]
+                A[r:r + nx, b.iu(k - 1):b.iu(k - 1) + nu] = -self.Jg[k - 1][:, nx:]
+        return A
+
+    def hess_lag(self, x, th, y, sigma_f=1.0):
+        W = self.base.hess_lag(x, th, y, sigma_f)
+        if self._here(x):
+            b, nx, nu = self.base, self.base.nx, self.base.nu
+            for k in range(b.N):
+                rows = list(range(b.ix(k), b.ix(k) + nx)) + list(range(b.iu(k), b.iu(k) + nu))
+                W[np.ix_(rows, rows)] = self.Wg[k]
+            rows = list(range(b.ix(b.N), b.ix(b.N) + nx))
+            W[np.ix_(rows, rows)] = self.WNg
+        return W
+
+
+def oracle_step_with_gpu_derivatives(osol, st_copy, theta, gpu_state, lay, d):
+    """Run ONE oracle iteration from st_copy (a deep copy of the oracle's state before the step) with the GPU's
+    derivative blocks substituted at the current point; returns (trace, state after)."""
+    import copy
+    n, N, nx, nz = d.n, d.horizon_N, d.nx, d.nx + d.nu
+    Jg = gpu_state[lay["J"]:lay["J"] + N * nx * nz].reshape(N, nx, nz)
+    Wg = gpu_state[lay["W"]:lay["W"] + N * nz * nz].reshape(N, nz, nz)
+    WNg = gpu_state[lay["W"] + N * nz * nz:lay["W"] + N * nz * nz + nx * nx].reshape(nx, nx)
+    sol = copy.copy(osol)
+    if st_copy.resto is None:
+        sol.p = WithGpuDerivatives(osol.p, st_copy.x, Jg, Wg, WNg)
+    else:
+        sub = copy.copy(st_copy.resto.sub)
+        rp = copy.copy(sub.p)
+        rp.base = WithGpuDerivatives(rp.base, st_copy.resto.state.x[:n], Jg, Wg, WNg)
+        sub.p = rp
+        st_copy.resto.sub = sub
+    tr = sol.iterate(st_copy, theta)
+    return tr, st_copy
 
 
 def inertia_is_stable(solver, tr, rel=1e-12, seed=0):
