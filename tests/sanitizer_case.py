@@ -12,7 +12,7 @@ from paper_2606_26341_b200 import jipm, workloads as wl  # noqa: E402
 CASES = [("C0 batch 8", 0, {}, 8, 5, {}),
          ("C1 batch 2", 1, {}, 2, 5, {}),
          ("C1 reduced, watchdog after one shortened step", 1, dict(horizon_N=7), 4, 40, dict(watchdog_trigger=1)),
-         ("C3 reduced (restoration)", 3, dict(horizon_N=6, n_obstacles=5), 2, 40, {}),
+         ("C3 reduced (restoration phases)", 3, dict(horizon_N=6, n_obstacles=5), 2, 120, {}),
          ("C2 reduced (2 agents)", 2, dict(horizon_N=5, n_agents=2), 2, 6, {}),
          ("N3 quaternion family reduced", 5, dict(horizon_N=8), 2, 6, {})]
 

@@ -549,6 +549,25 @@ def test_batch_size_slot_and_order_independence():
             assert np.array_equal(res[k], ref[k][idx]), (R, k)
 
 
+@pytest.mark.parametrize("cfg", [1, 2, 3, 5])
+def test_repeated_runs_are_bit_identical(cfg):
+    """compute-sanitizer is closed on this GPU pool (profiles/r2_sanitizer.md); this is the race check that can be run:
+    the same reduced batch -- restoration, watchdog and soft-restoration paths included -- solved three times, with
+    different numbers of resident slots (so different neighbours and SM placement): every output bit-identical."""
+    d = wl.config_dims(cfg, **REDUCED[cfg])
+    d, theta, x0 = wl.generate(cfg, 24, d)
+    ref = None
+    for R in (0, 5, 24):
+        s, _, _ = make_solver(d, resident_slots=R)
+        res = {k: v.cpu().numpy() for k, v in s.solve_batch(x0, theta).items()}
+        s.close()
+        if ref is None:
+            ref = res
+            continue
+        for k in ("x", "lam", "zL", "zU", "status", "iters"):
+            assert np.array_equal(res[k], ref[k], equal_nan=True), (cfg, R, k)
+
+
 def test_host_entry_matches_device_entry_and_edge_cases():
     from paper_2606_26341_b200 import jipm
     d, theta, x0 = wl.generate(0, 37)
