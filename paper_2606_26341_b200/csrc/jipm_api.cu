@@ -152,21 +152,30 @@ static int build_layout(jipm_solver* s, int sm_budget_doubles) {
     };
     int o = 0;
     L.nsm = 0;
+    L.pv0 = 0; L.npad = npad; L.tpad = tpad;
+    const int n_primal = (int)(sizeof(primal) / sizeof(primal[0]));
+    auto even = [](int c) { return (c + 1) & ~1; };  // keep 16-byte alignment
+    int hot_total = 0;
+    for (const Ent& e : hot) hot_total += even(e.cnt);
+    const int hot_fits = hot_total <= sm_budget_doubles ? 1 : 0;  // the whole hot group is shared-memory resident
+    // Arrays are placed in priority order; the first that does not fit ends the shared-memory part (everything after
+    // it lives in the slot's L2 scratch).  A first-fit variant that keeps the small vectors on chip and sends the
+    // factor blocks to L2 was measured on C2, C3 and the quaternion family and is 4-9 % SLOWER per slot-iteration
+    // (DESIGN.md section 6): the factor blocks and J are the hotter data.
     bool in_sm = true;
     auto place = [&](int Lay::*f, int cnt0) {
-        const int cnt = (cnt0 + 1) & ~1;  // keep 16-byte alignment
+        const int cnt = even(cnt0);
         if (in_sm && o + cnt > sm_budget_doubles) { in_sm = false; L.nsm = o; }
         L.*f = o;
         o += cnt;
     };
     for (const Ent& e : hot) place(e.f, e.cnt);
-    const int hot_fits = in_sm ? 1 : 0;  // the whole hot group is shared-memory resident
-    L.pv0 = o; L.npad = npad; L.tpad = tpad;
+    L.pv0 = o;
     for (auto f : primal) place(f, n);
     for (const Ent& e : cold) place(e.f, e.cnt);
     if (in_sm) { in_sm = false; L.nsm = o; }
     L.tail0 = o;
-    o += tpad * (int)(sizeof(primal) / sizeof(primal[0]));
+    o += tpad * n_primal;
     L.total = o;
     return hot_fits;
 }

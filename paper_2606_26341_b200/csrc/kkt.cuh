@@ -23,11 +23,16 @@
 #pragma once
 #include "core.cuh"
 
+#ifndef JIPM_USE_DMMA
+#define JIPM_USE_DMMA 1   // FP64 tensor-core path of the multi-agent stage products (measured: DESIGN.md section 6)
+#endif
+
 namespace jipm {
 
 template <class C>
 struct Kkt {
     static constexpr int NX = C::NX, NU = C::NU, NZ = C::NZ, PD = C::PD, AX = C::AX, AU = C::AU, NA = C::NA, NT = C::NT, LDJ = C::LDJ;
+    static constexpr bool USE_DMMA = JIPM_USE_DMMA != 0;
     using X = Ctx<C>;
     // J_k = [A B] is block diagonal over the agents (AX x (AX | AU) blocks): every product with J runs over one
     // agent's rows / columns only.  agent of column j of z = (x, u):
@@ -55,6 +60,16 @@ struct Kkt {
             if (NE % NT == 0 || e < NE) f(e);
         }
     }
+
+    // FP64 tensor-core MMA (sm_80+ "DMMA", legacy warp-level path: tcgen05 has no f64 kind): D(8x8) += A(8x4) B(4x8).
+    // Lane l holds A[l/4][l%4], B[l%4][l/4] and D[l/4][2(l%4)], D[l/4][2(l%4)+1].  Used only for the multi-agent
+    // family, whose stage products are 48 x 12 x 16 / 16 x 12 x 64 contractions per agent.
+    __device__ static __forceinline__ void dmma884(double& d0, double& d1, double a, double b) {
+        asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                     : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+    }
+    // index in z = (x, u) of entry c (0 .. AX+AU-1) of agent a's own (x_a, u_a)
+    __device__ static __forceinline__ int zmap(int a, int c) { return c < AX ? AX * a + c : NX + AU * a + (c - AX); }
 
     // dot product with 4 independent partial sums (dependent-chain latency / 4), compile-time length and strides: fully unrolled, immediate offsets
     template <int LEN, int SA, int SB>
@@ -243,25 +258,61 @@ struct Kkt {
                 c.tm.sync();
             }
             // TJ = T_{k+1} J_k
+            if constexpr (NA > 1 && USE_DMMA) {
+                // per agent a: TJ[:, z_a] = T[:, x_a] (NX x AX) * J_a (AX x (AX+AU)) on the FP64 tensor cores
+                constexpr int AZ = AX + AU, MT = NX / 8, NTL = AZ / 8;
+                static_assert(AX % 4 == 0 && NX % 8 == 0 && AZ % 8 == 0, "DMMA tiling");
+                const int wl = lane & 31, g = wl >> 2, t = wl & 3;
+                for (int tile = lane >> 5; tile < NA * MT * NTL; tile += NT / 32) {
+                    const int a = tile / (MT * NTL), rem = tile % (MT * NTL), mt = rem / NTL, nt = rem % NTL;
+                    double d0 = 0.0, d1 = 0.0;
+                    const int cB = zmap(a, 8 * nt + g);
+#pragma unroll
+                    for (int ks = 0; ks < AX / 4; ++ks)
+                        dmma884(d0, d1, sT[(8 * mt + g) * NX + AX * a + 4 * ks + t], sJ[(AX * a + 4 * ks + t) * LDJ + cB]);
+                    sTJ[(8 * mt + g) * NZ + zmap(a, 8 * nt + 2 * t)] = d0;
+                    sTJ[(8 * mt + g) * NZ + zmap(a, 8 * nt + 2 * t + 1)] = d1;
+                }
+            } else {
             tile_for<NX * NZ>(lane, [&](int e) {
                 const int l = e / NZ, j = e % NZ;
                 const int aj = col_agent(j);
                 sTJ[e] = dotc<AX, 1, LDJ>(sT + l * NX + AX * aj, sJ + AX * aj * LDJ + j);
             });
+            }
             c.tm.sync();
             { const long long t2 = clock64(); c.tick(8, t2 - tq); tq = t2; }
             // M = Q_k + J^T (T J) + condensed slacks
             const double* Wg = c.Wk(k);
-            tile_for<NZ * NZ>(lane, [&](int e) {
-                const int a = e / NZ, j = e % NZ;
-                const int aa = col_agent(a);
-                double m = dotc<AX, LDJ, NZ>(sJ + AX * aa * LDJ + a, sTJ + AX * aa * NZ + j);
-                if (useW) m += Wg[e];
+            auto m_extra = [&](double m, int a, int j) {  // what M gets besides J^T (T J): W, Sigma, the condensed slacks
+                if (useW) m += Wg[a * NZ + j];
                 if (a == j) m += Sig[c.zidx(k, j)];
                 if (k >= 1 && ng > 0 && a < NX && j < NX && a % AX < PD && j % AX < PD)
                     m += cnd[(k - 1) * NPOS * NPOS + (PD * (a / AX) + a % AX) * NPOS + PD * (j / AX) + j % AX];
-                tA[e] = m;
+                return m;
+            };
+            if constexpr (NA > 1 && USE_DMMA) {
+                // per agent aa: M[z_aa, :] = J_aa^T ((AX+AU) x AX) * TJ[x_aa, :] (AX x NZ)
+                constexpr int AZ = AX + AU, MTm = AZ / 8, NTn = NZ / 8;
+                const int wl = lane & 31, g = wl >> 2, t = wl & 3;
+                for (int tile = lane >> 5; tile < NA * MTm * NTn; tile += NT / 32) {
+                    const int aa = tile / (MTm * NTn), rem = tile % (MTm * NTn), mt = rem / NTn, nt = rem % NTn;
+                    double d0 = 0.0, d1 = 0.0;
+                    const int rA = zmap(aa, 8 * mt + g);
+#pragma unroll
+                    for (int ks = 0; ks < AX / 4; ++ks)
+                        dmma884(d0, d1, sJ[(AX * aa + 4 * ks + t) * LDJ + rA], sTJ[(AX * aa + 4 * ks + t) * NZ + 8 * nt + g]);
+                    const int j0 = 8 * nt + 2 * t;
+                    tA[rA * NZ + j0] = m_extra(d0, rA, j0);
+                    tA[rA * NZ + j0 + 1] = m_extra(d1, rA, j0 + 1);
+                }
+            } else {
+            tile_for<NZ * NZ>(lane, [&](int e) {
+                const int a = e / NZ, j = e % NZ;
+                const int aa = col_agent(a);
+                tA[e] = m_extra(dotc<AX, LDJ, NZ>(sJ + AX * aa * LDJ + a, sTJ + AX * aa * NZ + j), a, j);
             });
+            }
             c.tm.sync();
             { const long long t2 = clock64(); c.tick(9, t2 - tq); tq = t2; }
             // Gauss-Jordan pivots on the controls NX .. NZ-1, four per barrier: every element from the previous tile

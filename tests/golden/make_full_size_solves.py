@@ -23,8 +23,8 @@ import numpy as np  # noqa: E402
 from oracle import families as ofam, ipm as oipm  # noqa: E402
 from paper_2606_26341_b200 import workloads as wl  # noqa: E402
 
-COUNT = {1: 48, 2: 16, 3: 32, 5: 48}
-MAX_ITER = {1: 3000, 2: 600, 3: 1500, 5: 3000}   # the oracle is cut here; a problem that reaches the cap is stored as such
+COUNT = {1: 48, 2: 8, 3: 8, 5: 16}
+MAX_ITER = {1: 3000, 2: 300, 3: 600, 5: 3000}   # the oracle is cut here; a problem that reaches the cap is stored as such
 
 
 def solve_one(args):
