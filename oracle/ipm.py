@@ -93,6 +93,14 @@ class Options:
     tiny_step_cviol: float = 1e-4
     soft_resto_factor: float = 1.0 - 1e-4   # required reduction of the primal-dual error (0 = off)
     max_soft_resto_iters: int = 10
+    # Table I row 7 (reading AM of DESIGN.md section 3): 0 = monotone schedule (IPOPT's default),
+    # 1 = adaptive barrier parameter (Mehrotra probing) with the switch to the monotone schedule
+    mu_strategy: int = 0
+    adaptive_red_fact: float = 0.9999       # required reduction of the KKT error w.r.t. the last adaptive_red_iters
+    adaptive_red_iters: int = 4
+    adaptive_monotone_init: float = 0.8     # mu of the monotone phase = this x average complementarity
+    adaptive_sigma_max: float = 100.0
+    adaptive_mu_max_fact: float = 1e3       # mu never exceeds this x the first average complementarity
 
     @property
     def mu_min(self) -> float:
@@ -120,6 +128,9 @@ class State:
     soft_count: int = 0
     tiny_last: bool = False           # the previous iteration took a tiny step (Table I row 4)
     tiny_flag: bool = False           # two tiny steps in a row: force a barrier decrease at the next A-3
+    mu_free: bool = True              # adaptive strategy (Table I row 7): free mode (True) or monotone phase
+    kkt_hist: list = field(default_factory=list)   # KKT errors of the last accepted free-mode iterates
+    mu_max: float = -1.0              # upper bound of the adaptive mu (set at the first iteration)
 
 
 @dataclass
@@ -457,7 +468,35 @@ class Solver:
         # too small to make progress: TINY_STEP.
         force = st.tiny_flag
         st.tiny_flag = False
-        while tr["nmu"] < o.max_mu_updates and (
+        adaptive = o.mu_strategy == 1 and not hasattr(p, "set_mu") and (self.nL + self.nU) > 0
+        tr["mu_mode"], tr["mu_switch"] = 0, 0
+        if adaptive:
+            # Table I row 7: the adaptive rule runs while the KKT error keeps falling ("free mode");
+            # when an iterate fails to reduce it below adaptive_red_fact x the largest of the last adaptive_red_iters
+            # values, the monotone schedule takes over from mu = adaptive_monotone_init x average complementarity
+            # until its barrier problem is solved; then the adaptive rule returns.
+            sLc, sUc = self.slacks(x)
+            avg = (float(np.sum((sLc * st.zL)[self.hasL])) + float(np.sum((sUc * st.zU)[self.hasU]))) / (self.nL + self.nU)
+            kkt = self.pd_error(x, y, st.zL, st.zU, g, cv, A, 0.0)
+            if st.mu_max < 0.0:
+                st.mu_max = o.adaptive_mu_max_fact * avg
+            if st.mu_free:
+                hist = st.kkt_hist[-o.adaptive_red_iters:]
+                if hist and kkt > o.adaptive_red_fact * max(hist):
+                    st.mu_free = False
+                    st.mu = min(st.mu_max, max(o.mu_min, o.adaptive_monotone_init * avg))
+                    st.tau = max(o.tau_min, 1.0 - st.mu)
+                    st.filt = []
+                    st.wd, st.n_short, st.soft, st.soft_count = None, 0, False, 0
+                    tr["mu_switch"] = 1
+                else:
+                    st.kkt_hist = hist + [kkt]
+            elif self.opt_error(x, y, st.zL, st.zU, g, cv, A, st.mu) <= o.kappa_eps * st.mu:
+                st.mu_free = True
+                st.kkt_hist = [kkt]
+                tr["mu_switch"] = 2
+            tr["mu_mode"] = 1 if st.mu_free else 2
+        while not adaptive and tr["nmu"] < o.max_mu_updates and (
                 force or self.opt_error(x, y, st.zL, st.zU, g, cv, A, st.mu) <= o.kappa_eps * st.mu):
             if not st.mu > o.mu_min:
                 if force:
@@ -474,17 +513,13 @@ class Solver:
             if hasattr(p, "set_mu"):
                 p.set_mu(st.mu)
                 fv, g = p.f(x, th), p.grad_f(x, th)
-        mu, tau = st.mu, st.tau
         W = p.hess_lag(x, th, y, 1.0)
         # A-4 search direction
         sL, sU = self.slacks(x)
         Sigma = np.where(self.hasL, st.zL / sL, 0.0) + np.where(self.hasU, st.zU / sU, 0.0)
-        gphi = self.grad_phi(x, g, mu)
-        b = [-(g + A.T @ y - st.zL + st.zU + self.damping(mu)), -cv,
-             np.where(self.hasL, mu - sL * st.zL, 0.0), np.where(self.hasU, mu - sU * st.zU, 0.0)]
-        resume = None
+        resume, probed = None, False
         while True:
-            ic = self.inertia_correction(W, Sigma, A, mu, st.delta_w_last, resume)
+            ic = self.inertia_correction(W, Sigma, A, st.mu, st.delta_w_last, resume)
             if ic is None:
                 tr["kind"] = "ic_fail"
                 tr["nfact"] = tr["nref"] = 0
@@ -492,6 +527,28 @@ class Solver:
                 return self.enter_restoration(st, th, tr, fv, cv)
             fac, dw, dc, nf = ic
             tr["nfact"] += nf
+            if adaptive and st.mu_free and not probed:
+                # Mehrotra's probing with the factorisation of this iteration (it does not depend on mu): the
+                # affine-scaling step is the Newton step on (5) with mu = 0; mu_aff = average complementarity after
+                # the largest step that stays feasible; sigma = (mu_aff / average complementarity)^3; mu = sigma x avg.
+                probed = True
+                b_aff = [-(g + A.T @ y - st.zL + st.zU), -cv, np.where(self.hasL, -sL * st.zL, 0.0),
+                         np.where(self.hasU, -sU * st.zU, 0.0)]
+                da, _, _ = self.solve_full(fac, W, A, x, st.zL, st.zU, dw, dc, b_aff)
+                a_p = self.ftb_primal(x, da[0], 1.0)
+                a_d = self.ftb_dual(st.zL, st.zU, da[2], da[3], 1.0)
+                mu_aff = (float(np.sum(((sL + a_p * da[0]) * (st.zL + a_d * da[2]))[self.hasL]))
+                          + float(np.sum(((sU - a_p * da[0]) * (st.zU + a_d * da[3]))[self.hasU]))) / (self.nL + self.nU)
+                sigma = min(o.adaptive_sigma_max, (mu_aff / avg) ** 3) if avg > 0.0 else 1.0
+                tr["sigma"], tr["mu_aff"], tr["aff_step"] = sigma, mu_aff, da
+                st.mu = min(st.mu_max, max(o.mu_min, sigma * avg))
+                st.tau = max(o.tau_min, 1.0 - st.mu)
+                st.filt = []
+                st.wd, st.n_short, st.soft, st.soft_count = None, 0, False, 0
+            mu, tau = st.mu, st.tau
+            gphi = self.grad_phi(x, g, mu)
+            b = [-(g + A.T @ y - st.zL + st.zU + self.damping(mu)), -cv,
+                 np.where(self.hasL, mu - sL * st.zL, 0.0), np.where(self.hasU, mu - sU * st.zU, 0.0)]
             (dx, dy, dzL, dzU), tr["nref"], failed = self.solve_full(fac, W, A, x, st.zL, st.zU, dw, dc, b)
             if not failed:
                 break

@@ -324,3 +324,76 @@ def test_solve_full_reports_failure_only_above_the_singular_ratio():
     s.o.residual_ratio_singular = 1e300
     d, nref, failed = s.solve_full(bad, W, A, x, z, z, 0.0, 0.0, b)
     assert not failed
+
+
+# ---- adaptive barrier parameter with the switch to the monotone schedule (Table I row 7) ------------------------
+def one_dim_bound_problem():
+    return SmallNLP(1, 0, lambda x: x[0], lambda x: [1.0], lambda x: [[0.0]])
+
+
+def test_adaptive_mu_probing_by_hand():
+    """min x s.t. x >= 0 at x = 0.5, z = 2 (no damping, no bound relaxation).  Affine-scaling step = Newton step on (5)
+    with mu = 0:  row 1 of (6): -dz = -(1 - 2) -> dz = -1;  row 3: z dx + s dz = -s z -> 2 dx - 0.5 = -1 -> dx = -0.25.
+    Both reach at most half-way to their bounds, so the step lengths to the boundary are 1:
+    mu_aff = (0.5 - 0.25)(2 - 1) = 0.25, average complementarity s z = 1, sigma = 0.25^3 = 1/64, mu = 0.015625;
+    the upper bound of mu is 1e3 x the first average complementarity = 1000; the filter is reset."""
+    o = ipm.Options(mu_strategy=1, kappa_d=0.0, bound_relax_factor=0.0)
+    s = ipm.Solver(one_dim_bound_problem(), [0.0], [INF], o)
+    st = s.initialise([0.5], None)
+    st.zL[:] = 2.0
+    st.filt = [(1.0, 1.0)]
+    tr = s.iterate(st, None)
+    assert tr["mu_mode"] == 1 and tr["mu_switch"] == 0
+    np.testing.assert_allclose(tr["aff_step"][0], [-0.25], rtol=1e-13)
+    np.testing.assert_allclose(tr["aff_step"][2], [-1.0], rtol=1e-13)
+    assert tr["mu_aff"] == pytest.approx(0.25, rel=1e-13) and tr["sigma"] == pytest.approx(1.0 / 64.0, rel=1e-13)
+    assert st.mu == pytest.approx(0.015625, rel=1e-13) and st.mu_max == pytest.approx(1000.0)
+    assert st.tau == max(0.99, 1.0 - st.mu) and st.kkt_hist and len(st.kkt_hist) == 1
+    # the Newton step of the iteration used the NEW mu: Sigma = 4, grad phi = 1 - mu/0.5, dx = -(1 - 2 mu)/4
+    np.testing.assert_allclose(tr["step"][0], [-(1.0 - 2.0 * 0.015625) / 4.0], rtol=1e-12)
+    # mu is clipped at its floor: from z = 1 the affine step reaches the bound exactly, mu_aff = 0
+    st = s.initialise([0.5], None)
+    s.iterate(st, None)
+    assert st.mu == o.mu_min
+
+
+def test_adaptive_mu_switches_to_monotone_and_back():
+    """Free mode keeps the KKT errors of the last 4 accepted iterates; an iterate whose error exceeds 0.9999 x the largest
+    of them sends the solver to the monotone schedule with mu = 0.8 x average complementarity (filter reset, no probing);
+    it returns to the adaptive rule once the barrier problem is solved (E_mu <= 10 mu)."""
+    o = ipm.Options(mu_strategy=1, kappa_d=0.0, bound_relax_factor=0.0)
+    s = ipm.Solver(one_dim_bound_problem(), [0.0], [INF], o)
+    st = s.initialise([0.5], None)
+    st.zL[:] = 2.0
+    # KKT error here: |1 - z| / 1 + |s z - 0| / 1 = 1 + 1 = 2
+    st.kkt_hist = [9.0, 1.5, 1.9, 1.0, 1.2]          # only the last four count: max 1.9 < 2 -> no progress
+    tr = s.iterate(st, None)
+    assert tr["mu_switch"] == 1 and tr["mu_mode"] == 2 and not st.mu_free and "sigma" not in tr
+    assert st.mu == pytest.approx(0.8, rel=1e-14)
+    # with the same history but its largest recent value 2.1 the iterate counts as progress and is appended
+    st = s.initialise([0.5], None)
+    st.zL[:] = 2.0
+    st.kkt_hist = [9.0, 1.5, 2.1, 1.0, 1.2]
+    tr = s.iterate(st, None)
+    assert tr["mu_switch"] == 0 and st.mu_free and st.kkt_hist[:4] == [1.5, 2.1, 1.0, 1.2] and len(st.kkt_hist) == 5
+    # monotone phase: mu stays until E_mu <= kappa_eps mu, then the adaptive rule is back with a fresh history
+    st = s.initialise([0.5], None)
+    st.zL[:] = 2.0
+    st.mu_free, st.mu, st.mu_max = False, 1e-3, 1000.0   # E_mu = max(|1-2|, |1 - 1e-3|) = 1 > 10 * 1e-3: stay
+    tr = s.iterate(st, None)
+    assert tr["mu_mode"] == 2 and tr["mu_switch"] == 0 and st.mu == 1e-3 and tr["nmu"] == 0
+    st = s.initialise([0.5], None)
+    st.zL[:] = 2.0
+    st.mu_free, st.mu, st.mu_max = False, 0.8, 1000.0    # E_mu = 1 <= 8: solved -> free mode, probing in the same iteration
+    tr = s.iterate(st, None)
+    assert tr["mu_switch"] == 2 and tr["mu_mode"] == 1 and st.mu_free and "sigma" in tr and len(st.kkt_hist) == 1
+
+
+def test_adaptive_mu_solves_the_same_problems():
+    """The adaptive strategy reaches the same solutions as the monotone one on box QPs (closed form: clip)."""
+    a = np.array([-2.0, 0.3, 5.0, 0.9, -0.5])
+    l, u = np.full(5, -1.0), np.full(5, 1.0)
+    p = SmallNLP(5, 0, lambda x: 0.5 * (x - a) @ (x - a), lambda x: x - a, lambda x: np.eye(5))
+    st = ipm.Solver(p, l, u, ipm.Options(mu_strategy=1)).solve(np.zeros(5), None)
+    assert st.status == ipm.ST_SOLVED
+    np.testing.assert_allclose(st.x, np.clip(a, l, u), atol=2e-7)
