@@ -59,11 +59,15 @@ typedef struct {
     /* refinement failure ("pretend singular", reading S-7) and Table I rows 3-5 */
     double residual_ratio_singular, residual_improvement_factor;
     double tiny_step_tol, tiny_step_y_tol, tiny_step_cviol, soft_resto_factor;
+    /* adaptive barrier parameter with the switch to the monotone schedule (Table I row 7) */
+    double adaptive_red_fact, adaptive_monotone_init, adaptive_sigma_max, adaptive_mu_max_fact;
     int32_t max_iter, max_backtrack, max_soc, refine_min, refine_max, max_mu_updates;
     int32_t init_slacks, enable_restoration;
     int32_t watchdog_trigger, watchdog_trial_max, max_soft_resto_iters;
     int32_t polish_max; /* extra refinement steps (<= this many) taken after the stop rule is met while the residual ratio
                            is above 1e-15 and still shrinking: accuracy of the step only, no decision depends on it */
+    int32_t mu_strategy;        /* 0 monotone schedule (default, IPOPT's), 1 adaptive (Mehrotra probing) with the switch */
+    int32_t adaptive_red_iters; /* KKT errors remembered by the progress test of the adaptive mode */
 } jipm_options;
 
 /* Fill *o with the defaults.  o: HOST.  Returns JIPM_ERR_ARG if o is NULL. */
@@ -131,8 +135,10 @@ int jipm_residency(jipm_solver* s, int64_t* res);
  *        4 gave up: back at the entry iterate, backtracked from there)
  *   [17] soft restoration (0 none, 1 step accepted by the error reduction, 2 accepted by the original criterion)
  *   [18] tiny step taken? [19] #refinement failures treated as a singular matrix
+ *   [20] barrier strategy of the iteration (0 monotone schedule, 1 adaptive rule, 2 monotone phase of the adaptive
+ *        strategy) [21] switch taken (0 none, 1 adaptive -> monotone, 2 monotone -> adaptive)
  *   kind [5] also takes 5 = tiny step, 6 = soft restoration step. */
-#define JIPM_TRACE_W 20
+#define JIPM_TRACE_W 22
 /* Enable tracing for the next solves: trace DEVICE [P x max_records x JIPM_TRACE_W] (or NULL to disable). */
 int jipm_debug_set_trace(jipm_solver* s, double* trace, int64_t max_records);
 
@@ -144,9 +150,9 @@ int jipm_debug_set_trace(jipm_solver* s, double* trace, int64_t max_records);
  * theta_max, #filter entries, theta at entry, zeta), [16]=(p, n) [2m], [17]=(z_p, z_n) [2m], [18]=x_R [n],
  * [19]=restoration filter (256 pairs).  With mode = 1 the fields [1]-[5] hold the restoration iterate and scalars
  * and [6] still holds the REGULAR filter.
- * Line-search memory of the active problem (Table I rows 3-5): [20]=16 scalars (#consecutive shortened steps,
+ * Line-search memory of the active problem (Table I rows 3-5, 7): [20]=24 scalars (#consecutive shortened steps,
  * watchdog active?, #watchdog trials, watchdog reference theta, phi, grad_phi^T d, alpha, soft phase?, #soft
- * iterations, last step tiny?, tiny flag), [21]=watchdog entry iterate and direction: x, z_L, z_U, dx, dz_L, dz_U
+ * iterations, last step tiny?, tiny flag, adaptive mode free?, upper bound of mu, #remembered KKT errors, the errors [4]), [21]=watchdog entry iterate and direction: x, z_L, z_U, dx, dz_L, dz_U
  * (n + 2m each: the restoration variables follow the n entries), then y, dy (m each). */
 int jipm_debug_state_layout(jipm_solver* s, int64_t* lay, int64_t n_lay);
 

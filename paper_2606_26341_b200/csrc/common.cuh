@@ -38,6 +38,7 @@ struct Lay {
     int xR, DR2, filtR, rc2;  // restoration mode: reference point, scaling D_R^2, its own filter, condensed rhs
     // watchdog (Table I row 3): entry iterate and its search direction
     int wx, wzL, wzU, wdx, wdzL, wdzU, wy, wdy;
+    int ab1, ab3, ab4;   // right-hand side of the affine-scaling step (adaptive barrier parameter, Table I row 7)
 };
 
 // per-launch arguments
@@ -81,9 +82,9 @@ __host__ __device__ inline DbgLay make_dbglay(int n, int m, int N, int NX, int N
     d.J = o; o += N * NX * NZ; d.W = o; o += N * NZ * NZ + NX * NX;
     // restoration mode (Step R): scalars, (p, n), (z_p, z_n), reference point x_R, the restoration filter
     d.rs = o; o += 16; d.pn = o; o += 2 * m; d.zpn = o; o += 2 * m; d.xR = o; o += n; d.filtR = o; o += 2 * MAX_FILTER;
-    // line-search memory (Table I rows 3-5): 16 scalars; the watchdog's entry iterate and direction: six vectors of
+    // line-search memory (Table I rows 3-5, 7): 24 scalars; the watchdog's entry iterate and direction: six vectors of
     // n + 2m (x, zL, zU, dx, dzL, dzU), then y, dy
-    d.ls = o; o += 16; d.wd = o; o += 6 * (n + 2 * m) + 2 * m;
+    d.ls = o; o += 24; d.wd = o; o += 6 * (n + 2 * m) + 2 * m;
     d.len = o;
     return d;
 }

@@ -34,6 +34,10 @@ struct Solver {
     // barrier parameter changes and on entering / leaving restoration, so nothing is parked across modes
     int n_short, wd_active, wd_trials, soft, soft_count, tiny_last, tiny_flag;
     double wd_theta, wd_phi, wd_gd, wd_alpha;
+    // adaptive barrier parameter (Table I row 7): free mode or monotone phase, the upper bound of mu,
+    // the KKT errors of the last accepted free-mode iterates (regular problem only; restoration is always monotone)
+    int mu_free, nhist;
+    double mu_max, hist[4];
     // restoration mode (Table I row 6): mode 1 iterates on X = [x; p; n] with the same kernel
     // code; the regular problem's scalars are parked in *_reg until the exit test succeeds
     int mode, nX, nfilt_reg;
@@ -58,6 +62,10 @@ struct Solver {
     __device__ __forceinline__ void reset_ls_memory() {
         n_short = wd_active = wd_trials = soft = soft_count = tiny_last = tiny_flag = 0;
         wd_theta = wd_phi = wd_gd = wd_alpha = 0.0;
+    }
+    __device__ __forceinline__ void reset_mu_memory() {
+        mu_free = 1; nhist = 0; mu_max = -1.0;
+        hist[0] = hist[1] = hist[2] = hist[3] = 0.0;
     }
     __device__ __forceinline__ double* V(int off) const { return c.v(off); }
     __device__ __forceinline__ double* VH(int off) const { return c.vh(off); }
@@ -333,9 +341,7 @@ struct Solver {
         // compulsory step while the stage recursion can stop anywhere below 1e-10; the error left in Delta y is that
         // ratio times cond(7).  Up to three more steps while the ratio is above 1e-15 and still shrinking bring the
         // step within the parity tolerance of the oracle's (eq 8); they change no decision.
-        // (restoration mode: the step mixes components of size 1e4 (p, n) with multipliers of size 1, and the ratio is
-        // norm-wise: polish until it stops shrinking)
-        const double polish_floor = mode ? 1e-18 : 1e-15;
+        const double polish_floor = 1e-15;
         for (int extra = 0; extra < o->polish_max && !failed && rat > polish_floor && nref < o->refine_max; ++extra) {
             reduced_solve(VX(L->r1), VH(L->r2), VX(L->r3), VX(L->r4), e1, e2, e3, e4);
             for (int i = lane; i < nX; i += NT) { d1[i] += e1[i]; d3[i] += e3[i]; d4[i] += e4[i]; }

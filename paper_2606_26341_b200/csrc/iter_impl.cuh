@@ -89,6 +89,7 @@ __device__ void Solver<C>::init_problem(long long id) {
     theta_min = o->theta_min_fact * fmax(1.0, theta);
     nfilt = 0; k = 0; nrec = 0;
     reset_ls_memory();
+    reset_mu_memory();
     status = fin ? JIPM_ST_NOT_RUN : JIPM_ST_NONFINITE;
 }
 
@@ -588,7 +589,48 @@ __device__ void Solver<C>::iterate() {
     const double mu_min = o->tol / 10.0;
     bool force = tiny_flag != 0;
     tiny_flag = 0;
-    while (nmu < o->max_mu_updates && (force || opt_error(mu, sd, sc) <= o->kappa_eps * mu)) {
+    const int ncomp = pb->nL + pb->nU;
+    const bool adaptive = o->mu_strategy == 1 && mode == 0 && ncomp > 0;
+    double avg = 0.0;
+    if (adaptive) {
+        // Table I row 7: the adaptive rule runs while the KKT error keeps falling ("free mode"); an
+        // iterate that fails to bring it below adaptive_red_fact x the largest of the last adaptive_red_iters values
+        // hands over to the monotone schedule from mu = adaptive_monotone_init x average complementarity until its
+        // barrier problem is solved; then the adaptive rule returns.  (b1 holds the dual residual without damping.)
+        double s1 = 0.0, s3 = 0.0;
+        for (int i = lane; i < nX; i += NT) {
+            const double l = lo(i), u = hi(i);
+            s1 += fabs(b1[i]);
+            if (l > -INFINITY) s3 += (x[i] - l) * zL[i];
+            if (u < INFINITY) s3 += (u - x[i]) * zU[i];
+        }
+        s1 = c.tm.sum(s1); s3 = c.tm.sum(s3);
+        avg = s3 / ncomp;
+        const double kkt = s1 / nX + (m > 0 ? theta / m : 0.0) + s3 / ncomp;
+        if (mu_max < 0.0) mu_max = o->adaptive_mu_max_fact * avg;
+        const int keep = o->adaptive_red_iters < 4 ? o->adaptive_red_iters : 4;
+        if (mu_free) {
+            double hmax = 0.0;
+            const int nh = nhist < keep ? nhist : keep;
+            for (int q = 0; q < nh; ++q) hmax = fmax(hmax, hist[(nhist - 1 - q) & 3]);
+            if (nh > 0 && kkt > o->adaptive_red_fact * hmax) {
+                mu_free = 0;
+                mu = fmin(mu_max, fmax(mu_min, o->adaptive_monotone_init * avg));
+                tau = fmax(o->tau_min, 1.0 - mu);
+                nfilt = 0;
+                wd_active = 0; wd_trials = 0; n_short = 0; soft = 0; soft_count = 0;
+                rec[21] = 1.0;
+            } else {
+                hist[nhist & 3] = kkt; nhist++;
+            }
+        } else if (opt_error(mu, sd, sc) <= o->kappa_eps * mu) {
+            mu_free = 1;
+            hist[0] = kkt; nhist = 1;
+            rec[21] = 2.0;
+        }
+        rec[20] = mu_free ? 1.0 : 2.0;
+    }
+    while (!adaptive && nmu < o->max_mu_updates && (force || opt_error(mu, sd, sc) <= o->kappa_eps * mu)) {
         if (!(mu > mu_min)) {
             if (force) {
                 status = mode ? JIPM_ST_RESTORATION_FAILED : JIPM_ST_TINY_STEP;
@@ -615,28 +657,63 @@ __device__ void Solver<C>::iterate() {
             f = o->rho_resto * f_pn + 0.5 * zeta * f_q;
         }
     }
-    rec[11] = nmu; rec[13] = mu; rec[14] = theta;
-    // right-hand side of (6) (it does not depend on the perturbations)
-    for (int i = lane; i < nX; i += NT) {
-        const double l = lo(i), u = hi(i);
-        const bool hl = l > -INFINITY, hu = u < INFINITY;
-        double dmp = 0.0;
-        if (hl && !hu) dmp = o->kappa_d * mu;
-        if (hu && !hl) dmp = -o->kappa_d * mu;
-        b1[i] = -(b1[i] + dmp);
-        b3[i] = hl ? mu - (x[i] - l) * zL[i] : 0.0;
-        b4[i] = hu ? mu - (u - x[i]) * zU[i] : 0.0;
-    }
+    rec[11] = nmu; rec[14] = theta;
     for (int i = lane; i < m; i += NT) b2[i] = -cv[i];
     c.tm.sync();
     // A-4 search direction with inertia correction (Algorithm IC); a solve whose refinement on (6) fails
     // sends the matrix back to Algorithm IC as if it were singular (reading S-7)
     int nfact = 0, npsing = 0, nref = 0;
     double dw = 0.0, dc = 0.0;
-    bool resume = false;
+    bool resume = false, rhs_built = false;
     c.tick(15, clock64() - t_hd);
     while (true) {
-        if (!ic_loop(resume, dw, dc, nfact)) { enter_restoration(rec, KIND_IC_FAIL); trace_put(rec); return; }
+        if (!ic_loop(resume, dw, dc, nfact)) { rec[13] = mu; enter_restoration(rec, KIND_IC_FAIL); trace_put(rec); return; }
+        if (!rhs_built) {
+            if (adaptive && mu_free) {
+                // Mehrotra's probing with the factorisation of this iteration (it does not depend on mu): affine-scaling
+                // step = Newton step on (5) with mu = 0 (into the correction's vectors, free at this point); mu_aff =
+                // average complementarity after the largest feasible step; sigma = (mu_aff / average)^3; mu = sigma avg
+                Vec a1 = VX(L->ab1); Vec a3 = VX(L->ab3); Vec a4 = VX(L->ab4);
+                Vec sx = VX(L->sx); double* sy = V(L->sy); Vec szL = VX(L->szL); Vec szU = VX(L->szU);
+                for (int i = lane; i < nX; i += NT) {
+                    const double l = lo(i), u = hi(i);
+                    a1[i] = -b1[i];
+                    a3[i] = (l > -INFINITY) ? -(x[i] - l) * zL[i] : 0.0;
+                    a4[i] = (u < INFINITY) ? -(u - x[i]) * zU[i] : 0.0;
+                }
+                c.tm.sync();
+                bool failed_aff;
+                solve_full(a1, b2, a3, a4, sx, sy, szL, szU, failed_aff);
+                const double a_p = ftb_primal(x, sx, 1.0);
+                const double a_d = ftb_dual(zL, zU, szL, szU, 1.0);
+                double sa = 0.0;
+                for (int i = lane; i < nX; i += NT) {
+                    const double l = lo(i), u = hi(i);
+                    if (l > -INFINITY) sa += ((x[i] - l) + a_p * sx[i]) * (zL[i] + a_d * szL[i]);
+                    if (u < INFINITY) sa += ((u - x[i]) - a_p * sx[i]) * (zU[i] + a_d * szU[i]);
+                }
+                const double mu_aff = c.tm.sum(sa) / ncomp;
+                const double r = mu_aff / avg;
+                const double sigma = (avg > 0.0) ? fmin(o->adaptive_sigma_max, r * r * r) : 1.0;
+                mu = fmin(mu_max, fmax(mu_min, sigma * avg));
+                tau = fmax(o->tau_min, 1.0 - mu);
+                nfilt = 0;
+                wd_active = 0; wd_trials = 0; n_short = 0; soft = 0; soft_count = 0;
+            }
+            // right-hand side of (6) (it does not depend on the perturbations)
+            for (int i = lane; i < nX; i += NT) {
+                const double l = lo(i), u = hi(i);
+                const bool hl = l > -INFINITY, hu = u < INFINITY;
+                double dmp = 0.0;
+                if (hl && !hu) dmp = o->kappa_d * mu;
+                if (hu && !hl) dmp = -o->kappa_d * mu;
+                b1[i] = -(b1[i] + dmp);
+                b3[i] = hl ? mu - (x[i] - l) * zL[i] : 0.0;
+                b4[i] = hu ? mu - (u - x[i]) * zU[i] : 0.0;
+            }
+            c.tm.sync();
+            rhs_built = true;
+        }
         bool failed;
         const long long t_sf = clock64();
         nref = solve_full(b1, b2, b3, b4, dx, dy, dzL, dzU, failed);
@@ -645,6 +722,7 @@ __device__ void Solver<C>::iterate() {
         npsing++;
         resume = true;
     }
+    rec[13] = mu;
     rec[1] = nfact; rec[2] = dw; rec[3] = dc; rec[4] = nref; rec[19] = npsing;
     if (dw > 0.0) dw_last = dw;
     // A-5 line search

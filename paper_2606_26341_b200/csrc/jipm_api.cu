@@ -79,6 +79,8 @@ extern "C" int jipm_default_options(jipm_options* o) {
     o->tiny_step_tol = 10.0 * 2.220446049250313e-16; o->tiny_step_y_tol = 1e-2; o->tiny_step_cviol = 1e-4;
     o->soft_resto_factor = 1.0 - 1e-4;
     o->watchdog_trigger = 10; o->watchdog_trial_max = 3; o->max_soft_resto_iters = 10; o->polish_max = 3;
+    o->mu_strategy = 0; o->adaptive_red_iters = 4; o->adaptive_red_fact = 0.9999; o->adaptive_monotone_init = 0.8;
+    o->adaptive_sigma_max = 100.0; o->adaptive_mu_max_fact = 1e3;
     return JIPM_OK;
 }
 
@@ -144,7 +146,7 @@ static int build_layout(jipm_solver* s, int sm_budget_doubles) {
     int Lay::*const primal[] = {
         &Lay::x, &Lay::rr, &Lay::dx, &Lay::Sig, &Lay::xt, &Lay::zL, &Lay::zU, &Lay::b1, &Lay::dzL, &Lay::dzU, &Lay::b3, &Lay::b4,
         &Lay::g, &Lay::Hd, &Lay::r1, &Lay::r3, &Lay::r4, &Lay::e1, &Lay::e3, &Lay::e4, &Lay::sx, &Lay::szL, &Lay::szU,
-        &Lay::wx, &Lay::wzL, &Lay::wzU, &Lay::wdx, &Lay::wdzL, &Lay::wdzU,
+        &Lay::wx, &Lay::wzL, &Lay::wzU, &Lay::wdx, &Lay::wdzL, &Lay::wdzU, &Lay::ab1, &Lay::ab3, &Lay::ab4,
     };
     const Ent cold[] = {
         {&Lay::rk, rkn}, {&Lay::sy, m}, {&Lay::csoc, m}, {&Lay::bs2, m}, {&Lay::rc2, m},

@@ -38,6 +38,8 @@ __device__ void Solver<C>::dbg_load(const double* st) {
     n_short = (int)st[D.ls + 0]; wd_active = (int)st[D.ls + 1]; wd_trials = (int)st[D.ls + 2];
     wd_theta = st[D.ls + 3]; wd_phi = st[D.ls + 4]; wd_gd = st[D.ls + 5]; wd_alpha = st[D.ls + 6];
     soft = (int)st[D.ls + 7]; soft_count = (int)st[D.ls + 8]; tiny_last = (int)st[D.ls + 9]; tiny_flag = (int)st[D.ls + 10];
+    mu_free = (int)st[D.ls + 11]; mu_max = st[D.ls + 12]; nhist = (int)st[D.ls + 13];
+    for (int q = 0; q < 4; ++q) hist[q] = st[D.ls + 14 + q];   // hist[j & 3] = j-th remembered KKT error
     if (wd_active) {
         const int nw = pb->n + 2 * pb->m;
         Vec w[6] = {VX(L->wx), VX(L->wzL), VX(L->wzU), VX(L->wdx), VX(L->wdzL), VX(L->wdzU)};
@@ -73,6 +75,8 @@ __device__ void Solver<C>::dbg_store(double* st) {
         st[D.ls + 0] = n_short; st[D.ls + 1] = wd_active; st[D.ls + 2] = wd_trials; st[D.ls + 3] = wd_theta;
         st[D.ls + 4] = wd_phi; st[D.ls + 5] = wd_gd; st[D.ls + 6] = wd_alpha; st[D.ls + 7] = soft;
         st[D.ls + 8] = soft_count; st[D.ls + 9] = tiny_last; st[D.ls + 10] = tiny_flag;
+        st[D.ls + 11] = mu_free; st[D.ls + 12] = mu_max; st[D.ls + 13] = nhist;
+        for (int q = 0; q < 4; ++q) st[D.ls + 14 + q] = hist[q];
     }
     if (wd_active) {
         const int nw = pb->n + 2 * pb->m;

@@ -14,7 +14,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libjipm.so")
 
-TRACE_W = 20
+TRACE_W = 22
 ST_NOT_RUN, ST_SOLVED, ST_MAXITER, ST_LOCALLY_INFEASIBLE = -1, 0, 1, 2
 ST_RESTORATION_FAILED, ST_RESTO_AT_FEASIBLE_POINT, ST_NONFINITE, ST_TINY_STEP = 3, 4, 5, 6
 
@@ -26,14 +26,16 @@ _DOUBLE_FIELDS = [
     "delta_w_min", "delta_w_0", "delta_w_max", "kappa_w_minus", "kappa_w_plus", "kappa_w_plus_first",
     "delta_c_bar", "kappa_c", "residual_ratio_max", "rho_resto", "kappa_resto", "z_reset_threshold",
     "residual_ratio_singular", "residual_improvement_factor",
-    "tiny_step_tol", "tiny_step_y_tol", "tiny_step_cviol", "soft_resto_factor"]
+    "tiny_step_tol", "tiny_step_y_tol", "tiny_step_cviol", "soft_resto_factor",
+    "adaptive_red_fact", "adaptive_monotone_init", "adaptive_sigma_max", "adaptive_mu_max_fact"]
 _INT_FIELDS = ["max_iter", "max_backtrack", "max_soc", "refine_min", "refine_max", "max_mu_updates",
-               "init_slacks", "enable_restoration", "watchdog_trigger", "watchdog_trial_max", "max_soft_resto_iters"]
+               "init_slacks", "enable_restoration", "watchdog_trigger", "watchdog_trial_max", "max_soft_resto_iters",
+               "mu_strategy", "adaptive_red_iters"]
+_INT_LAYOUT = _INT_FIELDS[:-2] + ["polish_max"] + _INT_FIELDS[-2:]   # order of the int32 members in jipm_options
 
 
 class Options(C.Structure):
-    _fields_ = ([(f, C.c_double) for f in _DOUBLE_FIELDS] + [(f, C.c_int32) for f in _INT_FIELDS]
-                + [("polish_max", C.c_int32)])
+    _fields_ = [(f, C.c_double) for f in _DOUBLE_FIELDS] + [(f, C.c_int32) for f in _INT_LAYOUT]
 
 
 class FamilyDims(C.Structure):

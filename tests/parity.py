@@ -15,7 +15,7 @@ from oracle import ipm as oipm
 KIND_CODE = {"newton": 0, "soc": 1, "ls_fail": 2, "ic_fail": 3, "": 4, "tiny": 5, "soft": 6}
 # GPU trace record columns (include/jipm.h)
 T_MODE, T_NFACT, T_DW, T_DC, T_NREF, T_KIND, T_LS, T_SOC, T_ALPHA, T_ALPHAZ, T_FTYPE, T_NMU, T_E0, T_MU = range(14)
-T_THETA, T_PHI, T_WD, T_SOFT, T_TINY, T_NPSING = 14, 15, 16, 17, 18, 19
+T_THETA, T_PHI, T_WD, T_SOFT, T_TINY, T_NPSING, T_MUMODE, T_MUSWITCH = 14, 15, 16, 17, 18, 19, 20, 21
 
 
 def oracle_for(d, xL, xU, opts=None):
@@ -58,6 +58,9 @@ def decisions_equal(gpu_rec: np.ndarray, otr: dict) -> tuple[bool, str]:
         return True, ""
     if int(gpu_rec[T_NMU]) != otr["nmu"]:
         return False, f"nmu {int(gpu_rec[T_NMU])} vs {otr['nmu']}"
+    for col, key in ((T_MUMODE, "mu_mode"), (T_MUSWITCH, "mu_switch")):
+        if int(gpu_rec[col]) != int(otr.get(key, 0)):
+            return False, f"{key} {int(gpu_rec[col])} vs {otr.get(key, 0)}"
     if kind == 3:
         return True, ""
     if int(gpu_rec[T_NFACT]) != otr["nfact"]:
@@ -171,17 +174,55 @@ def sensitivity_gap(solver, tr, rel=1e-12, seed=1):
     return iterate_gap(solver, lin, d)
 
 
+def residual_rounding_gap(solver, tr, ulps=4.0, seed=2):
+    """How far the step moves when the right-hand side of (6) carries the rounding error ANY fp64 evaluation leaves in
+    it: the constraint residual c(x) is a difference of numbers of size |A| |x| and the dual residual grad f + A^T y - z_L
+    + z_U a sum of terms of size |A|^T |y| + z_L + z_U, so each component is known to a few ulps of those magnitudes, not of
+    its own (the standard componentwise model, `ulps` = 4).  Same matrix, same solver, right-hand side perturbed by
+    ulps eps u (|A| |x| + |c|) and ulps eps u (|A|^T |y| + z_L + z_U + |b_1|), u ~ U(-1, 1); measured like
+    second_opinion_gap.  Matters when the primal iterate has converged to rounding level (theta = 2e-13) while delta_w
+    is 1e12 ... 1e16: dy = delta_w (A A^T)^-1 c + ... then IS the rounding noise of c times delta_w (seen with the adaptive
+    barrier strategy on the reduced workload-3 problem 2, iterations 178-187: the two codes evaluate theta = 2.39e-13 and
+    2.82e-13 at the same point and the multiplier steps differ by 1e3)."""
+    from oracle.linsolve import DenseLDL
+    lin = tr.get("lin")
+    if lin is None:
+        return 0.0
+    rng = np.random.default_rng(seed)
+    eps = 2.220446049250313e-16
+    A, b = lin["A"], lin["b"]
+    s1 = np.abs(A).T @ np.abs(lin["y"]) + lin["zL"] + lin["zU"] + np.abs(b[0]) if solver.m else lin["zL"] + lin["zU"] + np.abs(b[0])
+    bp = [b[0] + ulps * eps * s1 * rng.uniform(-1.0, 1.0, b[0].shape)]
+    if solver.m:
+        s2 = np.abs(A) @ np.abs(lin["x"]) + np.abs(b[1])
+        bp.append(b[1] + ulps * eps * s2 * rng.uniform(-1.0, 1.0, b[1].shape))
+    else:
+        bp.append(b[1])
+    bp += [b[2], b[3]]
+    K = solver.kkt_matrix(lin["W"], lin["Sigma"], A, tr["dw"], tr["dc"])
+    if not np.all(np.isfinite(K)):
+        return np.inf
+    try:
+        d, _, _ = solver.solve_full(DenseLDL(K), lin["W"], A, lin["x"], lin["zL"], lin["zU"], tr["dw"], tr["dc"], bp)
+    except Exception:
+        return np.inf
+    return iterate_gap(solver, lin, d)
+
+
 def step_is_well_posed(solver, tr, tol):
     """(well-posed?, text): the criteria above with the parity tolerance, plus the rounding floor of the step itself:
     e_v (eq 8) is a COMPONENTWISE measure, and a solver that is backward stable in the usual normwise sense delivers every
-    component of (dx, dy) to within a few ulps of the LARGEST component.  When 8 eps alpha_max max(||dx||, ||dy||)_inf
-    already exceeds the tolerance, the small components of the next iterate cannot be asked to 1e-8 (seen on restoration
-    steps with delta_w 1e9: ||dy||_inf = 5e8, differences of 2e-6 on multipliers of size 200, i.e. 4e-14 of ||dy||)."""
+    component of the step to within a few ulps of the LARGEST component of (dx, dy, dz_L, dz_U) -- the refinement of
+    reading S-7 stops on the common max-norm of the four blocks.  When 8 eps alpha_max ||step||_inf already exceeds the
+    tolerance, the small components of the next iterate cannot be asked to 1e-8 (seen on restoration steps with delta_w
+    1e9: ||dy||_inf = 5e8, differences of 2e-6 on multipliers of size 200, i.e. 4e-14 of ||dy||; and on steps with an
+    active slack, Sigma = 1e10: dz = 1e10, the multiplier of the inequality is a difference of nearly equal numbers
+    times 1e10)."""
     lin = tr.get("lin")
     if lin is not None:
         a_ref = solver.ftb_primal(lin["x"], lin["d"][0], lin["tau"])
-        big = max(float(np.max(np.abs(lin["d"][0]))), float(np.max(np.abs(lin["d"][1]))) if solver.m else 0.0)
-        floor = 8.0 * 2.220446049250313e-16 * a_ref * big
+        big = max(float(np.max(np.abs(v))) if v.size else 0.0 for v in lin["d"])   # all four blocks: the refinement of
+        floor = 8.0 * 2.220446049250313e-16 * a_ref * big                          # reading S-7 stops on their common norm
         if not np.isfinite(floor) or floor > tol:
             return False, f"8 eps alpha_max ||step||_inf = {floor:.1e}"
     g1 = second_opinion_gap(solver, tr)
@@ -190,9 +231,12 @@ def step_is_well_posed(solver, tr, tol):
     g2 = sensitivity_gap(solver, tr)
     if g2 > tol:
         return False, f"rounding-level perturbation of W, A moves the step by {g2:.1e}"
+    g3 = residual_rounding_gap(solver, tr)
+    if g3 > tol:
+        return False, f"rounding of the residuals c, grad L (4 ulps of their terms) moves the step by {g3:.1e}"
     if len((tr.get("lin") or {}).get("tried", [])) > 1 and not inertia_is_stable(solver, tr):
         return False, "inertia changes under a rounding-level perturbation of W, A"
-    return True, f"{max(g1, g2):.1e}"
+    return True, f"{max(g1, g2, g3):.1e}"
 
 
 class WithGpuDerivatives:
@@ -363,6 +407,10 @@ def snapshot_state(lay, st, n, m):
     snap[lay["ls"]:lay["ls"] + 11] = [cur.n_short, int(wd is not None), wd.trials if wd else 0, wd.theta if wd else 0.0,
                                       wd.phi if wd else 0.0, wd.gd if wd else 0.0, wd.alpha if wd else 0.0,
                                       int(cur.soft), cur.soft_count, int(cur.tiny_last), int(cur.tiny_flag)]
+    hist = list(cur.kkt_hist)
+    snap[lay["ls"] + 11:lay["ls"] + 14] = [int(cur.mu_free), cur.mu_max, len(hist)]
+    for j in range(max(0, len(hist) - 4), len(hist)):
+        snap[lay["ls"] + 14 + (j & 3)] = hist[j]
     if wd is not None:
         nw, o = n + 2 * m, lay["wd"]
         for q, v in enumerate((wd.x, wd.zL, wd.zU, wd.d[0], wd.d[2], wd.d[3])):

@@ -119,12 +119,13 @@ def check_batch(cfg, P, dims_kw, max_rec=400, gopts=None, need_identical=None):
         otr = []
         st = osol.solve(x0[i], theta[i], otr)
         for t in otr:
-            for key in ("wd", "soft", "tiny", "npsing"):
+            for key in ("wd", "soft", "tiny", "npsing", "mu_mode", "mu_switch"):
                 if t.get(key):
                     seen[key] = seen.get(key, 0) + 1
             if t.get("mode") == 1:
                 seen["resto"] = seen.get("resto", 0) + 1
             t.pop("lin", None)
+            t.pop("aff_step", None)
         ok, it, why = par.compare_problem(g["trace"][i], int(g["status"][i]), int(g["iters"][i]), st, otr)
         same += int(ok)
         if ok and st.status == 0:
@@ -177,6 +178,8 @@ FORCED = {
     "tiny": dict(tiny_step_tol=1e-4, tol=1e-12),
     "soft_off": dict(soft_resto_factor=0.0, watchdog_trigger=0),
     "pretend_singular": dict(residual_ratio_max=1e-300, residual_ratio_singular=1e-300, refine_max=2),
+    "adaptive_mu": dict(mu_strategy=1),
+    "adaptive_mu_quadrotor": dict(mu_strategy=1),
 }
 
 
@@ -186,17 +189,21 @@ def test_forced_fallback_branches_match_the_oracle(name):
     same on both sides) make every C0 problem take the branch, and the whole trajectories must still be identical:
     watchdog after ONE shortened step; a tiny-step threshold of 1e-4 with tol 1e-12 (tiny steps, the forced barrier
     decrease and the TINY_STEP status); soft restoration and watchdog switched off (the round-1 path); a refinement
-    target nobody can meet (every solve fails: delta_w climbs the whole ladder, restoration, RESTORATION_FAILED)."""
+    target nobody can meet (every solve fails: delta_w climbs the whole ladder, restoration, RESTORATION_FAILED); the
+    adaptive barrier parameter of Table I row 7 (Mehrotra probing, switch to the monotone schedule and back)."""
     from paper_2606_26341_b200 import jipm
     o = jipm.default_options()
     for k, v in FORCED[name].items():
         setattr(o, k, v)
     if name == "watchdog":   # C0 hardly ever backtracks: the reduced quadrotor family does (all four watchdog codes occur)
         frac, report, seen = check_batch(1, 12, REDUCED[1], gopts=o)
+    elif name == "adaptive_mu_quadrotor":   # Table I row 7 on the reduced quadrotor family: probing every iteration
+        frac, report, seen = check_batch(1, 12, REDUCED[1], gopts=o)
     else:
         P = 48 if name != "pretend_singular" else 6
         frac, report, seen = check_batch(0, P, {}, gopts=o, need_identical=DECISION_FRACTION)
-    want = {"watchdog": "wd", "tiny": "tiny", "pretend_singular": "npsing"}.get(name)
+    want = {"watchdog": "wd", "tiny": "tiny", "pretend_singular": "npsing", "adaptive_mu": "mu_mode",
+            "adaptive_mu_quadrotor": "mu_mode"}.get(name)
     if want:
         assert seen.get(want, 0) > 0, seen
 
@@ -312,9 +319,11 @@ def test_full_size_c2_c3_first_iterations(cfg):
     s.close()
 
 
-@pytest.mark.parametrize("cfg,P,kw", [(0, 48, {}), (1, 10, {}), (2, 6, dict(horizon_N=5, n_agents=2)),
-                                      (3, 4, dict(horizon_N=6, n_obstacles=5)), (5, 8, dict(horizon_N=8))])
-def test_per_iteration_decisions_from_oracle_states(cfg, P, kw):
+@pytest.mark.parametrize("cfg,P,kw,opt", [(0, 48, {}, {}), (1, 10, {}, {}), (2, 6, dict(horizon_N=5, n_agents=2), {}),
+                                          (3, 4, dict(horizon_N=6, n_obstacles=5), {}), (5, 8, dict(horizon_N=8), {}),
+                                          (1, 12, dict(horizon_N=7), dict(mu_strategy=1)),
+                                          (3, 4, dict(horizon_N=6, n_obstacles=5), dict(mu_strategy=1))])
+def test_per_iteration_decisions_from_oracle_states(cfg, P, kw, opt):
     """The paper's own correctness method: save the full state at every iteration of the
     reference run, load it, step ONCE, compare.  Every iteration of every problem -- regular AND restoration mode,
     watchdog / soft-restoration memory included, hard long-running instances included -- is replayed on the GPU from
@@ -326,19 +335,28 @@ def test_per_iteration_decisions_from_oracle_states(cfg, P, kw):
     partial pivoting, same refinement -- disagree by more than 1e-8 in the resulting iterate, or (b) the rounding error
     another fp64 derivative code leaves in W, A (a relative 1e-12 on every entry of A and on every multiplier-weighted
     term of W: a hundredth of what test_derivative_blocks_against_oracle tolerates) moves the resulting iterate by more
-    than 1e-8, or (c) an inertia read by Algorithm IC changes under that perturbation.  None of the three looks at the
-    GPU's result.  A step with identical decisions whose iterate still differs by more than 1e-8 gets one more
+    than 1e-8, or (c) an inertia read by Algorithm IC changes under that perturbation, or (d) the normwise rounding floor
+    8 eps alpha_max ||(dx, dy, dz_L, dz_U)||_inf of the step already exceeds 1e-8, or (e) the rounding any fp64 code leaves
+    in the residuals c(x) and grad L (4 ulps of the terms they are summed from) moves the resulting iterate by more than
+    1e-8 (a converged primal iterate under delta_w = 1e12 ... 1e16: dy is delta_w times the rounding noise of c).  None of
+    the five looks at the GPU's result.  A step with identical decisions whose iterate still differs by more than 1e-8 gets one more
     comparison: the oracle's iteration is re-run from the same state on the derivative blocks J_k, W_k the GPU evaluated
     (parity.WithGpuDerivatives; the blocks themselves are held to 1e-11 / 1e-10 by
     test_derivative_blocks_against_oracle) -- agreement to 1e-8 then shows that linear algebra and line search are the
     oracle's and only the rounding of the two derivative codes, amplified by the conditioning of (7), separates them;
     such steps are counted as identical and their number is printed."""
     import torch
+    from paper_2606_26341_b200 import jipm
     d = wl.config_dims(cfg, **kw)
     d, theta, x0 = wl.generate(cfg, P, d)
-    s, xL, xU = make_solver(d)
+    gopts = None
+    if opt:
+        gopts = jipm.default_options()
+        for k_, v_ in opt.items():
+            setattr(gopts, k_, v_)
+    s, xL, xU = make_solver(d, opts=gopts)
     lay = s.state_layout()
-    prob, osol = par.oracle_for(d, xL, xU)
+    prob, osol = par.oracle_for(d, xL, xU, oracle_options(gopts))
     n, m = d.n, d.m
     rows, refs = [], []
 
@@ -360,6 +378,7 @@ def test_per_iteration_decisions_from_oracle_states(cfg, P, kw):
             well, wtext = par.step_is_well_posed(act, tr, STEP_PARITY_TOL)
             gap = (0.0 if well else np.inf, wtext)
             tr.pop("lin", None)
+            tr.pop("aff_step", None)
             moved = tr["kind"] in ("newton", "soc", "tiny", "soft") and st.status == -1
             nxt = next_iterate(st) if moved else None
             mem = par.ls_memory(st) if moved and not tr.get("exit_resto") and not tr.get("enter_resto") else None
@@ -413,7 +432,7 @@ def test_per_iteration_decisions_from_oracle_states(cfg, P, kw):
                 got = [int(got[q]) for q in (0, 1, 2, 7, 8, 9, 10)]
                 if got != mem:
                     ok, why = False, f"line-search memory {got} vs {mem}"
-        for key in ("wd", "soft", "tiny", "npsing"):
+        for key in ("wd", "soft", "tiny", "npsing", "mu_mode", "mu_switch"):
             if otr.get(key):
                 seen[key] = seen.get(key, 0) + 1
         if otr["kind"] in ("newton", "soc"):
