@@ -237,9 +237,13 @@ def run_jipm(args):
     d, theta, x0 = wl.generate(cfg, P, first_id=shard_first_id(rank, P))  # queue sharded by rank
     xL, xU = wl.bounds(d)
     opts = None
-    if args.max_iter > 0:
+    if args.max_iter > 0 or args.opt:
         opts = jipm.default_options()
-        opts.max_iter = args.max_iter
+        if args.max_iter > 0:
+            opts.max_iter = args.max_iter
+        for kv in args.opt:   # option sweeps: not the bench configuration
+            key, val = kv.split("=", 1)
+            setattr(opts, key, type(getattr(opts, key))(float(val)))
     s = jipm.Solver(d.family, d.horizon_N, d.n_agents, d.n_obstacles, d.dt, xL, xU, opts, resident_slots=args.slots)
     dev = torch.device("cuda", local)
     x0_d = torch.as_tensor(x0, device=dev)
@@ -336,6 +340,7 @@ def run_jipm(args):
                        "resident_slots": s.stats()["slots"], "l2": "flushed between timed steps (256 MiB fill)",
                        **({"max_iter_cap": args.max_iter, "note": "profiling run, not a bench value"}
                           if args.max_iter > 0 else {}),
+                       **({"option_overrides": list(args.opt), "note": "option sweep, not a bench value"} if args.opt else {}),
                        "parallelism": f"queue sharded over {world} GPU(s), no collective"},
             "iterations_per_s": iters_all * K / secs,
             "slot_us_per_iteration": us_per_iter,
@@ -451,6 +456,8 @@ def main():
     ap.add_argument("--slots", type=int, default=0, help="resident slots (0: library picks)")
     ap.add_argument("--impl", default="jipm", choices=["jipm", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
+                    help="override one solver option (repeatable), e.g. --opt watchdog_trigger=0: option sweeps only")
     ap.add_argument("--max-iter", type=int, default=0,
                     help="cap IPM iterations per problem (profiling runs only: keeps the kernel short under ncu; "
                          "a line produced with this flag says so in config and is not a bench value)")
