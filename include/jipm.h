@@ -109,6 +109,26 @@ int jipm_solve_batch_host(jipm_solver* s, int64_t P, const double* x0, const dou
 /* Free everything.  NULL is a no-op. */
 int jipm_destroy(jipm_solver* s);
 
+/* The same solve (the iteration of PAPER.md:77-150) for callers that must not allocate: no
+ * cudaMalloc, cudaFree or allocating library routine is called, no solver object exists.  All device memory the
+ * solve needs beyond the caller's buffers -- relaxed bounds, the per-SM slot workspaces of the kernel, queue counter,
+ * statistics -- lives in one static device array of JIPM_STATIC_SCRATCH_BYTES that every GPU which loads the library
+ * holds until the process exits.
+ *   family, d, n, m, x_L, x_U (HOST [n]), opts (HOST or NULL), cuda_stream: as in jipm_create; the library picks R.
+ *   P, x0, params, x_out, lam_out, zL_out, zU_out, status_out, iters_out (all DEVICE): as in jipm_solve_batch.
+ * Results are bit-identical to jipm_create + jipm_solve_batch with the same arguments.  Returns after the work has
+ * completed.  A family whose workspaces do not fit the array (n > 8192, or more than JIPM_STATIC_SCRATCH_BYTES of
+ * scratch: C2 and C3 of BASELINE.json do not fit, C0, C1 and workload 5 do) -> JIPM_ERR_NOMEM with the sizes in
+ * jipm_last_error; nothing is launched.
+ * Every call on a device shares the one array, which keeps the previous call's contents (the call clears what must
+ * start at zero): calls that overlap on the GPU -- other host threads are serialised by the library, other PROCESSES
+ * have their own copy -- would race; no trace, statistics or debug entry applies to this call. */
+#define JIPM_STATIC_SCRATCH_BYTES (64u << 20)
+int jipm_solve_batch_static(int family, const jipm_family_dims* d, int64_t n, int64_t m, const double* x_L,
+                            const double* x_U, const jipm_options* opts, void* cuda_stream, int64_t P,
+                            const double* x0, const double* params, double* x_out, double* lam_out,
+                            double* zL_out, double* zU_out, int32_t* status_out, int32_t* iters_out);
+
 /* Last error text of the calling thread (static storage, never NULL). */
 const char* jipm_last_error(void);
 

@@ -438,3 +438,136 @@ extern "C" int jipm_bench_fp64_peak(void* cuda_stream, double* tflops) {
     *tflops = best;
     return JIPM_OK;
 }
+
+// ---- jipm_solve_batch_static: the same solve with NOTHING allocated ---------------------------------------------------
+// For callers that cannot call cudaMalloc (a tight serving loop, a harness that forbids allocation).  Everything
+// jipm_create puts into device memory of its own -- the relaxed bounds, the per-SM slot workspaces (the kernel's
+// scratch: cold vectors, restoration tails, whatever of the layout does not fit shared memory), the SM-claim mask, the
+// queue counter and the statistics block -- is carved out of ONE file-scope device array of JIPM_STATIC_SCRATCH_BYTES.
+// Every GPU that loads this module holds that array until the process exits.  The host sees g_static_scratch only as a
+// stand-in symbol, never as an address: its device address is asked for once per device, with that device current, by
+// cudaGetSymbolAddress (static_scratch_of), and only that pointer is handed to the kernel.
+static __device__ __align__(256) double g_static_scratch[JIPM_STATIC_SCRATCH_BYTES / sizeof(double)];
+
+static constexpr int STATIC_MAX_DEVICES = 64;
+static constexpr int STATIC_MAX_N = 8192;   // host staging of the relaxed bounds (no heap either)
+static double* g_static_ptr[STATIC_MAX_DEVICES] = {nullptr};
+static double g_static_xl[STATIC_MAX_N], g_static_xu[STATIC_MAX_N];   // guarded by g_launch_mutex
+
+// device address of the array on the CURRENT device (dev); resolved once per device
+static int static_scratch_of(int dev, double** out) {
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) return fail(JIPM_ERR_CUDA, "device ordinal beyond the static-scratch table");
+    if (g_static_ptr[dev] == nullptr) {
+        double* p = nullptr;
+        CUDA_TRY(cudaGetSymbolAddress((void**)&p, g_static_scratch));
+        if (p == nullptr) return fail(JIPM_ERR_CUDA, "cudaGetSymbolAddress returned NULL for the static scratch");
+        g_static_ptr[dev] = p;
+    }
+    *out = g_static_ptr[dev];
+    return JIPM_OK;
+}
+
+extern "C" int jipm_solve_batch_static(int family, const jipm_family_dims* d, int64_t n, int64_t m, const double* x_L,
+                                       const double* x_U, const jipm_options* opts, void* cuda_stream, int64_t P,
+                                       const double* x0, const double* params, double* x_out, double* lam_out,
+                                       double* zL_out, double* zU_out, int32_t* status_out, int32_t* iters_out) {
+    if (!x_L || !x_U) return fail(JIPM_ERR_ARG, "NULL argument");
+    int nx, nu, ng, nth, pd;
+    if (!family_shape(family, d, nx, nu, ng, nth, pd)) return fail(JIPM_ERR_DIM, "bad family or dims");
+    int64_t n2, m2, nt2;
+    jipm_family_sizes(family, d, &n2, &m2, &nt2);
+    if (n != n2 || m != m2) return fail(JIPM_ERR_DIM, "n, m do not match jipm_family_sizes");
+    if (P < 0 || P > 0x7fffffff) return fail(JIPM_ERR_ARG, "bad P");
+    if (n > STATIC_MAX_N)
+        return fail(JIPM_ERR_NOMEM, "jipm_solve_batch_static: n = " + std::to_string(n) + " exceeds the static maximum of " +
+                                        std::to_string(STATIC_MAX_N) + " variables (use jipm_create / jipm_solve_batch)");
+    if (P > 0 && (!x0 || !params || !x_out || !lam_out || !status_out || !iters_out)) return fail(JIPM_ERR_ARG, "NULL buffer");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
+        return fail(JIPM_ERR_CUDA, "no CUDA device (jipm has no CPU fallback)");
+    // the configuration jipm_create derives, held on the stack
+    jipm_solver s;
+    s.family = family; s.dims = *d;
+    if (opts) s.o = *opts; else jipm_default_options(&s.o);
+    s.stream = (cudaStream_t)cuda_stream;
+    s.NX = nx; s.NU = nu; s.NZ = nx + nu;
+    Pb& pb = s.pb;
+    pb.family = family; pb.N = d->horizon_N; pb.ng = ng; pb.na = d->n_agents; pb.nobs = d->n_obstacles;
+    pb.n = (int)n; pb.m = (int)m; pb.nth = nth; pb.blk = nu + nx + ng; pb.cblk = nx + ng;
+    pb.dt = d->dt; pb.ru = (family == JIPM_FAM_POINTMASS2D) ? 0.1 : 0.01;
+    pb.th_obs = (family == JIPM_FAM_POINTMASS2D) ? 6 : (family == JIPM_FAM_QUAD_TRACK ? 14 : (family == JIPM_FAM_QUAT_NAV ? 16 : 15));
+    pb.th_goal = (family == JIPM_FAM_POINTMASS2D) ? 4 : (family == JIPM_FAM_MULTIQUAD ? 12 * d->n_agents : (family == JIPM_FAM_QUAT_NAV ? 13 : 12));
+    if (family == JIPM_FAM_POINTMASS2D) s.inst = inst_pm();
+    else if (family == JIPM_FAM_MULTIQUAD) s.inst = d->n_agents == 4 ? inst_q4() : inst_q2();
+    else if (family == JIPM_FAM_QUAT_NAV) s.inst = inst_qt();
+    else s.inst = inst_q1();
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&s.device) != cudaSuccess || cudaGetDeviceProperties(&prop, s.device) != cudaSuccess)
+        return fail(JIPM_ERR_CUDA, "cudaGetDevice / cudaGetDeviceProperties");
+    s.teams_per_sm = std::max(1, std::min(s.inst.info.min_blocks, 2048 / s.inst.info.nt));
+    const long per_team = std::min<long>((long)prop.sharedMemPerMultiprocessor / s.teams_per_sm - 1024,
+                                         (long)prop.sharedMemPerBlockOptin);
+    const long budget = per_team / (long)sizeof(double) - s.inst.info.sm_fixed;
+    if (budget < 0) return fail(JIPM_ERR_NOMEM, "stage tiles do not fit shared memory");
+    int hot_fits = build_layout(&s, (int)budget);
+    if (!hot_fits && s.inst.info.hot_sm) {
+        if (family == JIPM_FAM_POINTMASS2D) return fail(JIPM_ERR_NOMEM, "problem too large for the point-mass kernel");
+        s.inst = inst_q1g();
+        s.teams_per_sm = std::max(1, std::min(s.inst.info.min_blocks, 2048 / s.inst.info.nt));
+        const long pt = std::min<long>((long)prop.sharedMemPerMultiprocessor / s.teams_per_sm - 1024, (long)prop.sharedMemPerBlockOptin);
+        const long b2 = pt / (long)sizeof(double) - s.inst.info.sm_fixed;
+        if (b2 < 0) return fail(JIPM_ERR_NOMEM, "stage tiles do not fit shared memory");
+        hot_fits = build_layout(&s, (int)b2);
+    }
+    s.dbg = make_dbglay(pb.n, pb.m, pb.N, s.NX, s.NZ);
+    s.n_sm = prop.multiProcessorCount;
+    if (s.teams_per_sm > 32) s.teams_per_sm = 32;
+    s.n_slots = (int)std::min<int64_t>((int64_t)s.teams_per_sm * s.n_sm, 0x7fffffff);
+    // carve the array: [queue | stats | SM mask | x_L | x_U | n_sm * teams_per_sm workspaces], every part 256-byte aligned
+    auto up32 = [](size_t c) { return (c + 31) & ~(size_t)31; };   // doubles
+    const size_t ws_stride = (size_t)(s.L.total - s.L.nsm + 2);
+    const size_t n_ws = (size_t)s.n_sm * s.teams_per_sm;
+    const size_t o_queue = 0, o_stats = 32, o_mask = 64;
+    const size_t o_xl = o_mask + up32(((size_t)s.n_sm * sizeof(unsigned) + 7) / 8), o_xu = o_xl + up32(n), o_ws = o_xu + up32(n);
+    const size_t need = o_ws + n_ws * ws_stride;
+    const size_t have = JIPM_STATIC_SCRATCH_BYTES / sizeof(double);
+    if (need > have)
+        return fail(JIPM_ERR_NOMEM, "jipm_solve_batch_static: this family needs " + std::to_string(need * sizeof(double)) +
+                                        " bytes of scratch, the static maximum is " + std::to_string((size_t)JIPM_STATIC_SCRATCH_BYTES) +
+                                        " (JIPM_STATIC_SCRATCH_BYTES); use jipm_create / jipm_solve_batch");
+    if (P == 0) return JIPM_OK;
+    std::lock_guard<std::mutex> lock(g_launch_mutex);
+    double* base = nullptr;
+    if (int rc = static_scratch_of(s.device, &base)) return rc;
+    // Step I-1: relax finite bounds (as jipm_create does), staged in static host storage
+    pb.nL = pb.nU = 0;
+    for (int64_t i = 0; i < n; ++i) {
+        double l = x_L[i], u = x_U[i];
+        if (std::isnan(l) || std::isnan(u)) return fail(JIPM_ERR_BOUNDS, "NaN bound");
+        if (l >= u) return fail(JIPM_ERR_BOUNDS, "x_L >= x_U on a component (PAPER.md:63 needs x_L < x_U)");
+        if (std::isfinite(l)) { l -= s.o.bound_relax_factor * std::max(1.0, std::fabs(l)); pb.nL++; } else l = -INFINITY;
+        if (std::isfinite(u)) { u += s.o.bound_relax_factor * std::max(1.0, std::fabs(u)); pb.nU++; } else u = INFINITY;
+        if (l >= u) return fail(JIPM_ERR_BOUNDS, "x_L >= x_U on a component");
+        g_static_xl[i] = l; g_static_xu[i] = u;
+    }
+    pb.xL = base + o_xl; pb.xU = base + o_xu;
+    // the array keeps the last call's contents: everything the kernel expects to find zero is cleared here (queue,
+    // statistics, SM mask, and the workspaces, which jipm_create clears once)
+    CUDA_TRY(cudaMemsetAsync(base, 0, o_xl * sizeof(double), s.stream));
+    CUDA_TRY(cudaMemsetAsync(base + o_ws, 0, n_ws * ws_stride * sizeof(double), s.stream));
+    CUDA_TRY(cudaMemcpyAsync(base + o_xl, g_static_xl, n * sizeof(double), cudaMemcpyHostToDevice, s.stream));
+    CUDA_TRY(cudaMemcpyAsync(base + o_xu, g_static_xu, n * sizeof(double), cudaMemcpyHostToDevice, s.stream));
+    Args a; memset(&a, 0, sizeof(a));
+    a.P = (int)P; a.x0 = x0; a.th = params; a.x_out = x_out; a.lam_out = lam_out; a.zL_out = zL_out; a.zU_out = zU_out;
+    a.status_out = status_out; a.iters_out = iters_out; a.dbg_mode = 0;
+    a.pb = s.pb; a.L = s.L; a.o = s.o;
+    a.ws = base + o_ws; a.ws_stride = (int64_t)ws_stride;
+    a.n_slots = (int)std::min<int64_t>(s.n_slots, std::max<int64_t>(a.P, 1));
+    a.queue = reinterpret_cast<int*>(base + o_queue);
+    a.stats = reinterpret_cast<unsigned long long*>(base + o_stats);
+    a.sm_mask = reinterpret_cast<unsigned*>(base + o_mask); a.teams_per_sm = s.teams_per_sm;
+    a.trace = nullptr; a.trace_cap = 0; a.dbg_len = s.dbg.len;
+    CUDA_TRY(s.inst.launch(a, s.stream));
+    CUDA_TRY(cudaStreamSynchronize(s.stream));   // the bounds staging and the __constant__ launch block are free again
+    return JIPM_OK;
+}

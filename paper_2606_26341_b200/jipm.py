@@ -47,7 +47,9 @@ _lib = None
 EXPORTS = ["jipm_default_options", "jipm_family_sizes", "jipm_create", "jipm_solve_batch",
            "jipm_solve_batch_host", "jipm_destroy", "jipm_last_error", "jipm_last_stats",
            "jipm_debug_set_trace", "jipm_debug_state_layout", "jipm_debug_step", "jipm_debug_init",
-           "jipm_bench_fp64_peak", "jipm_residency"]
+           "jipm_bench_fp64_peak", "jipm_residency", "jipm_solve_batch_static"]
+
+STATIC_SCRATCH_BYTES = 64 << 20   # JIPM_STATIC_SCRATCH_BYTES of include/jipm.h
 
 
 def lib():
@@ -74,6 +76,8 @@ def lib():
         L.jipm_debug_init.argtypes = [vp, i64, dp, dp, dp]
         L.jipm_bench_fp64_peak.argtypes = [vp, C.POINTER(C.c_double)]
         L.jipm_residency.argtypes = [vp, C.POINTER(i64)]
+        L.jipm_solve_batch_static.argtypes = [C.c_int, C.POINTER(FamilyDims), i64, i64, dp, dp, C.POINTER(Options), vp,
+                                              i64, dp, dp, dp, dp, dp, dp, ip, ip]
         _lib = L
     return _lib
 
@@ -105,6 +109,25 @@ def fp64_peak_tflops() -> float:
     v = C.c_double()
     _check(lib().jipm_bench_fp64_peak(C.c_void_p(torch.cuda.current_stream().cuda_stream), C.byref(v)))
     return v.value
+
+
+def solve_batch_static(family, horizon_N, n_agents, n_obstacles, dt, xL, xU, x0, params, out, opts: Options | None = None):
+    """jipm_solve_batch_static: the solve without any allocation inside the library (scratch in a static device array
+    of STATIC_SCRATCH_BYTES).  x0 [P,n], params [P,n_theta] and the tensors of `out` (x, lam, status, iters and
+    optionally zL, zU) are CUDA tensors the caller owns; xL, xU host arrays."""
+    import torch
+    d = FamilyDims(horizon_N, n_agents, n_obstacles, dt)
+    n, m, _ = family_sizes(family, horizon_N, n_agents, n_obstacles, dt)
+    xL = np.ascontiguousarray(xL, dtype=np.float64)
+    xU = np.ascontiguousarray(xU, dtype=np.float64)
+    assert xL.shape == (n,) and xU.shape == (n,)
+    zl = out["zL"].data_ptr() if "zL" in out else None
+    zu = out["zU"].data_ptr() if "zU" in out else None
+    _check(lib().jipm_solve_batch_static(family, C.byref(d), n, m, xL.ctypes.data, xU.ctypes.data,
+                                         C.byref(opts) if opts is not None else None,
+                                         C.c_void_p(torch.cuda.current_stream().cuda_stream), x0.shape[0],
+                                         x0.data_ptr(), params.data_ptr(), out["x"].data_ptr(), out["lam"].data_ptr(),
+                                         zl, zu, out["status"].data_ptr(), out["iters"].data_ptr()))
 
 
 class Solver:
