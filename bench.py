@@ -372,7 +372,8 @@ def run_jipm(args):
             cnt_o, budget = oracle_sample(cfg, cores)
             dt, so, it, cut = time_oracle(cfg, 0, cnt_o, cores, budget)
             sample = (f"first {cnt_o} problems of the same workload, one process per problem, each cut after "
-                      f"{budget:.0f} s ({cut} cut)")
+                      f"{budget:.0f} s ({cut} cut); bounded to about {budget:.0f} s of wall-clock on {cores} cores "
+                      "(SURVEY 8(d)'s 512 / 64 problems would take minutes per line)")
             val = so / dt
             if so == 0 and solved_all > 0:
                 per_solved = iters_all / solved_all
