@@ -587,6 +587,52 @@ def test_repeated_runs_are_bit_identical(cfg):
             assert np.array_equal(res[k], ref[k], equal_nan=True), (cfg, R, k)
 
 
+def test_concurrent_solvers_of_one_family_are_serialised():
+    """Launch arguments live in one __constant__ block per family instantiation (inst.cuh): two solvers of the SAME
+    family with DIFFERENT options, driven from two host threads on two streams at once, must each get their own
+    arguments (the library serialises them, include/jipm.h jipm_create): results bit-identical to the serial runs."""
+    import threading
+    import torch
+    from paper_2606_26341_b200 import jipm
+    d, theta, x0 = wl.generate(0, 200)
+    xL, xU = wl.bounds(d)
+    opts = [jipm.default_options(), jipm.default_options()]
+    opts[1].max_iter = 7                      # the second solver must stop early; with the first one's arguments it would not
+    x0_d, th_d = torch.as_tensor(x0, device="cuda"), torch.as_tensor(theta, device="cuda")
+    serial = []
+    for o in opts:
+        s = jipm.Solver(d.family, d.horizon_N, d.n_agents, d.n_obstacles, d.dt, xL, xU, o)
+        serial.append({k: v.cpu().numpy() for k, v in s.solve_batch(x0_d, th_d).items()})
+        s.close()
+    assert serial[1]["iters"].max() == 7 and serial[0]["iters"].max() > 7
+    torch.cuda.synchronize()
+    results, errors = [None, None], []
+
+    def work(j):
+        try:
+            st = torch.cuda.Stream()
+            with torch.cuda.stream(st):
+                s = jipm.Solver(d.family, d.horizon_N, d.n_agents, d.n_obstacles, d.dt, xL, xU, opts[j])
+                out = None
+                for _ in range(20):               # many launches per thread: the two sequences interleave
+                    out = s.solve_batch(x0_d, th_d)
+                st.synchronize()
+                results[j] = {k: v.cpu().numpy() for k, v in out.items()}
+                s.close()
+        except Exception as e:                    # noqa: BLE001
+            errors.append((j, repr(e)))
+
+    threads = [threading.Thread(target=work, args=(j,)) for j in (0, 1)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors
+    for j in (0, 1):
+        for k in ("x", "lam", "zL", "zU", "status", "iters"):
+            assert np.array_equal(results[j][k], serial[j][k], equal_nan=True), (j, k)
+
+
 def test_host_entry_matches_device_entry_and_edge_cases():
     from paper_2606_26341_b200 import jipm
     d, theta, x0 = wl.generate(0, 37)
