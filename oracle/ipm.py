@@ -31,6 +31,7 @@ from .linsolve import DenseLDL
 
 ST_NOT_RUN, ST_SOLVED, ST_MAXITER, ST_LOCALLY_INFEASIBLE = -1, 0, 1, 2
 ST_RESTORATION_FAILED, ST_RESTO_AT_FEASIBLE_POINT, ST_NONFINITE, ST_TINY_STEP = 3, 4, 5, 6
+ST_ACCEPTABLE = 7
 EPS = 2.220446049250313e-16
 
 
@@ -101,6 +102,14 @@ class Options:
     adaptive_monotone_init: float = 0.8     # mu of the monotone phase = this x average complementarity
     adaptive_sigma_max: float = 100.0
     adaptive_mu_max_fact: float = 1e3       # mu never exceeds this x the first average complementarity
+    # acceptable-level termination (NEXT-4; IPOPT feature, not in the paper: reading AT, off by default): stop after
+    # acceptable_iter consecutive regular iterations whose E_0 <= acceptable_tol and whose unscaled dual residual,
+    # constraint violation and complementarity stay below the three bounds
+    acceptable_tol: float = 1e-6
+    acceptable_dual_inf_tol: float = 1e10
+    acceptable_constr_viol_tol: float = 1e-2
+    acceptable_compl_inf_tol: float = 1e-2
+    acceptable_iter: int = 0                # IPOPT's default is 15; 0 = off
 
     @property
     def mu_min(self) -> float:
@@ -131,6 +140,7 @@ class State:
     mu_free: bool = True              # adaptive strategy (Table I row 7): free mode (True) or monotone phase
     kkt_hist: list = field(default_factory=list)   # KKT errors of the last accepted free-mode iterates
     mu_max: float = -1.0              # upper bound of the adaptive mu (set at the first iteration)
+    acc_count: int = 0                # consecutive acceptable iterations (reading AT)
 
 
 @dataclass
@@ -209,6 +219,15 @@ class Solver:
         e_c = float(np.max(np.abs(cval))) if cval.size else 0.0
         e_s = float(np.max(np.abs(comp))) / sc if comp.size else 0.0
         return max(e_d, e_c, e_s)
+
+    def error_parts(self, x, y, zL, zU, g, cval, A):
+        """Unscaled max-norms of the three blocks of (5) at mu = 0: dual residual, constraint
+        violation, complementarity."""
+        sL, sU = self.slacks(x)
+        rd = g + A.T @ y - zL + zU
+        comp = np.concatenate([(sL * zL)[self.hasL], (sU * zU)[self.hasU]])
+        return (float(np.max(np.abs(rd))) if rd.size else 0.0, float(np.max(np.abs(cval))) if cval.size else 0.0,
+                float(np.max(np.abs(comp))) if comp.size else 0.0)
 
     # ---- fraction to the boundary (PAPER.md:148 fn 2; [7] eq 15) --------------------------------------
     def ftb_primal(self, x, dx, tau):
@@ -460,6 +479,15 @@ class Solver:
         if e0 <= o.tol:
             st.status = tr["status"] = ST_SOLVED
             return tr
+        if o.acceptable_iter > 0 and not hasattr(p, "set_mu"):   # reading AT; never inside the restoration sub-solver
+            d_inf, c_inf, s_inf = self.error_parts(x, y, st.zL, st.zU, g, cv, A)
+            ok = (e0 <= o.acceptable_tol and d_inf <= o.acceptable_dual_inf_tol and c_inf <= o.acceptable_constr_viol_tol
+                  and s_inf <= o.acceptable_compl_inf_tol)
+            st.acc_count = st.acc_count + 1 if ok else 0
+            tr["acc"] = st.acc_count
+            if st.acc_count >= o.acceptable_iter:
+                st.status = tr["status"] = ST_ACCEPTABLE
+                return tr
         if st.k >= o.max_iter:
             st.status = tr["status"] = ST_MAXITER
             return tr
@@ -769,6 +797,7 @@ class Solver:
         st.filt.append(((1.0 - o.gamma_theta) * theta_k, phi_k - o.gamma_phi * theta_k))
         # the regular problem's line-search memory does not survive a restoration phase
         st.wd, st.n_short, st.soft, st.soft_count, st.tiny_last, st.tiny_flag = None, 0, False, 0, False, False
+        st.acc_count = 0   # acceptable iterations must be consecutive REGULAR iterations
         mu_bar = max(st.mu, float(np.max(np.abs(cv))))
         rp = RestoNLP(self.p, st.x, o.rho_resto, mu_bar)
         n, m, rho = self.n, self.m, o.rho_resto

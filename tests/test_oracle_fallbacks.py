@@ -397,3 +397,63 @@ def test_adaptive_mu_solves_the_same_problems():
     st = ipm.Solver(p, l, u, ipm.Options(mu_strategy=1)).solve(np.zeros(5), None)
     assert st.status == ipm.ST_SOLVED
     np.testing.assert_allclose(st.x, np.clip(a, l, u), atol=2e-7)
+
+
+# ---- acceptable-level termination (NEXT-4, reading AT) --------------------------------------------------------
+def one_dim_barrier(**opt):
+    """min x s.t. x >= 0 from x0 = 0.5, z == 1 (test_oracle_ipm.py): x_k = the barrier parameter of iteration k-1, so
+    E_0 at the start of iterations 0..4 is the complementarity x_k z = 0.5, 0.02, 1.504241e-4, 1.844914e-6, 2.505904e-9
+    (tests/golden/mu_schedule.txt) and the dual residual 1 - z is 0."""
+    p = SmallNLP(1, 0, lambda x: x[0], lambda x: [1.0], lambda x: [[0.0]])
+    s = ipm.Solver(p, [0.0], [INF], ipm.Options(kappa_d=0.0, bound_relax_factor=0.0, **opt))
+    return s, s.initialise([0.5], None)
+
+
+def run(s, st):
+    acc = []
+    while st.status == ipm.ST_NOT_RUN:
+        acc.append(s.iterate(st, None).get("acc"))
+    return acc
+
+
+def test_acceptable_level_termination_counts_consecutive_iterations():
+    """acceptable_tol = 1e-3: E_0 = 1.5e-4 at iteration 2 is the first acceptable one, 1.8e-6 at iteration 3 the second:
+    with acceptable_iter = 2 the solve stops THERE (k = 3, status ACCEPTABLE) instead of SOLVED at k = 4; with
+    acceptable_iter = 3 the third acceptable iterate already meets tol = 1e-8 and SOLVED wins (it is tested first)."""
+    s, st = one_dim_barrier(acceptable_tol=1e-3, acceptable_iter=2)
+    assert run(s, st) == [0, 0, 1, 2] and st.status == ipm.ST_ACCEPTABLE and st.k == 3
+    assert st.x[0] == pytest.approx(1.844914e-6, rel=2e-6)
+    s, st = one_dim_barrier(acceptable_tol=1e-3, acceptable_iter=3)
+    assert run(s, st) == [0, 0, 1, 2, None] and st.status == ipm.ST_SOLVED and st.k == 4
+    # off by default: the pinned trajectory is untouched
+    s, st = one_dim_barrier()
+    assert run(s, st) == [None] * 5 and st.status == ipm.ST_SOLVED and st.k == 4
+
+
+def test_acceptable_level_needs_every_component_bound_and_resets():
+    """The complementarity bound is on the UNSCALED product: with acceptable_compl_inf_tol = 1e-5 iteration 2
+    (x z = 1.5e-4) is not acceptable although E_0 <= acceptable_tol, iteration 3 is the first, and the solve ends SOLVED.
+    A dual bound of 0 can never hold on a problem whose dual residual is not exactly 0 (x0 away from z = 1 is not needed:
+    here it IS exactly 0, so the bound 0 still passes -- the constraint bound is the one that fails below).  A counter
+    left over from earlier iterations is cleared by one iteration that is not acceptable."""
+    s, st = one_dim_barrier(acceptable_tol=1e-3, acceptable_iter=2, acceptable_compl_inf_tol=1e-5)
+    assert run(s, st) == [0, 0, 0, 1, None] and st.status == ipm.ST_SOLVED
+    s, st = one_dim_barrier(acceptable_tol=1e-3, acceptable_iter=2, acceptable_dual_inf_tol=0.0)
+    assert run(s, st) == [0, 0, 1, 2] and st.status == ipm.ST_ACCEPTABLE          # dual residual 1 - z == 0 exactly
+    s, st = one_dim_barrier(acceptable_tol=1e-3, acceptable_iter=50)
+    st.acc_count = 7
+    assert s.iterate(st, None)["acc"] == 0 and st.acc_count == 0                     # E_0 = 0.5 at iteration 0
+    # with an equality constraint the violation bound counts: c = x1 + x2 - 1 at a point with |c| = 0.2 > 1e-2
+    p = SmallNLP(2, 1, lambda x: 0.0, lambda x: np.zeros(2), lambda x: np.zeros((2, 2)),
+                 lambda x: [x[0] + x[1] - 1.0], lambda x: [[1.0, 1.0]], None)
+    s2 = ipm.Solver(p, [-INF, -INF], [INF, INF], ipm.Options(acceptable_tol=1.0, acceptable_iter=1))
+    x = np.array([0.5, 0.7])
+    assert s2.error_parts(x, np.array([3.0]), np.zeros(2), np.zeros(2), np.zeros(2), np.array([0.2]),
+                          np.array([[1.0, 1.0]])) == (3.0, 0.2, 0.0)
+    st2 = s2.initialise(x, None)
+    tr = s2.iterate(st2, None)
+    assert tr["E0"] <= 1.0 and tr["acc"] == 0 and st2.status == ipm.ST_NOT_RUN   # E_0 = 0.2 acceptable, |c| = 0.2 is not
+    s3 = ipm.Solver(p, [-INF, -INF], [INF, INF], ipm.Options(acceptable_tol=1.0, acceptable_iter=1, acceptable_constr_viol_tol=0.5))
+    st3 = s3.initialise(x, None)
+    s3.iterate(st3, None)
+    assert st3.status == ipm.ST_ACCEPTABLE and st3.k == 0
