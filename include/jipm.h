@@ -37,7 +37,8 @@ enum { JIPM_FAM_POINTMASS2D = 0, JIPM_FAM_QUAD_TRACK = 1, JIPM_FAM_MULTIQUAD = 2
        JIPM_FAM_QUAT_NAV = 4 /* the paper's own vehicle: 13-state quaternion quadrotor, rotor speeds */ };
 enum { JIPM_ST_NOT_RUN = -1, JIPM_ST_SOLVED = 0, JIPM_ST_MAXITER = 1, JIPM_ST_LOCALLY_INFEASIBLE = 2,
        JIPM_ST_RESTORATION_FAILED = 3, JIPM_ST_RESTO_AT_FEASIBLE_POINT = 4, JIPM_ST_NONFINITE = 5,
-       JIPM_ST_TINY_STEP = 6 /* search direction too small to make progress at the smallest mu (Table I row 4) */ };
+       JIPM_ST_TINY_STEP = 6 /* search direction too small to make progress at the smallest mu (Table I row 4) */,
+       JIPM_ST_ACCEPTABLE = 7 /* acceptable-level termination (reading AT, off by default): NOT counted as converged */ };
 
 /* Problem family dimensions (BASELINE.json configs). */
 typedef struct {
@@ -61,6 +62,8 @@ typedef struct {
     double tiny_step_tol, tiny_step_y_tol, tiny_step_cviol, soft_resto_factor;
     /* adaptive barrier parameter with the switch to the monotone schedule (Table I row 7) */
     double adaptive_red_fact, adaptive_monotone_init, adaptive_sigma_max, adaptive_mu_max_fact;
+    /* acceptable-level termination (NEXT-4; an IPOPT feature the paper does not describe: DESIGN.md reading AT) */
+    double acceptable_tol, acceptable_dual_inf_tol, acceptable_constr_viol_tol, acceptable_compl_inf_tol;
     int32_t max_iter, max_backtrack, max_soc, refine_min, refine_max, max_mu_updates;
     int32_t init_slacks, enable_restoration;
     int32_t watchdog_trigger, watchdog_trial_max, max_soft_resto_iters;
@@ -68,6 +71,7 @@ typedef struct {
                            is above 1e-15 and still shrinking: accuracy of the step only, no decision depends on it */
     int32_t mu_strategy;        /* 0 monotone schedule (default, IPOPT's), 1 adaptive (Mehrotra probing) with the switch */
     int32_t adaptive_red_iters; /* KKT errors remembered by the progress test of the adaptive mode */
+    int32_t acceptable_iter;    /* stop after this many consecutive acceptable regular iterations; 0 = off (default) */
 } jipm_options;
 
 /* Fill *o with the defaults.  o: HOST.  Returns JIPM_ERR_ARG if o is NULL. */

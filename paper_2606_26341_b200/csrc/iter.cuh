@@ -38,6 +38,7 @@ struct Solver {
     // the KKT errors of the last accepted free-mode iterates (regular problem only; restoration is always monotone)
     int mu_free, nhist;
     double mu_max, hist[4];
+    int acc_count;   // consecutive acceptable regular iterations (acceptable-level termination, reading AT)
     // restoration mode (Table I row 6): mode 1 iterates on X = [x; p; n] with the same kernel
     // code; the regular problem's scalars are parked in *_reg until the exit test succeeds
     int mode, nX, nfilt_reg;
@@ -60,7 +61,7 @@ struct Solver {
         reset_ls_memory();
     }
     __device__ __forceinline__ void reset_ls_memory() {
-        n_short = wd_active = wd_trials = soft = soft_count = tiny_last = tiny_flag = 0;
+        n_short = wd_active = wd_trials = soft = soft_count = tiny_last = tiny_flag = acc_count = 0;
         wd_theta = wd_phi = wd_gd = wd_alpha = 0.0;
     }
     __device__ __forceinline__ void reset_mu_memory() {
@@ -143,6 +144,20 @@ struct Solver {
         }
         ed = c.tm.max(ed); es = c.tm.max(es);
         return fmax(fmax(ed / sd, cmax), es / sc);
+    }
+
+    // unscaled max-norms of the dual residual and of the complementarity products at mu = 0 (b1 holds the dual residual);
+    // with cmax they are the three bounds of the acceptable-level test (reading AT)
+    __device__ __noinline__ void error_parts(double& ed, double& es) const {
+        Vec x = VX(L->x); Vec zL = VX(L->zL); Vec zU = VX(L->zU); Vec rdb = VX(L->b1);
+        double a = 0.0, b = 0.0;
+        for (int i = lane; i < nX; i += NT) {
+            const double l = lo(i), u = hi(i);
+            a = fmax(a, fabs(rdb[i]));
+            if (l > -INFINITY) b = fmax(b, fabs((x[i] - l) * zL[i]));
+            if (u < INFINITY) b = fmax(b, fabs((u - x[i]) * zU[i]));
+        }
+        ed = c.tm.max(a); es = c.tm.max(b);
     }
 
     // filter ([7] sec 2.3): entries (theta_j, phi_j) in the workspace

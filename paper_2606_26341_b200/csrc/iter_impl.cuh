@@ -582,6 +582,14 @@ __device__ void Solver<C>::iterate() {
         else status = JIPM_ST_SOLVED;
         rec[5] = KIND_TERMINAL; trace_put(rec); return;
     }
+    if (o->acceptable_iter > 0 && mode == 0) {   // acceptable-level termination (reading AT): regular problem only
+        double ed, es;
+        error_parts(ed, es);
+        const bool okacc = e0 <= o->acceptable_tol && ed <= o->acceptable_dual_inf_tol &&
+                           cmax <= o->acceptable_constr_viol_tol && es <= o->acceptable_compl_inf_tol;
+        acc_count = okacc ? acc_count + 1 : 0;
+        if (acc_count >= o->acceptable_iter) { status = JIPM_ST_ACCEPTABLE; rec[5] = KIND_TERMINAL; trace_put(rec); return; }
+    }
     if (k >= o->max_iter) { status = JIPM_ST_MAXITER; rec[5] = KIND_TERMINAL; trace_put(rec); return; }
     // A-3 monotone barrier update (Table I row 7).  Two tiny steps in a row (Table I row 4) force one
     // decrease; when mu cannot decrease any more the search direction has become too small to make progress.

@@ -81,6 +81,8 @@ extern "C" int jipm_default_options(jipm_options* o) {
     o->watchdog_trigger = 10; o->watchdog_trial_max = 3; o->max_soft_resto_iters = 10; o->polish_max = 3;
     o->mu_strategy = 0; o->adaptive_red_iters = 4; o->adaptive_red_fact = 0.9999; o->adaptive_monotone_init = 0.8;
     o->adaptive_sigma_max = 100.0; o->adaptive_mu_max_fact = 1e3;
+    o->acceptable_tol = 1e-6; o->acceptable_dual_inf_tol = 1e10; o->acceptable_constr_viol_tol = 1e-2;
+    o->acceptable_compl_inf_tol = 1e-2; o->acceptable_iter = 0;
     return JIPM_OK;
 }
 

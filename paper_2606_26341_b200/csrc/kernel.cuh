@@ -40,6 +40,7 @@ __device__ void Solver<C>::dbg_load(const double* st) {
     soft = (int)st[D.ls + 7]; soft_count = (int)st[D.ls + 8]; tiny_last = (int)st[D.ls + 9]; tiny_flag = (int)st[D.ls + 10];
     mu_free = (int)st[D.ls + 11]; mu_max = st[D.ls + 12]; nhist = (int)st[D.ls + 13];
     for (int q = 0; q < 4; ++q) hist[q] = st[D.ls + 14 + q];   // hist[j & 3] = j-th remembered KKT error
+    acc_count = (int)st[D.ls + 18];
     if (wd_active) {
         const int nw = pb->n + 2 * pb->m;
         Vec w[6] = {VX(L->wx), VX(L->wzL), VX(L->wzU), VX(L->wdx), VX(L->wdzL), VX(L->wdzU)};
@@ -77,6 +78,7 @@ __device__ void Solver<C>::dbg_store(double* st) {
         st[D.ls + 8] = soft_count; st[D.ls + 9] = tiny_last; st[D.ls + 10] = tiny_flag;
         st[D.ls + 11] = mu_free; st[D.ls + 12] = mu_max; st[D.ls + 13] = nhist;
         for (int q = 0; q < 4; ++q) st[D.ls + 14 + q] = hist[q];
+        st[D.ls + 18] = acc_count;
     }
     if (wd_active) {
         const int nw = pb->n + 2 * pb->m;

@@ -17,6 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libjipm.so")
 TRACE_W = 22
 ST_NOT_RUN, ST_SOLVED, ST_MAXITER, ST_LOCALLY_INFEASIBLE = -1, 0, 1, 2
 ST_RESTORATION_FAILED, ST_RESTO_AT_FEASIBLE_POINT, ST_NONFINITE, ST_TINY_STEP = 3, 4, 5, 6
+ST_ACCEPTABLE = 7
 
 _DOUBLE_FIELDS = [
     "tol", "mu_init", "kappa_eps", "kappa_mu", "theta_mu", "tau_min", "s_max", "kappa_sigma",
@@ -27,11 +28,12 @@ _DOUBLE_FIELDS = [
     "delta_c_bar", "kappa_c", "residual_ratio_max", "rho_resto", "kappa_resto", "z_reset_threshold",
     "residual_ratio_singular", "residual_improvement_factor",
     "tiny_step_tol", "tiny_step_y_tol", "tiny_step_cviol", "soft_resto_factor",
-    "adaptive_red_fact", "adaptive_monotone_init", "adaptive_sigma_max", "adaptive_mu_max_fact"]
+    "adaptive_red_fact", "adaptive_monotone_init", "adaptive_sigma_max", "adaptive_mu_max_fact",
+    "acceptable_tol", "acceptable_dual_inf_tol", "acceptable_constr_viol_tol", "acceptable_compl_inf_tol"]
 _INT_FIELDS = ["max_iter", "max_backtrack", "max_soc", "refine_min", "refine_max", "max_mu_updates",
                "init_slacks", "enable_restoration", "watchdog_trigger", "watchdog_trial_max", "max_soft_resto_iters",
-               "mu_strategy", "adaptive_red_iters"]
-_INT_LAYOUT = _INT_FIELDS[:-2] + ["polish_max"] + _INT_FIELDS[-2:]   # order of the int32 members in jipm_options
+               "mu_strategy", "adaptive_red_iters", "acceptable_iter"]
+_INT_LAYOUT = _INT_FIELDS[:-3] + ["polish_max"] + _INT_FIELDS[-3:]   # order of the int32 members in jipm_options
 
 
 class Options(C.Structure):

@@ -411,6 +411,7 @@ def snapshot_state(lay, st, n, m):
     snap[lay["ls"] + 11:lay["ls"] + 14] = [int(cur.mu_free), cur.mu_max, len(hist)]
     for j in range(max(0, len(hist) - 4), len(hist)):
         snap[lay["ls"] + 14 + (j & 3)] = hist[j]
+    snap[lay["ls"] + 18] = cur.acc_count
     if wd is not None:
         nw, o = n + 2 * m, lay["wd"]
         for q, v in enumerate((wd.x, wd.zL, wd.zU, wd.d[0], wd.d[2], wd.d[3])):
@@ -421,7 +422,7 @@ def snapshot_state(lay, st, n, m):
 
 
 def ls_memory(st):
-    """(n_short, watchdog active, watchdog trials, soft, soft_count, tiny_last, tiny_flag) of the active problem."""
+    """(n_short, watchdog active, watchdog trials, soft, soft_count, tiny_last, tiny_flag, acceptable count) of the active problem."""
     cur = st if st.resto is None else st.resto.state
     return [cur.n_short, int(cur.wd is not None), cur.wd.trials if cur.wd else 0, int(cur.soft), cur.soft_count,
-            int(cur.tiny_last), int(cur.tiny_flag)]
+            int(cur.tiny_last), int(cur.tiny_flag), cur.acc_count]
