@@ -122,7 +122,7 @@ int jipm_destroy(jipm_solver* s);
  *   P, x0, params, x_out, lam_out, zL_out, zU_out, status_out, iters_out (all DEVICE): as in jipm_solve_batch.
  * Results are bit-identical to jipm_create + jipm_solve_batch with the same arguments.  Returns after the work has
  * completed.  A family whose workspaces do not fit the array (n > 8192, or more than JIPM_STATIC_SCRATCH_BYTES of
- * scratch: C2 and C3 of BASELINE.json do not fit, C0, C1 and workload 5 do) -> JIPM_ERR_NOMEM with the sizes in
+ * scratch: C0 and C1 of BASELINE.json fit (C1: 45 MB); workload 5 (81 MB), C3 (198 MB) and C2 (504 MB) do not) -> JIPM_ERR_NOMEM with the sizes in
  * jipm_last_error; nothing is launched.
  * Every call on a device shares the one array, which keeps the previous call's contents (the call clears what must
  * start at zero): calls that overlap on the GPU -- other host threads are serialised by the library, other PROCESSES
